@@ -1,0 +1,150 @@
+"""Pins for the oracle's energy, ground-state rule and generators (oracle_energy, oracle_enumerate,
+oracle_enumerate_seqs, oracle_seeded_*).  PAPER.md:67-69 (Eq. 1), :77-79 (Table 1), :81 (unique minimum,
+threshold), :552-575 (min / second-min scan, gap output)."""
+import numpy as np
+import pytest
+
+from oracle import gp_oracle as orc
+from tests import _bruteforce as bf
+from tests._golden import read_3x3_fixture, read_whole_maps
+
+HP = list(orc.HP_ENERGIES)
+NULL = orc.NULL_PHENO
+
+
+def bits(g, n):
+    return [(g >> i) & 1 for i in range(n)]
+
+
+def test_hp_table_is_the_papers():
+    # PAPER.md:77-79 Table 1 x10, letter 1 = H (reading R3); listing :519-525 has -23/-10/-10/0
+    assert HP[1 * 2 + 1] == -23 and HP[0 * 2 + 1] == HP[1 * 2 + 0] == -10 and HP[0] == 0
+
+
+def test_worked_energies_3x3(oracle_structures):
+    S = oracle_structures(3, 3)
+    for w in read_3x3_fixture()["genotypes"]:
+        assert [S.energy(d, bits(w["g"], 9), HP) for d in range(S.D)] == w["energies"]
+        ph, gap = S.enumerate(w["g"], 1)
+        assert ph[0] == (NULL if w["pheno"] is None else w["pheno"])
+        e = sorted(w["energies"])
+        assert gap[0] == e[0] - e[1]
+
+
+@pytest.mark.parametrize("dims", [(3, 3, 1), (4, 4, 1), (5, 5, 1), (2, 2, 2), (3, 3, 3), (6, 6, 1)])
+def test_closed_form_energies(oracle_structures, dims):
+    """all-H -> -23*NBP, all-P -> 0, alternating -> -10*NBP (every contact joins opposite parities),
+    single H at k -> -10 * (#contacts of monomer k); all of these are null when D >= 2."""
+    S = oracle_structures(*dims)
+    n = S.N
+    ds = range(0, S.D, max(1, S.D // 300))
+    alt = [i & 1 for i in range(n)]
+    for d in ds:
+        assert S.energy(d, [1] * n, HP) == -23 * S.NBP
+        assert S.energy(d, [0] * n, HP) == 0
+        assert S.energy(d, alt, HP) == -10 * S.NBP
+    _, contacts, _ = S.get(S.D // 2)
+    for k in (0, 1, n // 2, n - 1):
+        one = [int(i == k) for i in range(n)]
+        assert S.energy(S.D // 2, one, HP) == -10 * int((contacts == k).sum())
+    full = (1 << n) - 1
+    altg = sum(1 << i for i in range(1, n, 2))
+    for g in (0, full, altg):
+        ph, gap = S.enumerate(g, 1)
+        assert ph[0] == NULL and gap[0] == 0
+
+
+@pytest.mark.parametrize("dims", [(3, 3, 1), (3, 2, 1), (2, 2, 2)])
+def test_full_map_equals_bruteforce(oracle_structures, dims):
+    S = oracle_structures(*dims)
+    _, _, class_of, _, coords = bf.classify(dims)
+    ph, gap = S.enumerate(0, 1 << S.N)
+    for g in range(1 << S.N):
+        want, wgap = bf.ground_state(coords, class_of, bits(g, S.N), HP, 2)
+        assert ph[g] == (NULL if want is None else want), g
+        assert gap[g] == wgap
+
+
+def test_sampled_4x4_and_20_letters_equal_bruteforce(oracle_structures):
+    S = oracle_structures(4, 4)
+    _, _, class_of, _, coords = bf.classify((4, 4, 1))
+    rng = np.random.default_rng(5612)
+    for g in rng.integers(0, 1 << 16, 150).tolist():
+        want, wgap = bf.ground_state(coords, class_of, bits(g, 16), HP, 2)
+        ph, gap = S.enumerate(g, 1)
+        assert ph[0] == (NULL if want is None else want) and gap[0] == wgap
+    M = rng.integers(-750, -49, (20, 20))
+    M = np.minimum(M, M.T).astype(np.int32)
+    seqs = rng.integers(0, 20, (60, 16)).astype(np.uint8)
+    ph, gap = S.enumerate_seqs(seqs, M.reshape(-1), 20)
+    for n in range(60):
+        want, wgap = bf.ground_state(coords, class_of, seqs[n].tolist(), M.reshape(-1).tolist(), 20)
+        assert ph[n] == (NULL if want is None else want) and gap[n] == wgap
+
+
+def test_whole_maps_and_invariants(oracle_structures):
+    maps = read_whole_maps()
+    fx = read_3x3_fixture()
+    for name, dims in (("3x3", (3, 3, 1)), ("4x4", (4, 4, 1))):
+        S = oracle_structures(*dims)
+        n = S.N
+        ph = S.enumerate(0, 1 << n, want_gap=False)
+        hist = orc.designability(ph, S.C)
+        assert int(hist.sum()) == 1 << n                                    # sum rule
+        assert (int(hist[:-1].sum()), int(hist[-1])) == (maps[name]["folding"], maps[name]["null"])
+        assert sorted(hist[:-1].tolist(), reverse=True)[:5] == maps[name]["top5"][:5]
+        g = np.arange(1 << n)
+        rev = np.zeros_like(g)
+        for i in range(n):
+            rev |= ((g >> i) & 1) << (n - 1 - i)
+        assert (ph[rev] == ph).all()                                        # pheno(rev g) = pheno(g)
+        if name == "3x3":
+            assert hist.tolist() == fx["hist"] + [fx["null"]]
+
+
+def test_edge_single_structure_and_thresholds(oracle_structures):
+    S = oracle_structures(2, 2)                       # D = 1: every sequence folds under the true rule (R6)
+    ph, gap = S.enumerate(0, 16)
+    assert (ph == 0).all() and (gap == -32768).all()
+    S = oracle_structures(4, 4)
+    ph1, gap = S.enumerate(0, 1 << 16)
+    assert ((gap <= 0).all() and ((gap < 0) == (ph1 != NULL)).all())
+    for thr in (2, 3, 10, 24):
+        ph = S.enumerate(0, 1 << 16, threshold=thr, want_gap=False)
+        assert ((ph != NULL) == (-gap >= thr)).all()
+        assert (ph[ph != NULL] == ph1[ph != NULL]).all()
+    sub, subgap = S.enumerate(12345, 777)               # ranges are slices of the full map
+    assert (sub == ph1[12345:12345 + 777]).all() and (subgap == gap[12345:12345 + 777]).all()
+
+
+def test_hp_embedded_in_20_letters(oracle_structures):
+    """Letters 0-9 = P, 10-19 = H with HP energies must reproduce the 2-letter map (same path, wider alphabet)."""
+    S = oracle_structures(4, 4)
+    rng = np.random.default_rng(11)
+    seqs = rng.integers(0, 20, (3000, 16)).astype(np.uint8)
+    hp = (seqs >= 10).astype(np.int64)
+    M = np.array([[HP[(a >= 10) * 2 + (b >= 10)] for b in range(20)] for a in range(20)], np.int32)
+    ph20, gap20 = S.enumerate_seqs(seqs, M.reshape(-1), 20)
+    full, fullgap = S.enumerate(0, 1 << 16)
+    g = (hp << np.arange(16)).sum(1)
+    assert (ph20 == full[g]).all() and (gap20 == fullgap[g]).all()
+    ph2 = S.enumerate_seqs(hp.astype(np.uint8), HP, 2, want_gap=False)
+    assert (ph2 == full[g]).all()
+
+
+def test_generator():
+    # splitmix64 reference stream for seed 0 (public-domain reference implementation's well-known first outputs)
+    assert [orc.draw(0, c) for c in range(3)] == [0xE220A8397B1DCDAF, 0x6E789E6AA1B965F4, 0x06C45D188009454F]
+    seqs = orc.seeded_sequences(200805612, 0, 40000, 16)
+    assert seqs.max() == 19 and seqs.min() == 0
+    counts = np.bincount(seqs.reshape(-1), minlength=20)
+    chi2 = float(((counts - counts.mean()) ** 2 / counts.mean()).sum())
+    assert chi2 < 50.0                                    # 19 dof: P(chi2 > 50) ~ 1e-4
+    again = orc.seeded_sequences(200805612, 1000, 10, 16)
+    assert (again == seqs[1000:1010]).all()               # counter-based: ranges are slices
+    u = orc.draw(200805612, 5 * 16 + 3)
+    assert seqs[5, 3] == ((u >> 32) * 20) >> 32
+    M = orc.seeded_matrix(200805612)
+    assert (M == M.T).all() and M.min() >= -750 and M.max() <= -50 and len(np.unique(M)) > 100
+    u = orc.draw(200805612, (1 << 62) + 3 * 20 + 7)
+    assert M[3, 7] == -750 + (((u >> 32) * 701) >> 32)
