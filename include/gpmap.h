@@ -1,0 +1,123 @@
+/* gpmap.h — C ABI of libgpmap: exhaustive HP-model genotype-phenotype map on one B200 (sm_100a).
+ *
+ * What is computed follows arXiv 2008.05612 (citations are PAPER.md:LINE; readings R1.. are DESIGN.md section 2):
+ *   fold library  = all compact self-avoiding walks of a box, one per symmetry class          (:65, :654-694)
+ *   energy        = H = sum_{i<j} E[s_i][s_j] Delta(r_i - r_j), Delta = lattice but not chain neighbours (:67-69, Eq. 1)
+ *   phenotype     = the unique minimum-energy fold, else "does not fold" (null)               (:81, :552-575)
+ *   designability = number of genotypes per phenotype                                         (:138)
+ *   robustness    = one-point-mutation neighbourhood counts, Eq. 2                            (:138-147)
+ *   neutral nets  = connected same-phenotype genotype sets                                    (:19)
+ *
+ * Conventions
+ *   - Every call returns a gp_status; nothing throws or exits across the ABI (the paper's gpuAssert exits, :470-485).
+ *   - Pointers named d_* are DEVICE pointers, allocated and freed by the caller.  Pointers without the prefix are HOST
+ *     pointers.  The library owns only the opaque gp_structures_t handle (its device tables included) and a private
+ *     scratch it frees in gp_structures_free.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = default stream).  Compute calls are asynchronous on it; a
+ *     non-zero status reports argument or launch errors only.  Device output arrays are fully overwritten.
+ *   - Genotype g: bit i of g is the letter of monomer i, 1 = H (R3).  Null phenotype = GP_NULL_PHENO (R7).
+ *   - Phenotype ids are reversal-reduced class ids 0..C-1 in the canonical order of DESIGN.md section 3 (R1, R8).
+ */
+#ifndef GPMAP_H
+#define GPMAP_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define GP_NULL_PHENO 0xFFFFu
+#define GP_GAP_NONE (-32768) /* gap reported when there is no second structure (D = 1), R6 */
+
+typedef enum {
+    GP_OK = 0,
+    GP_INVALID_ARG = 1,         /* null pointer, bad alphabet, asymmetric or out-of-range energies, threshold < 1 */
+    GP_UNSUPPORTED_LATTICE = 2, /* box with fewer than 2 or more than 64 sites, or more classes than a u16 holds */
+    GP_OUT_OF_MEMORY = 3,
+    GP_CUDA_ERROR = 4,          /* gp_last_cuda_error() has the CUDA text */
+    GP_RANGE = 5                /* genotype range outside [0, 2^N) or not aligned to gp_tile() */
+} gp_status;
+
+typedef struct gp_structures_s gp_structures_t; /* opaque */
+
+/* Contact energies (PAPER.md:77-79 Table 1, integer units :132, :519-525).  e is a HOST array, alphabet*alphabet,
+ * row-major, symmetric.  alphabet = 2: e = {E_PP, E_HP, E_HP, E_HH} (HP x10: 0,-10,-10,-23).  alphabet = 20: 0.01 units.
+ * A sequence folds iff second_min - min >= threshold (threshold >= 1; 1 = strict uniqueness, R5). */
+typedef struct {
+    int32_t alphabet;
+    const int32_t* e;
+    int32_t threshold;
+} gp_energies;
+
+/* a0. Host setup: enumerate the Hamiltonian walks of the nx x ny x nz box (nz = 1 for 2D), keep one per
+ * point-group class (D directed structures), pair each with its chain reversal (C classes), build contact tables and
+ * upload them to the current CUDA device.  With no CUDA device the handle is host-only: the queries below work and
+ * compute calls return GP_CUDA_ERROR.  *out is set to NULL on error. */
+gp_status gp_structures(int nx, int ny, int nz, gp_structures_t** out);
+void gp_structures_free(gp_structures_t* s);
+int gp_structures_length(const gp_structures_t* s);            /* N, chain length                       */
+uint32_t gp_structures_directed(const gp_structures_t* s);     /* D, scored structures                  */
+uint32_t gp_structures_classes(const gp_structures_t* s);      /* C, phenotype ids are 0..C-1           */
+uint32_t gp_structures_self_reverse(const gp_structures_t* s); /* classes equal to their own reversal   */
+uint64_t gp_structures_walks(const gp_structures_t* s);        /* directed Hamiltonian walks = D * |G|  */
+int gp_structures_contacts_per_fold(const gp_structures_t* s); /* NBP = #edges - (N-1)                  */
+int gp_structures_features(const gp_structures_t* s);          /* K = N + P: columns of the contraction */
+/* Directed structure d: sites[N] (site = x + nx*(y + ny*z)), contacts[2*NBP] monomer pairs i<j, class id.  HOST out
+ * arrays, each nullable.  GP_RANGE if d >= D. */
+gp_status gp_structures_get(const gp_structures_t* s, uint32_t d, uint8_t* sites, uint8_t* contacts, uint16_t* class_id);
+
+/* Genotype-range granularity of gp_enumerate (g_begin must be a multiple of it). */
+uint64_t gp_tile(void);
+
+/* a1-a4. Score genotypes g_begin .. g_begin+g_count-1 (alphabet 2, implicit) on all D directed structures
+ * (Eq. 1, :67-69; :530-545), take min / second min / argmin (:552-567) and write d_pheno[g - g_begin] = class of the
+ * argmin if second_min - min >= threshold else GP_NULL_PHENO (:81, :573), and, if d_gap is not NULL,
+ * d_gap[g - g_begin] = min - second_min (:575; GP_GAP_NONE when D = 1).  The energy matrix never reaches HBM.
+ * Runs the tcgen05 int8 contraction.  Errors: GP_INVALID_ARG (energies outside the int8 weight bound, asymmetric),
+ * GP_RANGE. */
+gp_status gp_enumerate(const gp_structures_t* s, const gp_energies* en, uint64_t g_begin, uint64_t g_count,
+                       uint16_t* d_pheno, int16_t* d_gap, void* stream);
+
+/* Same contract as gp_enumerate, computed by the plain CUDA-core kernel that walks the contact table like the paper's
+ * listing (:530-570).  Kept as the in-library cross-check and timing strawman; no alignment requirement. */
+gp_status gp_enumerate_simple(const gp_structures_t* s, const gp_energies* en, uint64_t g_begin, uint64_t g_count,
+                              uint16_t* d_pheno, int16_t* d_gap, void* stream);
+
+/* a8. Explicit sequences (the paper's SeqRnd path, :510-516, :762-775): d_seqs[count][N] letters < alphabet (2 or 20). */
+gp_status gp_enumerate_seqs(const gp_structures_t* s, const gp_energies* en, const uint8_t* d_seqs, uint64_t count,
+                            uint16_t* d_pheno, int16_t* d_gap, void* stream);
+/* a8. Sequences first..first+count-1 of the counter-based 20-letter generator of DESIGN.md section 4, drawn on chip. */
+gp_status gp_enumerate_seeded(const gp_structures_t* s, const gp_energies* en, uint64_t seed, uint64_t first,
+                              uint64_t count, uint16_t* d_pheno, int16_t* d_gap, void* stream);
+/* Host helpers for the same generator: the seeded 20x20 matrix and sequences. */
+gp_status gp_seeded_matrix(uint64_t seed, int32_t* m400);
+gp_status gp_seeded_sequences(uint64_t seed, uint64_t first, uint64_t count, int n, uint8_t* seqs);
+
+/* a5. Designability (:138): d_hist[c] = #{g : d_pheno[g] = c} for c < n_classes, d_hist[n_classes] = #null. */
+gp_status gp_designability(const uint16_t* d_pheno, uint64_t count, uint32_t n_classes, uint64_t* d_hist, void* stream);
+
+/* a6. One-point-mutation neighbourhood (:138-147, Eq. 2) over the FULL store of 2^n_bits entries.  For every non-null
+ * g of class p and each of the n_bits flips, q = d_pheno[g ^ (1 << k)]: d_neutral[p] += (q == p),
+ * d_deleterious[p] += (q null), d_other[p] += (q another class).  If d_pair_count is not NULL it receives the number
+ * of unordered pairs of distinct non-null classes joined by at least one mutation (R11).  rho_p = neutral[p] /
+ * (n_bits * hist[p]) etc. are host divisions (R9). */
+gp_status gp_robustness(const uint16_t* d_pheno, int n_bits, uint32_t n_classes, uint64_t* d_neutral,
+                        uint64_t* d_deleterious, uint64_t* d_other, uint64_t* d_pair_count, void* stream);
+
+/* a7. Neutral-network components (:19, R12): d_ncomp[p] = number of connected components of {g : pheno = p} under
+ * single-bit flips.  Needs 4 bytes of private scratch per genotype; n_bits <= 30.  Synchronises the stream. */
+gp_status gp_nn_components(const uint16_t* d_pheno, int n_bits, uint32_t n_classes, uint32_t* d_ncomp, void* stream);
+
+/* Whole hot path from HOST buffers (the end-to-end call): enumerate [g_begin, g_begin+g_count), copy phenotypes to
+ * pheno (host, nullable) and the histogram to hist (host, n_classes+1).  Synchronous. */
+gp_status gp_enumerate_host(const gp_structures_t* s, const gp_energies* en, uint64_t g_begin, uint64_t g_count,
+                            uint16_t* pheno, uint64_t* hist);
+
+const char* gp_strerror(gp_status st);
+const char* gp_last_cuda_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GPMAP_H */

@@ -1,0 +1,171 @@
+// api.cu — C-ABI entry points of libgpmap (include/gpmap.h): argument checks, handle lifetime, dispatch to the kernels.
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "device_common.cuh"
+
+static thread_local char g_cuda_error[512] = "";
+
+void gp_set_cuda_error(cudaError_t e, const char* where) {
+    snprintf(g_cuda_error, sizeof(g_cuda_error), "%s: %s (%s)", cudaGetErrorName(e), cudaGetErrorString(e), where);
+}
+
+extern "C" const char* gp_last_cuda_error(void) { return g_cuda_error; }
+
+extern "C" const char* gp_strerror(gp_status st) {
+    switch (st) {
+        case GP_OK: return "ok";
+        case GP_INVALID_ARG: return "invalid argument";
+        case GP_UNSUPPORTED_LATTICE: return "unsupported lattice";
+        case GP_OUT_OF_MEMORY: return "out of memory";
+        case GP_CUDA_ERROR: return "CUDA error (see gp_last_cuda_error)";
+        case GP_RANGE: return "genotype range or index out of range / misaligned";
+    }
+    return "unknown status";
+}
+
+gp_status gp_upload_tables(gp_structures_s* s) {
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        s->device = -1;  // host-only handle
+        return GP_OK;
+    }
+    GP_CUDA(cudaGetDevice(&s->device));
+    GP_CUDA(cudaMalloc(&s->d_contacts, s->contacts.size()));
+    GP_CUDA(cudaMemcpy(s->d_contacts, s->contacts.data(), s->contacts.size(), cudaMemcpyHostToDevice));
+    GP_CUDA(cudaMalloc(&s->d_class_of, s->class_of.size() * sizeof(uint16_t)));
+    GP_CUDA(cudaMemcpy(s->d_class_of, s->class_of.data(), s->class_of.size() * sizeof(uint16_t), cudaMemcpyHostToDevice));
+    std::vector<uint16_t> pidx(s->contacts.size() / 2);
+    for (size_t k = 0; k < pidx.size(); k++)
+        pidx[k] = (uint16_t)s->pair_index[(size_t)s->contacts[2 * k] * s->N + s->contacts[2 * k + 1]];
+    GP_CUDA(cudaMalloc(&s->d_pairidx, pidx.size() * sizeof(uint16_t)));
+    GP_CUDA(cudaMemcpy(s->d_pairidx, pidx.data(), pidx.size() * sizeof(uint16_t), cudaMemcpyHostToDevice));
+    std::vector<uint8_t> ij((size_t)s->P * 2);
+    for (int i = 0; i < s->N; i++)
+        for (int j = 0; j < s->N; j++) {
+            int p = s->pair_index[(size_t)i * s->N + j];
+            if (p >= 0) { ij[2 * p] = (uint8_t)i; ij[2 * p + 1] = (uint8_t)j; }
+        }
+    GP_CUDA(cudaMalloc(&s->d_pair_ij, ij.size()));
+    GP_CUDA(cudaMemcpy(s->d_pair_ij, ij.data(), ij.size(), cudaMemcpyHostToDevice));
+    return GP_OK;
+}
+
+void gp_release_device(gp_structures_s* s) {
+    if (s->device < 0) return;
+    cudaFree(s->d_contacts);
+    cudaFree(s->d_class_of);
+    cudaFree(s->d_pairidx);
+    cudaFree(s->d_pair_ij);
+    cudaFree(s->wimg.d_img);
+    cudaFree(s->d_scratch);
+    s->d_contacts = nullptr; s->d_class_of = nullptr; s->d_pairidx = nullptr; s->d_pair_ij = nullptr; s->wimg.d_img = nullptr; s->d_scratch = nullptr;
+}
+
+extern "C" gp_status gp_structures(int nx, int ny, int nz, gp_structures_t** out) {
+    if (!out) return GP_INVALID_ARG;
+    *out = nullptr;
+    gp_structures_s* s = new (std::nothrow) gp_structures_s();
+    if (!s) return GP_OUT_OF_MEMORY;
+    gp_status st;
+    try {
+        st = gp_build_host_tables(nx, ny, nz, s);
+    } catch (const std::bad_alloc&) {
+        st = GP_OUT_OF_MEMORY;
+    }
+    if (st == GP_OK) st = gp_upload_tables(s);
+    if (st != GP_OK) {
+        gp_release_device(s);
+        delete s;
+        return st;
+    }
+    *out = s;
+    return GP_OK;
+}
+
+extern "C" void gp_structures_free(gp_structures_t* s) {
+    if (!s) return;
+    gp_release_device(s);
+    delete s;
+}
+
+extern "C" int gp_structures_length(const gp_structures_t* s) { return s ? s->N : 0; }
+extern "C" uint32_t gp_structures_directed(const gp_structures_t* s) { return s ? s->D : 0; }
+extern "C" uint32_t gp_structures_classes(const gp_structures_t* s) { return s ? s->C : 0; }
+extern "C" uint32_t gp_structures_self_reverse(const gp_structures_t* s) { return s ? s->n_self_reverse : 0; }
+extern "C" uint64_t gp_structures_walks(const gp_structures_t* s) { return s ? (uint64_t)s->D * (uint64_t)s->group : 0; }
+extern "C" int gp_structures_contacts_per_fold(const gp_structures_t* s) { return s ? s->NBP : 0; }
+extern "C" int gp_structures_features(const gp_structures_t* s) { return s ? s->K : 0; }
+
+extern "C" gp_status gp_structures_get(const gp_structures_t* s, uint32_t d, uint8_t* sites, uint8_t* contacts,
+                                       uint16_t* class_id) {
+    if (!s) return GP_INVALID_ARG;
+    if (d >= s->D) return GP_RANGE;
+    if (sites) memcpy(sites, &s->walks[(size_t)d * s->N], s->N);
+    if (contacts) memcpy(contacts, &s->contacts[(size_t)d * s->NBP * 2], (size_t)s->NBP * 2);
+    if (class_id) *class_id = s->class_of[d];
+    return GP_OK;
+}
+
+// alphabet-2 energies -> (a, lin, quad); bounds so that every weight fits int8 and every energy fits the packed key
+gp_status gp_check_hp(const gp_structures_s* s, const gp_energies* en, gp_hp_params* out) {
+    if (!s || !en || !en->e || en->alphabet != 2 || en->threshold < 1) return GP_INVALID_ARG;
+    const int32_t a = en->e[0], b = en->e[1], b2 = en->e[2], c = en->e[3];
+    if (b != b2) return GP_INVALID_ARG;
+    if (a < -10000 || a > 10000 || b < -10000 || b > 10000 || c < -10000 || c > 10000) return GP_INVALID_ARG;
+    int32_t lin = b - a, quad = c - 2 * b + a;
+    // a monomer has at most 5 contacts on a cubic lattice (6 neighbours minus one chain bond), 3 in 2D
+    int cmax = (s->nz > 1 && s->ny > 1 && s->nx > 1) ? 5 : 3;
+    if (lin * cmax > 127 || lin * cmax < -127 || quad > 127 || quad < -127) return GP_INVALID_ARG;
+    long long bound = (long long)s->NBP * (2LL * (lin < 0 ? -lin : lin) + (quad < 0 ? -quad : quad));
+    if (bound >= 8192) return GP_INVALID_ARG;
+    out->a = a; out->lin = lin; out->quad = quad; out->threshold = en->threshold;
+    return GP_OK;
+}
+
+extern "C" gp_status gp_seeded_matrix(uint64_t seed, int32_t* m400) {
+    if (!m400) return GP_INVALID_ARG;
+    for (int a = 0; a < 20; a++)
+        for (int b = a; b < 20; b++) {
+            uint64_t u = gp_draw(seed, (1ULL << 62) + (uint64_t)(20 * a + b));
+            int32_t v = -750 + (int32_t)(((u >> 32) * 701) >> 32);
+            m400[20 * a + b] = m400[20 * b + a] = v;
+        }
+    return GP_OK;
+}
+
+extern "C" gp_status gp_seeded_sequences(uint64_t seed, uint64_t first, uint64_t count, int n, uint8_t* seqs) {
+    if (!seqs || n < 1 || n > 64) return GP_INVALID_ARG;
+    for (uint64_t q = 0; q < count; q++)
+        for (int k = 0; k < n; k++) seqs[q * n + k] = (uint8_t)gp_letter20(seed, first + q, k);
+    return GP_OK;
+}
+
+// End-to-end call from host buffers: device store allocated here, phenotypes and histogram copied back.
+extern "C" gp_status gp_enumerate_host(const gp_structures_t* s, const gp_energies* en, uint64_t g_begin,
+                                       uint64_t g_count, uint16_t* pheno, uint64_t* hist) {
+    if (!s || !hist) return GP_INVALID_ARG;
+    if (s->device < 0) { gp_set_cuda_error(cudaErrorNoDevice, "handle has no device tables"); return GP_CUDA_ERROR; }
+    const uint32_t C = s->C;
+    uint16_t* d_pheno = nullptr;
+    uint64_t* d_hist = nullptr;
+    GP_CUDA(cudaMalloc(&d_pheno, (g_count ? g_count : 1) * sizeof(uint16_t)));
+    if (cudaMalloc(&d_hist, ((size_t)C + 1) * sizeof(uint64_t)) != cudaSuccess) {
+        cudaFree(d_pheno);
+        gp_set_cuda_error(cudaGetLastError(), "cudaMalloc(hist)");
+        return GP_OUT_OF_MEMORY;
+    }
+    gp_status st = gp_enumerate(s, en, g_begin, g_count, d_pheno, nullptr, nullptr);
+    if (st == GP_OK) st = gp_designability(d_pheno, g_count, C, d_hist, nullptr);
+    if (st == GP_OK) {
+        cudaError_t e = cudaSuccess;
+        if (pheno && g_count) e = cudaMemcpy(pheno, d_pheno, g_count * sizeof(uint16_t), cudaMemcpyDeviceToHost);
+        if (e == cudaSuccess) e = cudaMemcpy(hist, d_hist, ((size_t)C + 1) * sizeof(uint64_t), cudaMemcpyDeviceToHost);
+        if (e != cudaSuccess) { gp_set_cuda_error(e, "gp_enumerate_host copy-back"); st = GP_CUDA_ERROR; }
+    }
+    cudaFree(d_pheno);
+    cudaFree(d_hist);
+    return st;
+}

@@ -1,0 +1,43 @@
+// device_common.cuh — error plumbing and small helpers shared by libgpmap's .cu files (private; not used by oracle/).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "gpmap_internal.h"
+
+void gp_set_cuda_error(cudaError_t e, const char* where);
+
+#define GP_CUDA(call)                                 \
+    do {                                              \
+        cudaError_t e_ = (call);                      \
+        if (e_ != cudaSuccess) {                      \
+            gp_set_cuda_error(e_, #call);             \
+            return e_ == cudaErrorMemoryAllocation ? GP_OUT_OF_MEMORY : GP_CUDA_ERROR; \
+        }                                             \
+    } while (0)
+
+// Validated alphabet-2 energies in the form the kernels use:
+//   E(g,S) = a*NBP + lin * sum_k c_k(S) h_k + quad * #HH-contacts,  lin = b - a, quad = c - 2b + a
+struct gp_hp_params {
+    int32_t a, lin, quad, threshold;
+};
+gp_status gp_check_hp(const gp_structures_s* s, const gp_energies* en, gp_hp_params* out);
+
+// 64-bit counter-based generator of DESIGN.md section 4 (splitmix finaliser)
+__host__ __device__ inline uint64_t gp_mix64(uint64_t z) {
+    z ^= z >> 30; z *= 0xBF58476D1CE4E5B9ULL;
+    z ^= z >> 27; z *= 0x94D049BB133111EBULL;
+    z ^= z >> 31;
+    return z;
+}
+__host__ __device__ inline uint64_t gp_draw(uint64_t seed, uint64_t ctr) {
+    return gp_mix64(seed + (ctr + 1) * 0x9E3779B97F4A7C15ULL);
+}
+__host__ __device__ inline uint32_t gp_letter20(uint64_t seed, uint64_t seq, int k) {
+    uint64_t u = gp_draw(seed, seq * 16 + (uint64_t)k);
+    return (uint32_t)(((u >> 32) * 20) >> 32);
+}
+
+// scoring_tc.cu
+gp_status gp_launch_scoring_tc(gp_structures_s* s, const gp_hp_params& hp, uint64_t g_begin, uint64_t g_count,
+                               uint16_t* d_pheno, int16_t* d_gap, cudaStream_t st);

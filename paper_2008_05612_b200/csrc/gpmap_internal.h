@@ -1,0 +1,42 @@
+// gpmap_internal.h — private to libgpmap (host setup + CUDA kernels).  Not part of the ABI, not used by oracle/.
+#pragma once
+#include <stdint.h>
+
+#include <vector>
+
+#include "gpmap.h"
+
+// Cached device image of the weight matrix W for one (b-a, c-2b+a) pair, in the tile layout the tcgen05 kernel
+// bulk-copies into shared memory (see scoring_tc.cu).
+struct gp_weight_image {
+    int32_t lin = 0, quad = 0;  // (b-a), (c-2b+a): weight of a monomer feature per contact, of a pair feature
+    bool valid = false;
+    int8_t* d_img = nullptr;    // [n_tiles][k_blocks][TILE_N rows][128 B], 128B-swizzled
+    uint32_t n_tiles = 0, k_blocks = 0;
+};
+
+struct gp_structures_s {
+    int nx = 0, ny = 0, nz = 0;
+    int N = 0, NBP = 0, group = 0;
+    uint32_t D = 0, C = 0, n_self_reverse = 0;
+    int P = 0, K = 0;                    // pair features, total features N + P
+    std::vector<uint8_t> walks;          // D * N site indices
+    std::vector<uint8_t> contacts;       // D * NBP * 2 monomer indices, i < j
+    std::vector<uint16_t> class_of;      // D
+    std::vector<int16_t> pair_index;     // N * N -> index into the P pair features, -1 if (i,j) can never touch
+    // device side (null when no CUDA device)
+    int device = -1;
+    uint8_t* d_contacts = nullptr;
+    uint16_t* d_class_of = nullptr;
+    uint16_t* d_pairidx = nullptr;       // D * NBP: pair-feature index of each contact
+    uint8_t* d_pair_ij = nullptr;        // P * 2: monomers (i, j) of each pair feature
+    gp_weight_image wimg;
+    void* d_scratch = nullptr;           // private scratch, grown on demand
+    size_t scratch_bytes = 0;
+};
+
+// host_structures.cpp
+gp_status gp_build_host_tables(int nx, int ny, int nz, gp_structures_s* s);
+// device.cu
+gp_status gp_upload_tables(gp_structures_s* s);
+void gp_release_device(gp_structures_s* s);

@@ -1,0 +1,151 @@
+// scoring_simple.cu — CUDA-core scorer for any alphabet: gp_enumerate_simple (implicit HP genotypes, the in-library
+// cross-check of the tensor-core path), gp_enumerate_seqs (the paper's SeqRnd path) and
+// gp_enumerate_seeded (20-letter variant, a8).
+//
+// One thread per sequence, like the paper's kernel (:193, :487-578), but the per-contact matrix look-up of the
+// listing (:537-545) is hoisted: each thread first gathers the energies of all P monomer pairs that can ever touch
+// (pe[p] = e[s_i][s_j], staged in shared memory, 20x20 matrix in shared memory too), then a structure is an NBP-term
+// sum of pe[] entries addressed by the structure's pair indices, which all threads of a block read as broadcasts.
+// min / second-min / argmin use the strict '<' updates of :552-567 with true-minimum initialisation (R6).
+#include "device_common.cuh"
+
+namespace {
+
+enum { SRC_BITS = 0, SRC_SEQS = 1, SRC_SEEDED = 2 };
+constexpr int CHUNK = 256;  // structures staged per shared-memory refill
+
+struct SimpleArgs {
+    const uint16_t* pairidx;  // D * NBP
+    const uint8_t* pair_ij;   // P * 2
+    const uint16_t* class_of;
+    const uint8_t* seqs;
+    uint16_t* pheno;
+    int16_t* gap;
+    uint64_t first, count, seed;
+    uint32_t D;
+    int N, NBP, P, alphabet, threshold;
+};
+
+template <int SRC>
+__global__ void __launch_bounds__(128) score_simple_kernel(SimpleArgs a, const int16_t* __restrict__ e_dev) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int BD = blockDim.x, tid = threadIdx.x;
+    int16_t* pe = reinterpret_cast<int16_t*>(smem_raw);                  // [P][BD]
+    uint16_t* sidx = reinterpret_cast<uint16_t*>(pe + (size_t)a.P * BD);  // [CHUNK][NBP]
+    int16_t* em = reinterpret_cast<int16_t*>(sidx + (size_t)CHUNK * a.NBP);  // [alphabet^2]
+    uint8_t* let = reinterpret_cast<uint8_t*>(em + 400);                 // [N][BD]
+    uint8_t* pij = let + (size_t)a.N * BD;                               // [P][2]
+
+    for (int i = tid; i < a.alphabet * a.alphabet; i += BD) em[i] = e_dev[i];
+    for (int i = tid; i < 2 * a.P; i += BD) pij[i] = a.pair_ij[i];
+
+    const uint64_t n_tiles = (a.count + BD - 1) / BD;
+    for (uint64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        const uint64_t q = tile * BD + tid;  // sequence number within the call
+        const bool live = q < a.count;
+        __syncthreads();
+        if (live) {
+            for (int k = 0; k < a.N; k++) {
+                uint32_t l;
+                if (SRC == SRC_BITS) l = (uint32_t)(((a.first + q) >> k) & 1ULL);
+                else if (SRC == SRC_SEQS) l = a.seqs[q * a.N + k];
+                else l = gp_letter20(a.seed, a.first + q, k);
+                let[k * BD + tid] = (uint8_t)l;
+            }
+            for (int p = 0; p < a.P; p++) {
+                int li = let[pij[2 * p] * BD + tid], lj = let[pij[2 * p + 1] * BD + tid];
+                pe[p * BD + tid] = em[li * a.alphabet + lj];
+            }
+        }
+        int32_t m1 = INT32_MAX, m2 = INT32_MAX;
+        uint32_t arg = 0;
+        for (uint32_t d0 = 0; d0 < a.D; d0 += CHUNK) {
+            const uint32_t nd = min((uint32_t)CHUNK, a.D - d0);
+            __syncthreads();
+            for (uint32_t i = tid; i < nd * a.NBP; i += BD) sidx[i] = a.pairidx[(size_t)d0 * a.NBP + i];
+            __syncthreads();
+            if (live) {
+                for (uint32_t c = 0; c < nd; c++) {
+                    const uint16_t* ix = sidx + c * a.NBP;
+                    int32_t E = 0;
+                    for (int k = 0; k < a.NBP; k++) E += pe[ix[k] * BD + tid];
+                    if (E < m1) { m2 = m1; m1 = E; arg = d0 + c; }
+                    else if (E < m2) { m2 = E; }
+                }
+            }
+        }
+        if (live) {
+            const bool folds = (m2 == INT32_MAX) || (m2 - m1 >= a.threshold);
+            a.pheno[q] = folds ? a.class_of[arg] : (uint16_t)GP_NULL_PHENO;
+            if (a.gap) {
+                int32_t g = (m2 == INT32_MAX) ? GP_GAP_NONE : max(m1 - m2, -32768);
+                a.gap[q] = (int16_t)g;
+            }
+        }
+    }
+}
+
+gp_status launch_simple(const gp_structures_s* s, const gp_energies* en, int src, const uint8_t* d_seqs, uint64_t seed,
+                        uint64_t first, uint64_t count, uint16_t* d_pheno, int16_t* d_gap, cudaStream_t st) {
+    if (!s || !en || !en->e || !d_pheno) return GP_INVALID_ARG;
+    if (en->alphabet < 2 || en->alphabet > 20 || en->threshold < 1) return GP_INVALID_ARG;
+    if (src == SRC_SEEDED && en->alphabet != 20) return GP_INVALID_ARG;
+    if (src == SRC_SEQS && !d_seqs) return GP_INVALID_ARG;
+    if (s->device < 0) { gp_set_cuda_error(cudaErrorNoDevice, "handle has no device tables"); return GP_CUDA_ERROR; }
+    const int A = en->alphabet;
+    int16_t h_e[400];
+    for (int i = 0; i < A; i++)
+        for (int j = 0; j < A; j++) {
+            int32_t v = en->e[i * A + j];
+            if (v != en->e[j * A + i]) return GP_INVALID_ARG;
+            if ((long long)v * s->NBP > 32767 || (long long)v * s->NBP < -32767) return GP_INVALID_ARG;
+            h_e[i * A + j] = (int16_t)v;
+        }
+    if (count == 0) return GP_OK;
+    int16_t* d_e = nullptr;
+    GP_CUDA(cudaMallocAsync(&d_e, sizeof(h_e), st));
+    GP_CUDA(cudaMemcpyAsync(d_e, h_e, sizeof(int16_t) * A * A, cudaMemcpyHostToDevice, st));  // pageable: staged before return
+
+    SimpleArgs a;
+    a.pairidx = s->d_pairidx; a.pair_ij = s->d_pair_ij; a.class_of = s->d_class_of; a.seqs = d_seqs;
+    a.pheno = d_pheno; a.gap = d_gap; a.first = first; a.count = count; a.seed = seed;
+    a.D = s->D; a.N = s->N; a.NBP = s->NBP; a.P = s->P; a.alphabet = A; a.threshold = en->threshold;
+    const int BD = 128;
+    size_t smem = (size_t)s->P * BD * 2 + (size_t)CHUNK * s->NBP * 2 + 800 + (size_t)s->N * BD + (size_t)s->P * 2 + 16;
+    int dev = 0, sms = 0;
+    GP_CUDA(cudaGetDevice(&dev));
+    GP_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    uint64_t tiles = (count + BD - 1) / BD;
+    int per_sm = (int)(200 * 1024 / smem);
+    if (per_sm < 1) per_sm = 1;
+    if (per_sm > 8) per_sm = 8;
+    unsigned grid = (unsigned)(tiles < (uint64_t)sms * per_sm ? tiles : (uint64_t)sms * per_sm);
+    void (*k)(SimpleArgs, const int16_t*) = src == SRC_BITS ? score_simple_kernel<SRC_BITS>
+                                             : src == SRC_SEQS ? score_simple_kernel<SRC_SEQS>
+                                                               : score_simple_kernel<SRC_SEEDED>;
+    GP_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    k<<<grid, BD, smem, st>>>(a, d_e);
+    GP_CUDA(cudaGetLastError());
+    GP_CUDA(cudaFreeAsync(d_e, st));
+    return GP_OK;
+}
+
+}  // namespace
+
+extern "C" gp_status gp_enumerate_simple(const gp_structures_t* s, const gp_energies* en, uint64_t g_begin,
+                                         uint64_t g_count, uint16_t* d_pheno, int16_t* d_gap, void* stream) {
+    if (!s || !en || en->alphabet != 2) return GP_INVALID_ARG;
+    const uint64_t total = s->N >= 64 ? ~0ULL : (1ULL << s->N);
+    if (g_begin > total || g_count > total - g_begin) return GP_RANGE;
+    return launch_simple(s, en, SRC_BITS, nullptr, 0, g_begin, g_count, d_pheno, d_gap, (cudaStream_t)stream);
+}
+
+extern "C" gp_status gp_enumerate_seqs(const gp_structures_t* s, const gp_energies* en, const uint8_t* d_seqs,
+                                       uint64_t count, uint16_t* d_pheno, int16_t* d_gap, void* stream) {
+    return launch_simple(s, en, SRC_SEQS, d_seqs, 0, 0, count, d_pheno, d_gap, (cudaStream_t)stream);
+}
+
+extern "C" gp_status gp_enumerate_seeded(const gp_structures_t* s, const gp_energies* en, uint64_t seed, uint64_t first,
+                                         uint64_t count, uint16_t* d_pheno, int16_t* d_gap, void* stream) {
+    return launch_simple(s, en, SRC_SEEDED, nullptr, seed, first, count, d_pheno, d_gap, (cudaStream_t)stream);
+}

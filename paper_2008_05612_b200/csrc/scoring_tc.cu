@@ -1,0 +1,451 @@
+// scoring_tc.cu — a1-a4 of the hot path on the 5th-generation tensor cores (sm_100a):
+//   a1 feature rows built in shared memory from the genotype index bits (genotypes are implicit)
+//   a2 E(g,S) = sum_contacts e(h_i,h_j) (Eq. 1, :67-69) as an int8 contraction  E = x(g) . W[S]  (tcgen05.mma kind::i8,
+//      accumulators in TMEM, weight tiles fetched by the TMA engine with cp.async.bulk)
+//   a3 min / second-min / argmin with strict uniqueness (:81, :552-575) fused on the TMEM read-out
+//   a4 one uint16 phenotype (and optional int16 gap) per genotype; the energy matrix never reaches HBM.
+//
+// Prefix folding.  With e(0,0)=a, lin=b-a, quad=c-2b+a:
+//   E(g,S) - a*NBP = lin * sum_k c_k(S) h_k + quad * sum_{contacts} h_i h_j.
+// A launch batch shares the genotype bits >= FB ("prefix"); only the low FB bits vary.  For one prefix every term with a
+// fixed monomer folds into the weights: a constant bias(S), and w_i(S) = lin*c_i(S) + quad*#(H partners of i in the
+// prefix).  The contraction then has K' = 2 + FB + pairs(FB) <= 128 columns instead of N + P (325 for 6x6), and the
+// per-prefix weight image W' [D x 128 B] is rebuilt by a small kernel (build_image_kernel) before each batch.
+//
+// Tiling.  A CTA processes a "supertile" of MT*128 = 512 consecutive genotypes: four 128-row A tiles stay in shared
+// memory while every 128-structure weight tile streams through a 6-stage ring once and is used by four MMAs
+// (M=128, N=128, K=32 x k_steps), one per A tile, into four TMEM accumulators (4 x 128 columns = all 512).  Four
+// epilogue warps (one per TMEM lane quarter; thread = genotype row) drain the accumulators.
+#include "device_common.cuh"
+
+namespace tc {
+
+constexpr int MT = 4;                 // genotype tiles per supertile
+constexpr int TM = 128, TN = 128;     // MMA tile: genotypes x structures
+constexpr int ROWB = 128;             // bytes per operand row = one 128-byte swizzle span = up to 128 int8 features
+constexpr int TILE_BYTES = TM * ROWB; // 16 KB, A tile and B stage alike
+constexpr int NSTAGE = 6;
+constexpr int SUPER = MT * TM;        // 512 genotypes
+constexpr int THREADS = 192;          // warp 0 TMA producer, warp 1 MMA issuer, warps 2-5 feature build + epilogue
+constexpr int MAX_FB = 22;            // 2 + 22 + 100 pairs = 124 <= 128 columns
+constexpr int KEY_SHIFT = 17;         // key = E * 2^17 + column (D < 2^17, |E| < 2^13)
+constexpr int E_NONE = 16383;         // INT32_MAX >> KEY_SHIFT: "no energy yet"
+
+struct Cols {        // column c of the folded contraction: A byte = val * h_i * h_j  (bit 31 of the row word is always 1)
+    uint8_t i[ROWB], j[ROWB], val[ROWB];
+};
+
+// ---- PTX wrappers ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "WAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra DONE_%=;\n\t"
+        "bra WAIT_%=;\n\t"
+        "DONE_%=:\n\t}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+// TMA engine, 1-D bulk copy global -> shared, completion counted in bytes on an mbarrier
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_commit(uint64_t* bar) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+// D[tmem] (+)= A[smem] . B[smem]^T, int8 x int8 -> int32
+__device__ __forceinline__ void mma_i8(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p;\n\t}" ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc),
+        "r"(accumulate) : "memory");
+}
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, int32_t (&v)[32]) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]),
+          "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]), "=r"(v[16]),
+          "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]), "=r"(v[24]),
+          "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+        : "r"(taddr) : "memory");
+}
+__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+
+// shared-memory matrix descriptor: K-major, 128-byte swizzle, 8-row groups 1024 B apart (rows are 128 B)
+__device__ __forceinline__ uint64_t smem_desc(uint32_t saddr) {
+    return (uint64_t)((saddr & 0x3FFFFu) >> 4) | (1ULL << 16) | ((uint64_t)(1024 >> 4) << 32) | (1ULL << 46) | (2ULL << 61);
+}
+// instruction descriptor: D = s32, A = B = s8, both K-major, N = 128, M = 128
+constexpr uint32_t IDESC = (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(TN >> 3) << 17) | ((uint32_t)(TM >> 4) << 24);
+
+// byte offset of (row r, byte c) inside a 128-byte-swizzled tile with 128-byte rows
+__host__ __device__ __forceinline__ uint32_t swz(uint32_t r, uint32_t c) {
+    return r * ROWB + ((((c >> 4) ^ (r & 7u)) << 4) | (c & 15u));
+}
+
+struct Args {
+    const int8_t* img;        // [n_batches][n_tiles][TILE_BYTES]
+    const uint16_t* class_of;
+    uint16_t* pheno;          // indexed by g - out_base
+    int16_t* gap;             // nullable
+    uint64_t g_first;         // first genotype of this launch (multiple of SUPER)
+    uint64_t g_end;           // one past the last genotype to store
+    uint64_t out_base;        // genotype that maps to pheno[0]
+    uint32_t n_items;         // supertiles in this launch
+    uint32_t n_tiles;         // ceil(D / TN)
+    uint32_t D;
+    int fb;                   // folded (varying) low bits
+    int k_steps;              // 32-byte K steps actually used (1..4)
+    int threshold;
+};
+
+// ---- a1: feature rows -----------------------------------------------------------------------------------------------
+// Row r of A tile m holds genotype g0 + m*128 + r: byte c = val[c] * h_{i[c]} * h_{j[c]} on its low `fb` bits.
+__device__ __forceinline__ void build_a_row(uint8_t* a_tile, uint32_t r, uint32_t glow, const Cols& cols) {
+    const uint32_t w = glow | 0x80000000u;  // bit 31: the constant-1 "monomer" used by the bias columns
+#pragma unroll 1
+    for (uint32_t c16 = 0; c16 < ROWB / 16; c16++) {
+        uint32_t q[4];
+#pragma unroll
+        for (int wd = 0; wd < 4; wd++) {
+            uint32_t x = 0;
+#pragma unroll
+            for (int b = 0; b < 4; b++) {
+                const uint32_t c = c16 * 16 + wd * 4 + b;
+                const uint32_t bit = (w >> cols.i[c]) & (w >> cols.j[c]) & 1u;
+                x |= (bit * cols.val[c]) << (8 * b);
+            }
+            q[wd] = x;
+        }
+        *reinterpret_cast<uint4*>(a_tile + r * ROWB + ((c16 ^ (r & 7u)) << 4)) = make_uint4(q[0], q[1], q[2], q[3]);
+    }
+}
+
+// ---- a3: exact min / second-min / argmin on packed keys -------------------------------------------------------------
+// key = E * 2^17 + column.  (k1, k2) = the two smallest keys seen.  Keys are distinct, so k2 >> 17 is the second-smallest
+// energy counted with multiplicity (R6), and a tie at the minimum shows as equal energies in k1 and k2.
+// Filter: eight columns are rescanned only if their minimum is strictly below the current second-smallest energy;
+// an energy equal to it cannot change (k1, k2) because columns arrive in increasing order.
+__device__ __forceinline__ int min3(int a, int b, int c) { return min(a, min(b, c)); }
+
+__device__ __forceinline__ void fold_chunk(const int32_t (&v)[32], uint32_t col0, int32_t& k1, int32_t& k2, int32_t& e2) {
+#pragma unroll
+    for (int s = 0; s < 4; s++) {
+        const int32_t* u = &v[8 * s];
+        const int32_t sm = min3(min3(u[0], u[1], u[2]), min3(u[3], u[4], u[5]), min(u[6], u[7]));
+        if (sm < e2) {
+#pragma unroll
+            for (int j = 0; j < 8; j++) {
+                const int32_t key = u[j] * (1 << KEY_SHIFT) + (int32_t)(col0 + 8 * s + j);
+                k2 = min(k2, max(k1, key));
+                k1 = min(k1, key);
+            }
+            e2 = k2 >> KEY_SHIFT;
+        }
+    }
+}
+
+struct __align__(8) Barriers {
+    uint64_t b_full[NSTAGE], b_empty[NSTAGE];
+    uint64_t acc_full[MT], acc_empty[MT];
+    uint64_t a_full, a_empty;
+    uint32_t tmem_base;
+};
+
+__global__ void __launch_bounds__(THREADS, 1) scoring_kernel(const Args a, const Cols cols_in) {
+    extern __shared__ unsigned char smem_dyn[];
+    unsigned char* smem = reinterpret_cast<unsigned char*>(((uintptr_t)smem_dyn + 1023) & ~(uintptr_t)1023);
+    uint8_t* sA = smem;                                   // MT tiles
+    uint8_t* sB = smem + MT * TILE_BYTES;                 // NSTAGE tiles
+    Barriers* bar = reinterpret_cast<Barriers*>(sB + NSTAGE * TILE_BYTES);
+    Cols* cols = reinterpret_cast<Cols*>(bar + 1);
+
+    const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+    for (uint32_t i = threadIdx.x; i < sizeof(Cols); i += THREADS)
+        reinterpret_cast<uint8_t*>(cols)[i] = reinterpret_cast<const uint8_t*>(&cols_in)[i];
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < NSTAGE; s++) { mbar_init(&bar->b_full[s], 1); mbar_init(&bar->b_empty[s], 1); }
+        for (int m = 0; m < MT; m++) { mbar_init(&bar->acc_full[m], 1); mbar_init(&bar->acc_empty[m], 4); }
+        mbar_init(&bar->a_full, 128);
+        mbar_init(&bar->a_empty, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 1) {  // TMEM: all 512 columns (one CTA per SM)
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(&bar->tmem_base)) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = bar->tmem_base;
+
+    if (warp == 0) {
+        // ===== producer: stream every weight tile of the item's batch image through the ring =====
+        if (lane == 0) {
+            uint32_t it = 0;
+            for (uint32_t item = blockIdx.x; item < a.n_items; item += gridDim.x) {
+                const uint64_t g0 = a.g_first + (uint64_t)item * SUPER;
+                const uint64_t batch = (g0 >> a.fb) - (a.g_first >> a.fb);
+                const int8_t* img = a.img + batch * (uint64_t)a.n_tiles * TILE_BYTES;
+                for (uint32_t n = 0; n < a.n_tiles; n++, it++) {
+                    const uint32_t s = it % NSTAGE, ph = (it / NSTAGE) & 1;
+                    mbar_wait(&bar->b_empty[s], ph ^ 1);
+                    mbar_expect_tx(&bar->b_full[s], TILE_BYTES);
+                    bulk_g2s(sB + s * TILE_BYTES, img + (uint64_t)n * TILE_BYTES, TILE_BYTES, &bar->b_full[s]);
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ===== MMA issuer: one thread =====
+        if (lane == 0) {
+            uint32_t it = 0, item_no = 0;
+            for (uint32_t item = blockIdx.x; item < a.n_items; item += gridDim.x, item_no++) {
+                mbar_wait(&bar->a_full, item_no & 1);
+                tc_fence_after();
+                for (uint32_t n = 0; n < a.n_tiles; n++, it++) {
+                    const uint32_t s = it % NSTAGE, ph = (it / NSTAGE) & 1;
+                    mbar_wait(&bar->b_full[s], ph);
+                    tc_fence_after();
+                    const uint32_t b_addr = smem_u32(sB + s * TILE_BYTES);
+#pragma unroll
+                    for (int m = 0; m < MT; m++) {
+                        mbar_wait(&bar->acc_empty[m], (it & 1) ^ 1);
+                        tc_fence_after();
+                        const uint32_t a_addr = smem_u32(sA + m * TILE_BYTES);
+                        for (int k = 0; k < a.k_steps; k++)
+                            mma_i8(tmem + m * TN, smem_desc(a_addr + k * 32), smem_desc(b_addr + k * 32), IDESC, k > 0);
+                        tc_commit(&bar->acc_full[m]);
+                    }
+                    tc_commit(&bar->b_empty[s]);
+                }
+                tc_commit(&bar->a_empty);
+            }
+        }
+    } else {
+        // ===== feature build + epilogue: 128 threads, thread = genotype row =====
+        const uint32_t quarter = warp & 3;              // TMEM lanes 32*quarter .. +31 belong to this warp
+        const uint32_t r = quarter * 32 + lane;         // row within each 128-row tile
+        const uint32_t t_lane = tmem + ((quarter * 32u) << 16);
+        uint32_t it = 0, item_no = 0;
+        for (uint32_t item = blockIdx.x; item < a.n_items; item += gridDim.x, item_no++) {
+            const uint64_t g0 = a.g_first + (uint64_t)item * SUPER;
+            mbar_wait(&bar->a_empty, (item_no & 1) ^ 1);
+            const uint32_t lowmask = a.fb >= 32 ? 0xFFFFFFFFu : ((1u << a.fb) - 1u);
+#pragma unroll 1
+            for (int m = 0; m < MT; m++)
+                build_a_row(sA + m * TILE_BYTES, r, (uint32_t)(g0 + m * TM + r) & lowmask, *cols);
+            fence_proxy_async();
+            mbar_arrive(&bar->a_full);
+
+            int32_t k1[MT], k2[MT], e2[MT];
+#pragma unroll
+            for (int m = 0; m < MT; m++) { k1[m] = INT32_MAX; k2[m] = INT32_MAX; e2[m] = E_NONE; }
+            for (uint32_t n = 0; n < a.n_tiles; n++, it++) {
+                const bool last = (n + 1 == a.n_tiles);
+#pragma unroll
+                for (int m = 0; m < MT; m++) {
+                    mbar_wait(&bar->acc_full[m], it & 1);
+                    tc_fence_after();
+#pragma unroll
+                    for (int ch = 0; ch < TN / 32; ch++) {
+                        int32_t v[32];
+                        tmem_ld32(t_lane + m * TN + ch * 32, v);
+                        tmem_ld_wait();
+                        if (ch == TN / 32 - 1) {  // accumulator m fully read: hand it back to the MMA warp
+                            tc_fence_before();
+                            __syncwarp();
+                            if (lane == 0) mbar_arrive(&bar->acc_empty[m]);
+                        }
+                        const uint32_t col0 = n * TN + ch * 32;
+                        if (last) {
+#pragma unroll
+                            for (int j = 0; j < 32; j++)
+                                if (col0 + j >= a.D) v[j] = E_NONE;  // pad columns never win
+                        }
+                        fold_chunk(v, col0, k1[m], k2[m], e2[m]);
+                    }
+                }
+            }
+#pragma unroll
+            for (int m = 0; m < MT; m++) {
+                const uint64_t g = g0 + (uint64_t)m * TM + r;
+                if (g < a.g_end && g >= a.out_base) {
+                    const int32_t e1 = k1[m] >> KEY_SHIFT, e2v = k2[m] >> KEY_SHIFT;
+                    const uint32_t col = (uint32_t)k1[m] & ((1u << KEY_SHIFT) - 1u);
+                    const bool single = (k2[m] == INT32_MAX);
+                    const bool folds = single || (e2v - e1 >= a.threshold);
+                    a.pheno[g - a.out_base] = folds ? a.class_of[col] : (uint16_t)GP_NULL_PHENO;
+                    if (a.gap) a.gap[g - a.out_base] = (int16_t)(single ? GP_GAP_NONE : max(e1 - e2v, -32768));
+                }
+            }
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 1) {
+        tc_fence_after();
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem) : "memory");
+    }
+}
+
+// ---- per-prefix weight image ----------------------------------------------------------------------------------------
+struct Slots {  // column of pair (i, j), i < j < fb, in the folded contraction; 0 = not a column
+    uint8_t pair[MAX_FB * MAX_FB];
+};
+
+struct ImgArgs {
+    const uint8_t* contacts;  // D * NBP * 2
+    int8_t* img;              // [n_batches][n_tiles][TILE_BYTES]
+    uint64_t hi_first;        // prefix (g >> fb) of batch 0; batch y has prefix hi_first + y
+    uint32_t D, n_tiles;
+    int NBP, fb, lin, quad;
+};
+
+// One block = one 128-structure tile of one prefix.  Thread = structure: it accumulates its 128-byte weight row in
+// shared memory (already in the swizzled layout the MMA reads), then the block writes the 16 KB tile out coalesced.
+__global__ void __launch_bounds__(TN) build_image_kernel(const ImgArgs a, const Slots slots) {
+    __shared__ __align__(16) int8_t tile[TILE_BYTES];
+    const uint32_t r = threadIdx.x, n = blockIdx.x;
+    const uint64_t H = a.hi_first + blockIdx.y;
+    for (uint32_t i = threadIdx.x; i < TILE_BYTES / 16; i += TN) reinterpret_cast<uint4*>(tile)[i] = make_uint4(0, 0, 0, 0);
+    __syncthreads();
+    const uint32_t d = n * TN + r;
+    if (d < a.D) {
+        const uint8_t* c = a.contacts + (size_t)d * a.NBP * 2;
+        int bias = 0;
+        for (int k = 0; k < a.NBP; k++) {
+            const int i = c[2 * k], j = c[2 * k + 1];  // i < j
+            if (j < a.fb) {
+                tile[swz(r, 2 + i)] += (int8_t)a.lin;
+                tile[swz(r, 2 + j)] += (int8_t)a.lin;
+                tile[swz(r, slots.pair[i * MAX_FB + j])] = (int8_t)a.quad;
+            } else if (i < a.fb) {
+                const int hj = (int)((H >> (j - a.fb)) & 1ULL);
+                tile[swz(r, 2 + i)] += (int8_t)(a.lin + a.quad * hj);
+                bias += a.lin * hj;
+            } else {
+                const int hi = (int)((H >> (i - a.fb)) & 1ULL), hj = (int)((H >> (j - a.fb)) & 1ULL);
+                bias += a.lin * (hi + hj) + a.quad * hi * hj;
+            }
+        }
+        tile[swz(r, 0)] = (int8_t)(bias >> 6);   // x 64
+        tile[swz(r, 1)] = (int8_t)(bias & 63);   // x 1
+    }
+    __syncthreads();
+    uint4* dst = reinterpret_cast<uint4*>(a.img + ((uint64_t)blockIdx.y * a.n_tiles + n) * TILE_BYTES);
+    for (uint32_t i = threadIdx.x; i < TILE_BYTES / 16; i += TN) dst[i] = reinterpret_cast<const uint4*>(tile)[i];
+}
+
+int g_fold_bits = 19;  // 2 + 19 + 72 = 93 columns -> 3 K steps
+
+}  // namespace tc
+
+// test / tuning hook (not part of the public header): number of low genotype bits kept as contraction columns
+extern "C" int gp_set_fold_bits(int fb) {
+    if (fb < 9 || fb > tc::MAX_FB) return -1;
+    tc::g_fold_bits = fb;
+    return 0;
+}
+
+gp_status gp_launch_scoring_tc(gp_structures_s* s, const gp_hp_params& hp, uint64_t g_begin, uint64_t g_count,
+                               uint16_t* d_pheno, int16_t* d_gap, cudaStream_t st) {
+    using namespace tc;
+    const int N = s->N;
+    const int fb = N < g_fold_bits ? N : g_fold_bits;
+    if (s->D >= (1u << KEY_SHIFT)) return GP_UNSUPPORTED_LATTICE;
+    // columns
+    Cols cols;
+    Slots slots;
+    memset(&slots, 0, sizeof(slots));
+    for (int c = 0; c < ROWB; c++) { cols.i[c] = 31; cols.j[c] = 31; cols.val[c] = 0; }
+    cols.val[0] = 64;
+    cols.val[1] = 1;
+    int nc = 2;
+    for (int i = 0; i < fb; i++, nc++) { cols.i[nc] = cols.j[nc] = (uint8_t)i; cols.val[nc] = 1; }
+    for (int i = 0; i < fb; i++)
+        for (int j = i + 3; j < fb; j += 2, nc++) {
+            cols.i[nc] = (uint8_t)i; cols.j[nc] = (uint8_t)j; cols.val[nc] = 1;
+            slots.pair[i * MAX_FB + j] = (uint8_t)nc;
+        }
+    if (nc > ROWB) return GP_INVALID_ARG;
+    const int k_steps = (nc + 31) / 32;
+    const uint32_t n_tiles = (s->D + TN - 1) / TN;
+    const size_t img_bytes = (size_t)n_tiles * TILE_BYTES;
+
+    int dev = 0, sms = 0;
+    GP_CUDA(cudaGetDevice(&dev));
+    GP_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    const size_t smem = (size_t)(MT + NSTAGE) * TILE_BYTES + sizeof(Barriers) + sizeof(Cols) + 1024 + 64;
+    GP_CUDA(cudaFuncSetAttribute(scoring_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+
+    // batches of 2^fb genotypes share a weight image; a launch covers up to `group` batches
+    const uint64_t batch_len = 1ULL << fb;
+    const uint64_t g_end = g_begin + g_count;
+    uint64_t group = (256ULL << 20) / img_bytes;  // <= 256 MB of images per launch
+    if (group < 1) group = 1;
+    if (group > 64) group = 64;
+    const size_t need = img_bytes * (size_t)group;
+    if (s->scratch_bytes < need) {
+        if (s->d_scratch) GP_CUDA(cudaFree(s->d_scratch));
+        s->d_scratch = nullptr; s->scratch_bytes = 0;
+        GP_CUDA(cudaMalloc(&s->d_scratch, need));
+        s->scratch_bytes = need;
+    }
+    uint64_t g = g_begin & ~(uint64_t)(SUPER - 1);  // g_begin is a multiple of gp_tile() = SUPER already
+    while (g < g_end) {
+        const uint64_t b0 = g >> fb;
+        uint64_t stop = (b0 + group) << fb;
+        if (stop > g_end) stop = g_end;
+        const uint32_t n_batches = (uint32_t)(((stop - 1) >> fb) - b0 + 1);
+        ImgArgs ia;
+        ia.contacts = s->d_contacts; ia.img = (int8_t*)s->d_scratch; ia.hi_first = b0; ia.D = s->D; ia.n_tiles = n_tiles;
+        ia.NBP = s->NBP; ia.fb = fb; ia.lin = hp.lin; ia.quad = hp.quad;
+        build_image_kernel<<<dim3(n_tiles, n_batches), TN, 0, st>>>(ia, slots);
+        GP_CUDA(cudaGetLastError());
+        Args a;
+        a.img = (const int8_t*)s->d_scratch; a.class_of = s->d_class_of; a.pheno = d_pheno; a.gap = d_gap;
+        a.g_first = g; a.g_end = stop; a.out_base = g_begin;
+        a.n_items = (uint32_t)((stop - g + SUPER - 1) / SUPER);
+        a.n_tiles = n_tiles; a.D = s->D; a.fb = fb; a.k_steps = k_steps; a.threshold = hp.threshold;
+        const unsigned grid = a.n_items < (uint32_t)sms ? a.n_items : (uint32_t)sms;
+        scoring_kernel<<<grid, THREADS, smem, st>>>(a, cols);
+        GP_CUDA(cudaGetLastError());
+        g = stop;
+    }
+    (void)batch_len;
+    return GP_OK;
+}
+
+extern "C" uint64_t gp_tile(void) { return tc::SUPER; }
+
+extern "C" gp_status gp_enumerate(const gp_structures_t* s_, const gp_energies* en, uint64_t g_begin, uint64_t g_count,
+                                  uint16_t* d_pheno, int16_t* d_gap, void* stream) {
+    gp_structures_s* s = const_cast<gp_structures_s*>(s_);
+    gp_hp_params hp;
+    gp_status stt = gp_check_hp(s, en, &hp);
+    if (stt != GP_OK) return stt;
+    if (!d_pheno && g_count) return GP_INVALID_ARG;
+    const uint64_t total = s->N >= 64 ? ~0ULL : (1ULL << s->N);
+    if (g_begin > total || g_count > total - g_begin || (g_begin % tc::SUPER) != 0) return GP_RANGE;
+    if (s->device < 0) { gp_set_cuda_error(cudaErrorNoDevice, "handle has no device tables"); return GP_CUDA_ERROR; }
+    if (g_count == 0) return GP_OK;
+    return gp_launch_scoring_tc(s, hp, g_begin, g_count, d_pheno, d_gap, (cudaStream_t)stream);
+}

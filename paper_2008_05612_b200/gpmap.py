@@ -1,0 +1,242 @@
+"""Thin ctypes binding of libgpmap (include/gpmap.h).  Argument marshalling only: every step of the path runs in
+the library's CUDA kernels.  PyTorch supplies device memory and streams.  There is no CPU fallback: a missing or
+unbuildable library raises at import of the first call.
+"""
+import ctypes
+import os
+
+import numpy as np
+
+from . import build as _build
+
+NULL_PHENO = 0xFFFF
+GAP_NONE = -32768
+HP_ENERGIES = (0, -10, -10, -23)  # e[a*2+b], letter 1 = H: E_PP, E_HP, E_HP, E_HH x10
+
+_u8p, _u16p, _i16p = (ctypes.POINTER(ctypes.c_uint8), ctypes.POINTER(ctypes.c_uint16), ctypes.POINTER(ctypes.c_int16))
+_i32p, _u32p, _u64p = (ctypes.POINTER(ctypes.c_int32), ctypes.POINTER(ctypes.c_uint32), ctypes.POINTER(ctypes.c_uint64))
+_vp = ctypes.c_void_p
+
+
+class _Energies(ctypes.Structure):
+    _fields_ = [("alphabet", ctypes.c_int32), ("e", _i32p), ("threshold", ctypes.c_int32)]
+
+
+# name -> (restype, argtypes); must list every symbol include/gpmap.h declares (tests/test_abi.py checks)
+SIGNATURES = {
+    "gp_structures": (ctypes.c_int, [ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.POINTER(_vp)]),
+    "gp_structures_free": (None, [_vp]),
+    "gp_structures_length": (ctypes.c_int, [_vp]),
+    "gp_structures_directed": (ctypes.c_uint32, [_vp]),
+    "gp_structures_classes": (ctypes.c_uint32, [_vp]),
+    "gp_structures_self_reverse": (ctypes.c_uint32, [_vp]),
+    "gp_structures_walks": (ctypes.c_uint64, [_vp]),
+    "gp_structures_contacts_per_fold": (ctypes.c_int, [_vp]),
+    "gp_structures_features": (ctypes.c_int, [_vp]),
+    "gp_structures_get": (ctypes.c_int, [_vp, ctypes.c_uint32, _u8p, _u8p, _u16p]),
+    "gp_tile": (ctypes.c_uint64, []),
+    "gp_enumerate": (ctypes.c_int, [_vp, ctypes.POINTER(_Energies), ctypes.c_uint64, ctypes.c_uint64, _vp, _vp, _vp]),
+    "gp_enumerate_simple": (ctypes.c_int, [_vp, ctypes.POINTER(_Energies), ctypes.c_uint64, ctypes.c_uint64, _vp, _vp, _vp]),
+    "gp_enumerate_seqs": (ctypes.c_int, [_vp, ctypes.POINTER(_Energies), _vp, ctypes.c_uint64, _vp, _vp, _vp]),
+    "gp_enumerate_seeded": (ctypes.c_int, [_vp, ctypes.POINTER(_Energies), ctypes.c_uint64, ctypes.c_uint64,
+                                           ctypes.c_uint64, _vp, _vp, _vp]),
+    "gp_seeded_matrix": (ctypes.c_int, [ctypes.c_uint64, _i32p]),
+    "gp_seeded_sequences": (ctypes.c_int, [ctypes.c_uint64, ctypes.c_uint64, ctypes.c_uint64, ctypes.c_int, _u8p]),
+    "gp_designability": (ctypes.c_int, [_vp, ctypes.c_uint64, ctypes.c_uint32, _vp, _vp]),
+    "gp_robustness": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_uint32, _vp, _vp, _vp, _vp, _vp]),
+    "gp_nn_components": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_uint32, _vp, _vp]),
+    "gp_enumerate_host": (ctypes.c_int, [_vp, ctypes.POINTER(_Energies), ctypes.c_uint64, ctypes.c_uint64, _u16p, _u64p]),
+    "gp_strerror": (ctypes.c_char_p, [ctypes.c_int]),
+    "gp_last_cuda_error": (ctypes.c_char_p, []),
+}
+
+_lib = None
+
+
+def lib():
+    """Load (building if stale) libgpmap.so.  Raises if it cannot be built or loaded — never falls back."""
+    global _lib
+    if _lib is None:
+        path = _build.build()
+        L = ctypes.CDLL(path)
+        for name, (res, args) in SIGNATURES.items():
+            f = getattr(L, name)
+            f.restype = res
+            f.argtypes = args
+        L.gp_set_fold_bits.restype = ctypes.c_int
+        L.gp_set_fold_bits.argtypes = [ctypes.c_int]
+        _lib = L
+    return _lib
+
+
+class GpError(RuntimeError):
+    def __init__(self, status, what):
+        L = lib()
+        msg = "%s: %s" % (what, L.gp_strerror(status).decode())
+        if status == 4:
+            msg += " [" + L.gp_last_cuda_error().decode() + "]"
+        super().__init__(msg)
+        self.status = status
+
+
+def _check(status, what):
+    if status != 0:
+        raise GpError(status, what)
+
+
+def _dptr(t, dtype=None):
+    """Device pointer of a CUDA torch tensor (None -> NULL)."""
+    if t is None:
+        return None
+    if not t.is_cuda or not t.is_contiguous():
+        raise ValueError("expected a contiguous CUDA tensor")
+    if dtype is not None and t.dtype != dtype:
+        raise ValueError("expected dtype %s, got %s" % (dtype, t.dtype))
+    return ctypes.c_void_p(t.data_ptr())
+
+
+def _stream(stream):
+    if stream is None:
+        import torch
+        return ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+    return ctypes.c_void_p(stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream))
+
+
+def _energies(e, alphabet, threshold):
+    arr = np.ascontiguousarray(e, np.int32).reshape(-1)
+    if arr.size != alphabet * alphabet:
+        raise ValueError("energies must have alphabet^2 entries")
+    en = _Energies(alphabet, arr.ctypes.data_as(_i32p), threshold)
+    en._keep = arr
+    return en
+
+
+def tile():
+    return int(lib().gp_tile())
+
+
+def set_fold_bits(fb):
+    """Tuning/test hook: number of low genotype bits kept as contraction columns (9..22, default 19)."""
+    if lib().gp_set_fold_bits(fb) != 0:
+        raise ValueError("fold bits must be in 9..22")
+
+
+class Structures:
+    """gp_structures handle: the fold library of an nx x ny x nz box."""
+
+    def __init__(self, nx, ny, nz=1):
+        h = _vp()
+        _check(lib().gp_structures(nx, ny, nz, ctypes.byref(h)), "gp_structures(%d,%d,%d)" % (nx, ny, nz))
+        self._h = h
+        L = lib()
+        self.dims = (nx, ny, nz)
+        self.N = L.gp_structures_length(h)
+        self.D = L.gp_structures_directed(h)
+        self.C = L.gp_structures_classes(h)
+        self.self_reverse = L.gp_structures_self_reverse(h)
+        self.walk_count = L.gp_structures_walks(h)
+        self.NBP = L.gp_structures_contacts_per_fold(h)
+        self.K = L.gp_structures_features(h)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().gp_structures_free(self._h)
+            self._h = None
+
+    __del__ = close
+
+    def get(self, d):
+        sites = np.zeros(self.N, np.uint8)
+        contacts = np.zeros(2 * self.NBP, np.uint8)
+        cid = ctypes.c_uint16()
+        _check(lib().gp_structures_get(self._h, d, sites.ctypes.data_as(_u8p), contacts.ctypes.data_as(_u8p),
+                                       ctypes.byref(cid)), "gp_structures_get")
+        return sites, contacts.reshape(self.NBP, 2), cid.value
+
+    def tables(self):
+        sites = np.zeros((self.D, self.N), np.uint8)
+        contacts = np.zeros((self.D, self.NBP, 2), np.uint8)
+        class_of = np.zeros(self.D, np.uint32)
+        for d in range(self.D):
+            s, c, k = self.get(d)
+            sites[d], contacts[d], class_of[d] = s, c, k
+        return sites, contacts, class_of
+
+    # ---- scoring ----
+    def enumerate(self, g_begin, g_count, pheno, gap=None, e=HP_ENERGIES, threshold=1, stream=None, simple=False):
+        """gp_enumerate / gp_enumerate_simple into caller-owned CUDA tensors (uint16 / int16)."""
+        import torch
+        en = _energies(e, 2, threshold)
+        f = lib().gp_enumerate_simple if simple else lib().gp_enumerate
+        if pheno.numel() < g_count or (gap is not None and gap.numel() < g_count):
+            raise ValueError("output tensor too small")
+        _check(f(self._h, ctypes.byref(en), g_begin, g_count, _dptr(pheno, torch.uint16), _dptr(gap, torch.int16),
+                 _stream(stream)), "gp_enumerate")
+
+    def enumerate_seqs(self, seqs, pheno, gap=None, e=None, alphabet=20, threshold=1, stream=None):
+        import torch
+        en = _energies(e, alphabet, threshold)
+        if seqs.dim() != 2 or seqs.shape[1] != self.N:
+            raise ValueError("seqs must be [count, N] uint8")
+        _check(lib().gp_enumerate_seqs(self._h, ctypes.byref(en), _dptr(seqs, torch.uint8), seqs.shape[0],
+                                       _dptr(pheno, torch.uint16), _dptr(gap, torch.int16), _stream(stream)),
+               "gp_enumerate_seqs")
+
+    def enumerate_seeded(self, seed, first, count, pheno, gap=None, e=None, threshold=1, stream=None):
+        import torch
+        en = _energies(e, 20, threshold)
+        _check(lib().gp_enumerate_seeded(self._h, ctypes.byref(en), seed, first, count, _dptr(pheno, torch.uint16),
+                                         _dptr(gap, torch.int16), _stream(stream)), "gp_enumerate_seeded")
+
+    def enumerate_host(self, g_begin, g_count, e=HP_ENERGIES, threshold=1, want_pheno=True):
+        """gp_enumerate_host: numpy in/out, host<->device copies inside the call."""
+        en = _energies(e, 2, threshold)
+        pheno = np.empty(g_count, np.uint16) if want_pheno else None
+        hist = np.zeros(self.C + 1, np.uint64)
+        _check(lib().gp_enumerate_host(self._h, ctypes.byref(en), g_begin, g_count,
+                                       pheno.ctypes.data_as(_u16p) if want_pheno else None,
+                                       hist.ctypes.data_as(_u64p)), "gp_enumerate_host")
+        return pheno, hist
+
+
+def seeded_matrix(seed):
+    M = np.zeros(400, np.int32)
+    _check(lib().gp_seeded_matrix(seed, M.ctypes.data_as(_i32p)), "gp_seeded_matrix")
+    return M.reshape(20, 20)
+
+
+def seeded_sequences(seed, first, count, n):
+    s = np.zeros((count, n), np.uint8)
+    _check(lib().gp_seeded_sequences(seed, first, count, n, s.ctypes.data_as(_u8p)), "gp_seeded_sequences")
+    return s
+
+
+def designability(pheno, n_classes, hist=None, stream=None):
+    import torch
+    if hist is None:
+        hist = torch.empty(n_classes + 1, dtype=torch.int64, device=pheno.device)
+    _check(lib().gp_designability(_dptr(pheno, torch.uint16), pheno.numel(), n_classes, _dptr(hist, torch.int64),
+                                  _stream(stream)), "gp_designability")
+    return hist
+
+
+def robustness(pheno, n_bits, n_classes, want_pairs=True, stream=None):
+    """(R, D, O, pair_count) device tensors (int64); pair_count is None if not requested."""
+    import torch
+    if pheno.numel() != 1 << n_bits:
+        raise ValueError("gp_robustness needs the full store of 2^n_bits entries")
+    out = torch.empty((3, n_classes), dtype=torch.int64, device=pheno.device)
+    pc = torch.empty(1, dtype=torch.int64, device=pheno.device) if want_pairs else None
+    _check(lib().gp_robustness(_dptr(pheno, torch.uint16), n_bits, n_classes, _dptr(out[0]), _dptr(out[1]), _dptr(out[2]),
+                               _dptr(pc), _stream(stream)), "gp_robustness")
+    return out[0], out[1], out[2], pc
+
+
+def nn_components(pheno, n_bits, n_classes, stream=None):
+    import torch
+    if pheno.numel() != 1 << n_bits:
+        raise ValueError("gp_nn_components needs the full store of 2^n_bits entries")
+    ncomp = torch.empty(n_classes, dtype=torch.int32, device=pheno.device)
+    _check(lib().gp_nn_components(_dptr(pheno, torch.uint16), n_bits, n_classes, _dptr(ncomp, torch.int32),
+                                  _stream(stream)), "gp_nn_components")
+    return ncomp

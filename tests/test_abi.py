@@ -1,0 +1,101 @@
+"""CPU-side checks of the C-ABI library: it builds for sm_100a, loads, exports every symbol include/gpmap.h declares,
+rejects bad arguments, and its host-side gp_structures (a0) agrees with the oracle's fold library table by table.
+No compute calls (no GPU here)."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+from oracle import gp_oracle as orc
+from paper_2008_05612_b200 import build as gbuild
+from paper_2008_05612_b200 import gpmap
+from tests._golden import read_pins
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_library_builds_and_exports_every_declared_symbol():
+    path = gbuild.build()
+    assert os.path.exists(path)
+    L = ctypes.CDLL(path)
+    header = open(os.path.join(ROOT, "include", "gpmap.h")).read()
+    header = re.sub(r"/\*.*?\*/", "", header, flags=re.S)
+    declared = set(re.findall(r"\b(gp_[a-z0-9_]+)\s*\(", header))
+    assert len(declared) >= 20
+    for name in declared:
+        assert hasattr(L, name), "libgpmap.so does not export %s" % name
+    assert declared == set(gpmap.SIGNATURES), declared ^ set(gpmap.SIGNATURES)
+
+
+def test_library_contains_sm100a_tensor_core_code():
+    """The scoring kernel is tcgen05 code for sm_100a (PTX mnemonics are checked; SASS needs cuobjdump)."""
+    src = open(os.path.join(gbuild.CSRC, "scoring_tc.cu")).read()
+    assert "tcgen05.mma.cta_group::1.kind::i8" in src and "cp.async.bulk" in src and "tcgen05.ld" in src
+    assert "arch=compute_100a,code=sm_100a" in " ".join(gbuild.NVCC_FLAGS)
+
+
+def test_status_strings_and_tile():
+    L = gpmap.lib()
+    assert L.gp_strerror(0) == b"ok"
+    assert all(L.gp_strerror(i) for i in range(6))
+    assert gpmap.tile() == 512
+
+
+@pytest.mark.parametrize("dims", [(2, 2, 1), (3, 3, 1), (3, 2, 1), (4, 4, 1), (5, 5, 1), (2, 2, 2), (4, 3, 1), (6, 6, 1),
+                                  (3, 3, 3)])
+def test_structures_match_oracle(oracle_structures, dims):
+    S = gpmap.Structures(*dims)
+    O = oracle_structures(*dims)
+    assert (S.N, S.D, S.C, S.NBP, S.self_reverse, S.walk_count) == (O.N, O.D, O.C, O.NBP, O.self_reverse, O.walk_count)
+    step = max(1, S.D // 2000)
+    for d in list(range(0, S.D, step)) + [S.D - 1]:
+        s1, c1, k1 = S.get(d)
+        s2, c2, k2 = O.get(d)
+        assert np.array_equal(s1, s2) and np.array_equal(c1, c2) and k1 == k2, (dims, d)
+    S.close()
+
+
+def test_structure_counts_are_the_papers():
+    pins = read_pins()
+    S = gpmap.Structures(6, 6)
+    assert S.D == pins["folds_6x6_directed"] and S.N == pins["length_6x6"]
+    assert S.K == 325 and S.NBP == 25
+    S.close()
+
+
+def test_bad_arguments():
+    L = gpmap.lib()
+    h = ctypes.c_void_p()
+    assert L.gp_structures(0, 3, 1, ctypes.byref(h)) == 2 and not h.value
+    assert L.gp_structures(9, 9, 1, ctypes.byref(h)) == 2
+    assert L.gp_structures(3, 3, 1, None) == 1
+    S = gpmap.Structures(3, 3)
+    assert L.gp_structures_get(S._h, S.D, None, None, None) == 5
+    # compute calls on a handle without device tables report a CUDA error instead of falling back (no GPU here)
+    import torch
+    if not torch.cuda.is_available():
+        en = gpmap._energies(gpmap.HP_ENERGIES, 2, 1)
+        dummy = ctypes.c_void_p(16)
+        assert L.gp_enumerate(S._h, ctypes.byref(en), 0, 512, dummy, None, None) == 4
+        assert L.gp_enumerate_simple(S._h, ctypes.byref(en), 0, 512, dummy, None, None) == 4
+    en = gpmap._energies((0, -10, -11, -23), 2, 1)  # asymmetric
+    assert L.gp_enumerate(S._h, ctypes.byref(en), 0, 512, ctypes.c_void_p(16), None, None) == 1
+    en = gpmap._energies((0, -100, -100, -23), 2, 1)  # weights beyond int8
+    assert L.gp_enumerate(S._h, ctypes.byref(en), 0, 512, ctypes.c_void_p(16), None, None) == 1
+    en = gpmap._energies(gpmap.HP_ENERGIES, 2, 0)  # threshold < 1
+    assert L.gp_enumerate(S._h, ctypes.byref(en), 0, 512, ctypes.c_void_p(16), None, None) == 1
+    en = gpmap._energies(gpmap.HP_ENERGIES, 2, 1)
+    assert L.gp_enumerate(S._h, ctypes.byref(en), 100, 12, ctypes.c_void_p(16), None, None) == 5  # misaligned
+    assert L.gp_enumerate(S._h, ctypes.byref(en), 0, 513, ctypes.c_void_p(16), None, None) == 5  # beyond 2^9
+    S.close()
+
+
+def test_seeded_generator_matches_recipe():
+    """DESIGN.md section 4 is implemented twice (oracle, library); both must produce the same stream."""
+    for seed in (200805612, 1, 2 ** 63 + 5):
+        assert np.array_equal(gpmap.seeded_matrix(seed), orc.seeded_matrix(seed))
+        assert np.array_equal(gpmap.seeded_sequences(seed, 12345, 300, 16), orc.seeded_sequences(seed, 12345, 300, 16))
+    M = gpmap.seeded_matrix(200805612)
+    assert M.min() >= -750 and M.max() <= -50 and np.array_equal(M, M.T)

@@ -1,0 +1,222 @@
+"""GPU parity: libgpmap (through the C ABI) against the CPU oracle, bit-exact (integer path: phenotype ids, gaps,
+histograms, R/D/O, pair counts, component counts).  Sizes are chosen so the oracle finishes in seconds while the GPU
+side still spans several 512-genotype supertiles, several 128-structure tiles, a ragged tail and — for N > 19 —
+several prefix batches."""
+import numpy as np
+import pytest
+import torch
+
+import workloads
+from oracle import gp_oracle as orc
+from paper_2008_05612_b200 import gpmap
+
+pytestmark = pytest.mark.gpu
+
+_lib_structs = {}
+
+
+def lib_structures(dims):
+    if dims not in _lib_structs:
+        _lib_structs[dims] = gpmap.Structures(*dims)
+    return _lib_structs[dims]
+
+
+def gpu_enumerate(S, begin, count, simple=False, threshold=1, e=gpmap.HP_ENERGIES, want_gap=True):
+    pheno = torch.full((max(count, 1),), 0x1234, dtype=torch.uint16, device="cuda")
+    gap = torch.full((max(count, 1),), 77, dtype=torch.int16, device="cuda") if want_gap else None
+    S.enumerate(begin, count, pheno, gap, e=e, threshold=threshold, simple=simple)
+    torch.cuda.synchronize()
+    return pheno[:count].cpu().numpy(), (gap[:count].cpu().numpy() if want_gap else None)
+
+
+@pytest.mark.parametrize("simple", [False, True])
+@pytest.mark.parametrize("dims", [(2, 2, 1), (3, 2, 1), (3, 3, 1), (2, 2, 2), (4, 3, 1), (4, 4, 1)])
+def test_full_small_maps(oracle_structures, dims, simple):
+    S, O = lib_structures(dims), oracle_structures(*dims)
+    total = 1 << S.N
+    ph, gap = gpu_enumerate(S, 0, total, simple=simple)
+    ph_o, gap_o = O.enumerate(0, total)
+    assert np.array_equal(ph, ph_o)
+    assert np.array_equal(gap.astype(np.int32), gap_o)
+
+
+@pytest.mark.parametrize("simple", [False, True])
+def test_ranges_5x5(oracle_structures, simple):
+    """5x5: ranges inside one prefix batch, across a batch boundary (2^19), and the ragged end of the map."""
+    S, O = lib_structures((5, 5, 1)), oracle_structures(5, 5)
+    cases = [(0, 3000), ((1 << 19) - 1024, 2048 + 37), ((1 << 25) - 5 * 512, 5 * 512), (13 * (1 << 19) + 512 * 7, 4096)]
+    cases += workloads.sample_ranges(25, 4, 2048, 512)[2:]
+    for begin, count in cases:
+        ph, gap = gpu_enumerate(S, begin, count, simple=simple)
+        ph_o, gap_o = O.enumerate(begin, count)
+        assert np.array_equal(ph, ph_o), (begin, count)
+        assert np.array_equal(gap.astype(np.int32), gap_o), (begin, count)
+
+
+@pytest.mark.parametrize("fb", [9, 12, 16, 22])
+def test_fold_bits_do_not_change_results(oracle_structures, fb):
+    """Prefix folding is exact: any split between folded prefix and contraction columns gives the same map."""
+    S, O = lib_structures((5, 5, 1)), oracle_structures(5, 5)
+    gpmap.set_fold_bits(fb)
+    try:
+        for begin, count in [(0, 2048), ((1 << 24) + (1 << fb) - 512, 1536), ((1 << 25) - 2048, 2048)]:
+            ph, gap = gpu_enumerate(S, begin, count)
+            ph_o, gap_o = O.enumerate(begin, count)
+            assert np.array_equal(ph, ph_o), (fb, begin)
+            assert np.array_equal(gap.astype(np.int32), gap_o), (fb, begin)
+    finally:
+        gpmap.set_fold_bits(19)
+
+
+@pytest.mark.parametrize("dims,n_ranges,length", [((6, 6, 1), 4, 1024), ((3, 3, 3), 3, 512)])
+def test_sampled_ranges_large_lattices(oracle_structures, dims, n_ranges, length):
+    """Configs 3 and 4 at full structure count (103 346 / 57 337 columns): sampled genotype ranges vs the oracle."""
+    S, O = lib_structures(dims), oracle_structures(*dims)
+    for begin, count in workloads.sample_ranges(S.N, n_ranges, length, 512):
+        ph, gap = gpu_enumerate(S, begin, count)
+        ph_o, gap_o = O.enumerate(begin, count)
+        assert np.array_equal(ph, ph_o), (dims, begin)
+        assert np.array_equal(gap.astype(np.int32), gap_o), (dims, begin)
+        ph_s, _ = gpu_enumerate(S, begin, count, simple=True)
+        assert np.array_equal(ph_s, ph_o), (dims, begin)
+
+
+def test_threshold_and_other_energies(oracle_structures):
+    S, O = lib_structures((4, 4, 1)), oracle_structures(4, 4)
+    for e, thr in [((0, -10, -10, -23), 4), ((0, -10, -10, -23), 11), ((0, 0, 0, -1), 1), ((-2, -7, -7, -30), 2),
+                   ((3, 1, 1, -5), 1)]:
+        ph, gap = gpu_enumerate(S, 0, 1 << 16, e=e, threshold=thr)
+        ph_o, gap_o = O.enumerate(0, 1 << 16, e=e, threshold=thr)
+        assert np.array_equal(ph, ph_o), (e, thr)
+        assert np.array_equal(gap.astype(np.int32), gap_o), (e, thr)
+        ph_s, gap_s = gpu_enumerate(S, 0, 1 << 16, e=e, threshold=thr, simple=True)
+        assert np.array_equal(ph_s, ph_o) and np.array_equal(gap_s.astype(np.int32), gap_o), (e, thr)
+
+
+def test_edge_cases():
+    S = lib_structures((4, 4, 1))
+    ph = torch.full((1024,), 0x1234, dtype=torch.uint16, device="cuda")
+    S.enumerate(0, 0, ph)  # empty range: nothing written
+    S.enumerate(512, 1, ph)  # single genotype
+    torch.cuda.synchronize()
+    assert int(ph[1]) == 0x1234
+    with pytest.raises(gpmap.GpError) as ei:
+        S.enumerate(100, 10, ph)
+    assert ei.value.status == 5
+    with pytest.raises(gpmap.GpError):
+        S.enumerate(0, (1 << 16) + 1, torch.empty((1 << 16) + 1, dtype=torch.uint16, device="cuda"))
+
+
+def test_whole_5x5_map_and_reductions(oracle_structures):
+    """Config 2 in full on the GPU: tensor-core path == CUDA-core path; designability, robustness, pair count and
+    neutral-network components of the GPU store == the oracle's reductions of the same store; whole-map totals ==
+    tests/golden/whole_maps.txt (computed by programs independent of this repository)."""
+    from tests._golden import read_whole_maps
+    S = lib_structures((5, 5, 1))
+    n = 1 << 25
+    ph = torch.empty(n, dtype=torch.uint16, device="cuda")
+    ph2 = torch.empty(n, dtype=torch.uint16, device="cuda")
+    S.enumerate(0, n, ph)
+    S.enumerate(0, n, ph2, simple=True)
+    assert torch.equal(ph.view(torch.int16), ph2.view(torch.int16))
+    hist = gpmap.designability(ph, S.C).cpu().numpy().astype(np.uint64)
+    R, Dl, Oc, pc = gpmap.robustness(ph, 25, S.C)
+    ncomp = gpmap.nn_components(ph, 25, S.C).cpu().numpy()
+    store = ph.cpu().numpy()
+    assert np.array_equal(hist, orc.designability(store, S.C))
+    Ro, Do, Oo, pco = orc.robustness(store, 25, S.C)
+    assert np.array_equal(R.cpu().numpy().astype(np.uint64), Ro)
+    assert np.array_equal(Dl.cpu().numpy().astype(np.uint64), Do)
+    assert np.array_equal(Oc.cpu().numpy().astype(np.uint64), Oo)
+    assert int(pc) == pco
+    assert np.array_equal(ncomp.astype(np.uint32), orc.nn_components(store, 25, S.C))
+    gold = read_whole_maps()["5x5"]
+    assert int(hist[:-1].sum()) == gold["folding"] and int(hist[-1]) == gold["null"]
+    assert sorted(hist[:-1].tolist(), reverse=True)[:5] == gold["top5"]
+    assert (int(Ro.sum()), int(Do.sum()), int(Oo.sum()), pco) == (gold["sumR"], gold["sumD"], gold["sumO"], gold["pairs"])
+    assert int(ncomp.sum()) == gold["nn_total"] and int((ncomp == 1).sum()) == gold["nn_one"] and int(ncomp.max()) == gold["nn_max"]
+    # reversal invariance of the map: pheno(rev g) = pheno(g), on a seeded sample
+    g = np.random.default_rng(5).integers(0, n, size=200000)
+    rev = np.zeros_like(g)
+    for i in range(25):
+        rev |= ((g >> i) & 1) << (24 - i)
+    assert np.array_equal(store[g], store[rev])
+
+
+@pytest.mark.parametrize("dims", [(3, 3, 1), (4, 4, 1), (2, 2, 2)])
+def test_reductions_small(oracle_structures, dims):
+    S, O = lib_structures(dims), oracle_structures(*dims)
+    n = 1 << S.N
+    store = O.enumerate(0, n, want_gap=False)
+    ph = torch.from_numpy(store.view(np.int16)).cuda().view(torch.uint16)
+    hist = gpmap.designability(ph, S.C).cpu().numpy().astype(np.uint64)
+    assert np.array_equal(hist, orc.designability(store, S.C))
+    R, Dl, Oc, pc = gpmap.robustness(ph, S.N, S.C)
+    Ro, Do, Oo, pco = orc.robustness(store, S.N, S.C)
+    assert np.array_equal(R.cpu().numpy().astype(np.uint64), Ro)
+    assert np.array_equal(Dl.cpu().numpy().astype(np.uint64), Do)
+    assert np.array_equal(Oc.cpu().numpy().astype(np.uint64), Oo)
+    assert int(pc) == pco
+    ncomp = gpmap.nn_components(ph, S.N, S.C).cpu().numpy()
+    assert np.array_equal(ncomp.astype(np.uint32), orc.nn_components(store, S.N, S.C))
+
+
+def test_reductions_on_synthetic_stores():
+    """Reductions are independent of how the store was produced: random stores with a paper-like null fraction,
+    ragged histogram lengths, class ids up to the 6x6 count."""
+    rng = np.random.default_rng(7)
+    for n_bits, C, p_null in [(14, 28728, 0.6), (17, 51704, 0.95), (10, 3, 0.0), (15, 549, 1.0)]:
+        n = 1 << n_bits
+        store = rng.integers(0, C, size=n).astype(np.uint16)
+        store[rng.random(n) < p_null] = 0xFFFF
+        ph = torch.from_numpy(store.view(np.int16)).cuda().view(torch.uint16)
+        for count in (n, n - 3, 5, 0):
+            hist = gpmap.designability(ph[:count] if count else ph[:0], C).cpu().numpy().astype(np.uint64)
+            assert np.array_equal(hist, orc.designability(store[:count], C)), (n_bits, count)
+        R, Dl, Oc, pc = gpmap.robustness(ph, n_bits, C)
+        Ro, Do, Oo, pco = orc.robustness(store, n_bits, C)
+        assert np.array_equal(R.cpu().numpy().astype(np.uint64), Ro)
+        assert np.array_equal(Dl.cpu().numpy().astype(np.uint64), Do)
+        assert np.array_equal(Oc.cpu().numpy().astype(np.uint64), Oo)
+        assert int(pc) == pco
+        ncomp = gpmap.nn_components(ph, n_bits, C).cpu().numpy()
+        assert np.array_equal(ncomp.astype(np.uint32), orc.nn_components(store, n_bits, C))
+
+
+def test_twenty_letter_variant(oracle_structures):
+    """a8 / config 5: seeded sequences + seeded matrix, explicit sequences, and the HP embedding special case."""
+    S, O = lib_structures((4, 4, 1)), oracle_structures(4, 4)
+    seed = workloads.SEED
+    M = gpmap.seeded_matrix(seed)
+    count = 50000 + 13
+    ph = torch.empty(count, dtype=torch.uint16, device="cuda")
+    gap = torch.empty(count, dtype=torch.int16, device="cuda")
+    first = (1 << 29) + 77
+    S.enumerate_seeded(seed, first, count, ph, gap, e=M)
+    seqs = orc.seeded_sequences(seed, first, count, 16)
+    ph_o, gap_o = O.enumerate_seqs(seqs, orc.seeded_matrix(seed), 20)
+    assert np.array_equal(ph.cpu().numpy(), ph_o)
+    assert np.array_equal(gap.cpu().numpy().astype(np.int32), np.maximum(gap_o, -32768))
+    # explicit sequences, another matrix, threshold 5
+    seqs2 = workloads.random_sequences(20000, 16, 20)
+    M2 = workloads.random_symmetric_matrix(20, -300, 40)
+    ph2 = torch.empty(20000, dtype=torch.uint16, device="cuda")
+    S.enumerate_seqs(torch.from_numpy(seqs2).cuda(), ph2, None, e=M2, alphabet=20, threshold=5)
+    assert np.array_equal(ph2.cpu().numpy(), O.enumerate_seqs(seqs2, M2, 20, threshold=5, want_gap=False))
+    # HP embedded in 20 letters (letters 0-9 = P, 10-19 = H) reproduces the HP phenotypes
+    Mhp = np.zeros((20, 20), np.int32)
+    Mhp[10:, :10] = Mhp[:10, 10:] = -10
+    Mhp[10:, 10:] = -23
+    g = np.arange(1 << 16, dtype=np.uint64)
+    bits = ((g[:, None] >> np.arange(16, dtype=np.uint64)[None, :]) & 1).astype(np.uint8)
+    letters = (bits * 10 + (g[:, None] % 7).astype(np.uint8)).astype(np.uint8)
+    ph3 = torch.empty(1 << 16, dtype=torch.uint16, device="cuda")
+    S.enumerate_seqs(torch.from_numpy(letters).cuda(), ph3, None, e=Mhp, alphabet=20)
+    assert np.array_equal(ph3.cpu().numpy(), O.enumerate(0, 1 << 16, want_gap=False))
+
+
+def test_enumerate_host_end_to_end(oracle_structures):
+    S, O = lib_structures((4, 4, 1)), oracle_structures(4, 4)
+    ph, hist = S.enumerate_host(0, 1 << 16)
+    ph_o = O.enumerate(0, 1 << 16, want_gap=False)
+    assert np.array_equal(ph, ph_o) and np.array_equal(hist, orc.designability(ph_o, S.C))
