@@ -290,7 +290,7 @@ __global__ void __launch_bounds__(THREADS, 1) scoring_kernel(const Args a, const
                 if (g < a.g_end && g >= a.out_base) {
                     const int32_t e1 = k1[m] >> KEY_SHIFT, e2v = k2[m] >> KEY_SHIFT;
                     const uint32_t col = (uint32_t)k1[m] & ((1u << KEY_SHIFT) - 1u);
-                    const bool single = (k2[m] == INT32_MAX);
+                    const bool single = (e2v == E_NONE);  // pad columns carry E_NONE too
                     const bool folds = single || (e2v - e1 >= a.threshold);
                     a.pheno[g - a.out_base] = folds ? a.class_of[col] : (uint16_t)GP_NULL_PHENO;
                     if (a.gap) a.gap[g - a.out_base] = (int16_t)(single ? GP_GAP_NONE : max(e1 - e2v, -32768));
