@@ -109,10 +109,24 @@ gp_status gp_robustness(const uint16_t* d_pheno, int n_bits, uint32_t n_classes,
  * single-bit flips.  Needs 4 bytes of private scratch per genotype; n_bits <= 30.  Synchronises the stream. */
 gp_status gp_nn_components(const uint16_t* d_pheno, int n_bits, uint32_t n_classes, uint32_t* d_ncomp, void* stream);
 
-/* Whole hot path from HOST buffers (the end-to-end call): enumerate [g_begin, g_begin+g_count), copy phenotypes to
- * pheno (host, nullable) and the histogram to hist (host, n_classes+1).  Synchronous. */
+/* Whole hot path from HOST buffers (the end-to-end call): enumerate [g_begin, g_begin+g_count) (a1-a4), copy the
+ * phenotypes to pheno (host, g_count, nullable) and the histogram (a5) to hist (host, n_classes+1).  If rdo is not
+ * NULL the range must be an aligned sub-cube (g_count a power of two dividing g_begin, else GP_RANGE); the neighbour
+ * pass (a6) then runs over its log2(g_count) mutable bits and rdo (host, 3*n_classes) receives neutral | deleterious |
+ * other, pair_count (host, 1, nullable) the number of connected class pairs.  The energy matrix (16 bytes) is the only
+ * host input: genotypes are implicit.  Synchronous; allocates and frees its device buffers. */
 gp_status gp_enumerate_host(const gp_structures_t* s, const gp_energies* en, uint64_t g_begin, uint64_t g_count,
-                            uint16_t* pheno, uint64_t* hist);
+                            uint16_t* pheno, uint64_t* hist, uint64_t* rdo, uint64_t* pair_count);
+
+/* Number of CUDA kernels this library has launched in this process so far (all calls, all streams). */
+uint64_t gp_launch_count(void);
+
+/* Per-kernel device timing for bench.py's roofline line.  While enabled, every launch of the kernels below is
+ * bracketed by a CUDA event pair on its own stream.  gp_kernel_time waits for those launches, returns the summed device
+ * time in milliseconds and the number of launches since the last query, and forgets them.  Off by default. */
+enum { GP_KERNEL_SCORING = 0, GP_KERNEL_IMAGE = 1, GP_KERNEL_HIST = 2, GP_KERNEL_ROBUSTNESS = 3, GP_KERNEL_COUNT = 4 };
+void gp_kernel_timing(int enable);
+gp_status gp_kernel_time(int which, double* ms_total, uint64_t* launches);
 
 const char* gp_strerror(gp_status st);
 const char* gp_last_cuda_error(void);

@@ -1,6 +1,9 @@
 // api.cu — C-ABI entry points of libgpmap (include/gpmap.h): argument checks, handle lifetime, dispatch to the kernels.
 #include <cstdio>
 #include <cstring>
+#include <atomic>
+#include <mutex>
+#include <vector>
 #include <new>
 
 #include "device_common.cuh"
@@ -12,6 +15,57 @@ void gp_set_cuda_error(cudaError_t e, const char* where) {
 }
 
 extern "C" const char* gp_last_cuda_error(void) { return g_cuda_error; }
+
+static std::atomic<uint64_t> g_launches{0};
+void gp_count_launches(unsigned n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
+extern "C" uint64_t gp_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
+
+// ---- optional per-kernel timing: one CUDA event pair per launch, on the launching stream ----
+namespace {
+struct EvPair { cudaEvent_t a, b; };
+std::mutex g_time_mu;
+bool g_time_on = false;
+std::vector<EvPair> g_time_ev[GP_KERNEL_COUNT];
+}  // namespace
+
+void gp_time_begin(int which, cudaStream_t st) {
+    if (!g_time_on) return;
+    std::lock_guard<std::mutex> lk(g_time_mu);
+    EvPair p;
+    if (cudaEventCreate(&p.a) != cudaSuccess) return;
+    if (cudaEventCreate(&p.b) != cudaSuccess) { cudaEventDestroy(p.a); return; }
+    cudaEventRecord(p.a, st);
+    g_time_ev[which].push_back(p);
+}
+void gp_time_end(int which, cudaStream_t st) {
+    if (!g_time_on) return;
+    std::lock_guard<std::mutex> lk(g_time_mu);
+    if (!g_time_ev[which].empty()) cudaEventRecord(g_time_ev[which].back().b, st);
+}
+extern "C" void gp_kernel_timing(int enable) {
+    std::lock_guard<std::mutex> lk(g_time_mu);
+    g_time_on = enable != 0;
+}
+extern "C" gp_status gp_kernel_time(int which, double* ms_total, uint64_t* launches) {
+    if (which < 0 || which >= GP_KERNEL_COUNT || !ms_total || !launches) return GP_INVALID_ARG;
+    std::lock_guard<std::mutex> lk(g_time_mu);
+    double tot = 0;
+    uint64_t n = 0;
+    gp_status st = GP_OK;
+    for (EvPair& p : g_time_ev[which]) {
+        float ms = 0;
+        cudaError_t e = cudaEventSynchronize(p.b);
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, p.a, p.b);
+        if (e == cudaSuccess) { tot += ms; n++; }
+        else { gp_set_cuda_error(e, "gp_kernel_time"); st = GP_CUDA_ERROR; }
+        cudaEventDestroy(p.a);
+        cudaEventDestroy(p.b);
+    }
+    g_time_ev[which].clear();
+    *ms_total = tot;
+    *launches = n;
+    return st;
+}
 
 extern "C" const char* gp_strerror(gp_status st) {
     switch (st) {
@@ -143,29 +197,45 @@ extern "C" gp_status gp_seeded_sequences(uint64_t seed, uint64_t first, uint64_t
     return GP_OK;
 }
 
-// End-to-end call from host buffers: device store allocated here, phenotypes and histogram copied back.
+// End-to-end call from host buffers: device store allocated here, results copied back.
 extern "C" gp_status gp_enumerate_host(const gp_structures_t* s, const gp_energies* en, uint64_t g_begin,
-                                       uint64_t g_count, uint16_t* pheno, uint64_t* hist) {
+                                       uint64_t g_count, uint16_t* pheno, uint64_t* hist, uint64_t* rdo,
+                                       uint64_t* pair_count) {
     if (!s || !hist) return GP_INVALID_ARG;
     if (s->device < 0) { gp_set_cuda_error(cudaErrorNoDevice, "handle has no device tables"); return GP_CUDA_ERROR; }
     const uint32_t C = s->C;
+    int n_bits = 0;
+    if (rdo) {  // the neighbour pass needs an aligned sub-cube of the genotype space
+        while ((1ULL << n_bits) < g_count) n_bits++;
+        if (g_count == 0 || (1ULL << n_bits) != g_count || (g_begin & (g_count - 1)) != 0) return GP_RANGE;
+    } else if (pair_count) {
+        return GP_INVALID_ARG;
+    }
     uint16_t* d_pheno = nullptr;
-    uint64_t* d_hist = nullptr;
+    uint64_t* d_out = nullptr;  // hist[C+1] | R[C] | D[C] | O[C] | pair_count
+    const size_t n_out = (size_t)C + 1 + 3 * (size_t)C + 1;
     GP_CUDA(cudaMalloc(&d_pheno, (g_count ? g_count : 1) * sizeof(uint16_t)));
-    if (cudaMalloc(&d_hist, ((size_t)C + 1) * sizeof(uint64_t)) != cudaSuccess) {
+    if (cudaMalloc(&d_out, n_out * sizeof(uint64_t)) != cudaSuccess) {
         cudaFree(d_pheno);
-        gp_set_cuda_error(cudaGetLastError(), "cudaMalloc(hist)");
+        gp_set_cuda_error(cudaGetLastError(), "cudaMalloc(outputs)");
         return GP_OUT_OF_MEMORY;
     }
+    uint64_t* d_hist = d_out;
+    uint64_t* d_rdo = d_out + C + 1;
+    uint64_t* d_pc = d_rdo + 3 * (size_t)C;
     gp_status st = gp_enumerate(s, en, g_begin, g_count, d_pheno, nullptr, nullptr);
     if (st == GP_OK) st = gp_designability(d_pheno, g_count, C, d_hist, nullptr);
+    if (st == GP_OK && rdo)
+        st = gp_robustness(d_pheno, n_bits, C, d_rdo, d_rdo + C, d_rdo + 2 * (size_t)C, pair_count ? d_pc : nullptr, nullptr);
     if (st == GP_OK) {
         cudaError_t e = cudaSuccess;
         if (pheno && g_count) e = cudaMemcpy(pheno, d_pheno, g_count * sizeof(uint16_t), cudaMemcpyDeviceToHost);
         if (e == cudaSuccess) e = cudaMemcpy(hist, d_hist, ((size_t)C + 1) * sizeof(uint64_t), cudaMemcpyDeviceToHost);
+        if (e == cudaSuccess && rdo) e = cudaMemcpy(rdo, d_rdo, 3 * (size_t)C * sizeof(uint64_t), cudaMemcpyDeviceToHost);
+        if (e == cudaSuccess && pair_count) e = cudaMemcpy(pair_count, d_pc, sizeof(uint64_t), cudaMemcpyDeviceToHost);
         if (e != cudaSuccess) { gp_set_cuda_error(e, "gp_enumerate_host copy-back"); st = GP_CUDA_ERROR; }
     }
     cudaFree(d_pheno);
-    cudaFree(d_hist);
+    cudaFree(d_out);
     return st;
 }

@@ -6,6 +6,10 @@
 #include "gpmap_internal.h"
 
 void gp_set_cuda_error(cudaError_t e, const char* where);
+void gp_count_launches(unsigned n);  // feeds gp_launch_count(): every kernel launch of the library is counted
+// Optional per-kernel device timing (gp_kernel_timing / gp_kernel_time): CUDA events around one launch on its stream.
+void gp_time_begin(int which, cudaStream_t st);
+void gp_time_end(int which, cudaStream_t st);
 
 #define GP_CUDA(call)                                 \
     do {                                              \

@@ -225,9 +225,12 @@ extern "C" gp_status gp_designability(const uint16_t* d_pheno, uint64_t count, u
     const uint64_t want = (count / 8 + 1023) / 1024;
     const int per_sm = use_smem ? (int)((224 * 1024) / (smem + 1024) > 2 ? 2 : 1) : 2;
     unsigned grid = (unsigned)(want < (uint64_t)sm_count() * per_sm ? (want ? want : 1) : (uint64_t)sm_count() * per_sm);
+    gp_time_begin(GP_KERNEL_HIST, st);
     hist_kernel<<<grid, 1024, use_smem ? smem : 0, st>>>(d_pheno, count, n_classes,
                                                          reinterpret_cast<unsigned long long*>(d_hist), use_smem);
+    gp_time_end(GP_KERNEL_HIST, st);
     GP_CUDA(cudaGetLastError());
+    gp_count_launches(1);
     return GP_OK;
 }
 
@@ -256,12 +259,16 @@ extern "C" gp_status gp_robustness(const uint16_t* d_pheno, int n_bits, uint32_t
     }
     const uint64_t n_seg = 1ULL << (n_bits > TB ? n_bits - TB : 0);
     const uint64_t cap = (uint64_t)sm_count() * 2;
+    gp_time_begin(GP_KERNEL_ROBUSTNESS, st);
     robustness_kernel<<<(unsigned)(n_seg < cap ? n_seg : cap), RTHREADS, 0, st>>>(a);
+    gp_time_end(GP_KERNEL_ROBUSTNESS, st);
     GP_CUDA(cudaGetLastError());
+    gp_count_launches(1);
     if (d_pair_count) {
         popcount_kernel<<<(unsigned)((n_words + 255) / 256 < 4096 ? (n_words + 255) / 256 : 4096), 256, 0, st>>>(
             a.bitmap, n_words, reinterpret_cast<unsigned long long*>(d_pair_count));
         GP_CUDA(cudaGetLastError());
+        gp_count_launches(1);
         GP_CUDA(cudaFreeAsync(a.bitmap, st));
     }
     return GP_OK;
@@ -281,6 +288,7 @@ extern "C" gp_status gp_nn_components(const uint16_t* d_pheno, int n_bits, uint3
     uf_link_kernel<<<grid, 256, 0, st>>>(d_pheno, parent, n_bits);
     uf_count_kernel<<<grid, 256, 0, st>>>(d_pheno, parent, n, n_classes, d_ncomp);
     GP_CUDA(cudaGetLastError());
+    gp_count_launches(3);
     GP_CUDA(cudaFreeAsync(parent, st));
     GP_CUDA(cudaStreamSynchronize(st));
     return GP_OK;

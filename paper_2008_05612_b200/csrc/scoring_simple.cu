@@ -126,6 +126,7 @@ gp_status launch_simple(const gp_structures_s* s, const gp_energies* en, int src
     GP_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     k<<<grid, BD, smem, st>>>(a, d_e);
     GP_CUDA(cudaGetLastError());
+    gp_count_launches(1);
     GP_CUDA(cudaFreeAsync(d_e, st));
     return GP_OK;
 }

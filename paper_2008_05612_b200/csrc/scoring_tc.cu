@@ -418,7 +418,9 @@ gp_status gp_launch_scoring_tc(gp_structures_s* s, const gp_hp_params& hp, uint6
         ImgArgs ia;
         ia.contacts = s->d_contacts; ia.img = (int8_t*)s->d_scratch; ia.hi_first = b0; ia.D = s->D; ia.n_tiles = n_tiles;
         ia.NBP = s->NBP; ia.fb = fb; ia.lin = hp.lin; ia.quad = hp.quad;
+        gp_time_begin(GP_KERNEL_IMAGE, st);
         build_image_kernel<<<dim3(n_tiles, n_batches), TN, 0, st>>>(ia, slots);
+        gp_time_end(GP_KERNEL_IMAGE, st);
         GP_CUDA(cudaGetLastError());
         Args a;
         a.img = (const int8_t*)s->d_scratch; a.class_of = s->d_class_of; a.pheno = d_pheno; a.gap = d_gap;
@@ -426,8 +428,11 @@ gp_status gp_launch_scoring_tc(gp_structures_s* s, const gp_hp_params& hp, uint6
         a.n_items = (uint32_t)((stop - g + SUPER - 1) / SUPER);
         a.n_tiles = n_tiles; a.D = s->D; a.fb = fb; a.k_steps = k_steps; a.threshold = hp.threshold;
         const unsigned grid = a.n_items < (uint32_t)sms ? a.n_items : (uint32_t)sms;
+        gp_time_begin(GP_KERNEL_SCORING, st);
         scoring_kernel<<<grid, THREADS, smem, st>>>(a, cols);
+        gp_time_end(GP_KERNEL_SCORING, st);
         GP_CUDA(cudaGetLastError());
+        gp_count_launches(2);
         g = stop;
     }
     (void)batch_len;

@@ -45,7 +45,11 @@ SIGNATURES = {
     "gp_designability": (ctypes.c_int, [_vp, ctypes.c_uint64, ctypes.c_uint32, _vp, _vp]),
     "gp_robustness": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_uint32, _vp, _vp, _vp, _vp, _vp]),
     "gp_nn_components": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_uint32, _vp, _vp]),
-    "gp_enumerate_host": (ctypes.c_int, [_vp, ctypes.POINTER(_Energies), ctypes.c_uint64, ctypes.c_uint64, _u16p, _u64p]),
+    "gp_enumerate_host": (ctypes.c_int, [_vp, ctypes.POINTER(_Energies), ctypes.c_uint64, ctypes.c_uint64, _vp, _u64p,
+                                         _u64p, _u64p]),
+    "gp_launch_count": (ctypes.c_uint64, []),
+    "gp_kernel_timing": (None, [ctypes.c_int]),
+    "gp_kernel_time": (ctypes.c_int, [ctypes.c_int, ctypes.POINTER(ctypes.c_double), _u64p]),
     "gp_strerror": (ctypes.c_char_p, [ctypes.c_int]),
     "gp_last_cuda_error": (ctypes.c_char_p, []),
 }
@@ -113,6 +117,25 @@ def _energies(e, alphabet, threshold):
 
 def tile():
     return int(lib().gp_tile())
+
+
+def launch_count():
+    """Kernels launched by libgpmap in this process so far."""
+    return int(lib().gp_launch_count())
+
+
+KERNEL_SCORING, KERNEL_IMAGE, KERNEL_HIST, KERNEL_ROBUSTNESS = range(4)
+
+
+def kernel_timing(enable):
+    lib().gp_kernel_timing(1 if enable else 0)
+
+
+def kernel_time(which):
+    """(total device ms, launches) of one kernel since the last query (needs kernel_timing(True))."""
+    ms, n = ctypes.c_double(), ctypes.c_uint64()
+    _check(lib().gp_kernel_time(which, ctypes.byref(ms), ctypes.byref(n)), "gp_kernel_time")
+    return ms.value, n.value
 
 
 def set_fold_bits(fb):
@@ -188,14 +211,24 @@ class Structures:
         _check(lib().gp_enumerate_seeded(self._h, ctypes.byref(en), seed, first, count, _dptr(pheno, torch.uint16),
                                          _dptr(gap, torch.int16), _stream(stream)), "gp_enumerate_seeded")
 
-    def enumerate_host(self, g_begin, g_count, e=HP_ENERGIES, threshold=1, want_pheno=True):
-        """gp_enumerate_host: numpy in/out, host<->device copies inside the call."""
+    def enumerate_host(self, g_begin, g_count, e=HP_ENERGIES, threshold=1, want_pheno=True, want_robustness=False,
+                       pheno_out=None):
+        """gp_enumerate_host: host buffers in and out, host<->device copies inside the call.  pheno_out may be a
+        caller-owned (e.g. pinned) uint16 numpy array.  Returns (pheno, hist) or (pheno, hist, R, D, O, pair_count)."""
         en = _energies(e, 2, threshold)
-        pheno = np.empty(g_count, np.uint16) if want_pheno else None
+        pheno = pheno_out if pheno_out is not None else (np.empty(g_count, np.uint16) if want_pheno else None)
+        if pheno is not None and (pheno.dtype != np.uint16 or pheno.size < g_count or not pheno.flags.c_contiguous):
+            raise ValueError("pheno_out must be a contiguous uint16 array of at least g_count entries")
         hist = np.zeros(self.C + 1, np.uint64)
+        rdo = np.zeros((3, self.C), np.uint64) if want_robustness else None
+        pc = ctypes.c_uint64()
         _check(lib().gp_enumerate_host(self._h, ctypes.byref(en), g_begin, g_count,
-                                       pheno.ctypes.data_as(_u16p) if want_pheno else None,
-                                       hist.ctypes.data_as(_u64p)), "gp_enumerate_host")
+                                       ctypes.c_void_p(pheno.ctypes.data) if pheno is not None else None,
+                                       hist.ctypes.data_as(_u64p),
+                                       rdo.ctypes.data_as(_u64p) if want_robustness else None,
+                                       ctypes.byref(pc) if want_robustness else None), "gp_enumerate_host")
+        if want_robustness:
+            return pheno, hist, rdo[0], rdo[1], rdo[2], pc.value
         return pheno, hist
 
 

@@ -220,3 +220,20 @@ def test_enumerate_host_end_to_end(oracle_structures):
     ph, hist = S.enumerate_host(0, 1 << 16)
     ph_o = O.enumerate(0, 1 << 16, want_gap=False)
     assert np.array_equal(ph, ph_o) and np.array_equal(hist, orc.designability(ph_o, S.C))
+    # with the neighbour pass, from a pinned caller buffer
+    out = np.empty(1 << 16, np.uint16)
+    ph2, hist2, R, Dl, Oc, pc = S.enumerate_host(0, 1 << 16, want_robustness=True, pheno_out=out)
+    Ro, Do, Oo, pco = orc.robustness(ph_o, 16, S.C)
+    assert ph2 is out and np.array_equal(out, ph_o) and np.array_equal(hist2, hist)
+    assert np.array_equal(R, Ro) and np.array_equal(Dl, Do) and np.array_equal(Oc, Oo) and pc == pco
+    # a sub-cube of the 5x5 map: flips restricted to the tile's own 12 low bits
+    S5, O5 = lib_structures((5, 5, 1)), oracle_structures(5, 5)
+    b = 0x1A5 << 12
+    ph5, h5, R5, D5, Oc5, pc5 = S5.enumerate_host(b, 1 << 12, want_robustness=True)
+    ph5_o = O5.enumerate(b, 1 << 12, want_gap=False)
+    Ro, Do, Oo, pco = orc.robustness(ph5_o, 12, S5.C)
+    assert np.array_equal(ph5, ph5_o) and np.array_equal(R5, Ro) and np.array_equal(D5, Do) and np.array_equal(Oc5, Oo)
+    assert pc5 == pco
+    with pytest.raises(gpmap.GpError):
+        S5.enumerate_host(512, 1 << 12, want_robustness=True)  # not an aligned sub-cube
+    assert gpmap.launch_count() > 0
