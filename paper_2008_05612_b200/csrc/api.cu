@@ -174,7 +174,7 @@ gp_status gp_check_hp(const gp_structures_s* s, const gp_energies* en, gp_hp_par
     int cmax = (s->nz > 1 && s->ny > 1 && s->nx > 1) ? 5 : 3;
     if (lin * cmax > 127 || lin * cmax < -127 || quad > 127 || quad < -127) return GP_INVALID_ARG;
     long long bound = (long long)s->NBP * (2LL * (lin < 0 ? -lin : lin) + (quad < 0 ? -quad : quad));
-    if (bound >= 8192) return GP_INVALID_ARG;
+    if (bound > 8190) return GP_INVALID_ARG;  // pad structures score 8191 (scoring_tc.cu E_PAD)
     out->a = a; out->lin = lin; out->quad = quad; out->threshold = en->threshold;
     return GP_OK;
 }

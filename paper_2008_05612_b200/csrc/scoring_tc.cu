@@ -14,8 +14,11 @@
 //
 // Tiling.  A CTA processes a "supertile" of MT*128 = 512 consecutive genotypes: four 128-row A tiles stay in shared
 // memory while every 128-structure weight tile streams through a 6-stage ring once and is used by four MMAs
-// (M=128, N=128, K=32 x k_steps), one per A tile, into four TMEM accumulators (4 x 128 columns = all 512).  Four
-// epilogue warps (one per TMEM lane quarter; thread = genotype row) drain the accumulators.
+// (M=128, N=128, K=32 x k_steps), one per A tile, into four TMEM accumulators (4 x 128 columns = all 512).  Sixteen
+// epilogue warps drain them: warp group m (four warps, one per TMEM lane quarter; thread = genotype row) owns
+// accumulator m, so every SM sub-partition has four warps whose TMEM loads and min/max work overlap, and the drain loop
+// is one small rolled body that stays in the instruction cache (the first version unrolled 16 copies of it, 100 KB of
+// SASS, and spent its time in instruction-fetch stalls: profiles/r1_scoring_v1_ncu.md).
 #include "device_common.cuh"
 
 namespace tc {
@@ -26,10 +29,13 @@ constexpr int ROWB = 128;             // bytes per operand row = one 128-byte sw
 constexpr int TILE_BYTES = TM * ROWB; // 16 KB, A tile and B stage alike
 constexpr int NSTAGE = 6;
 constexpr int SUPER = MT * TM;        // 512 genotypes
-constexpr int THREADS = 192;          // warp 0 TMA producer, warp 1 MMA issuer, warps 2-5 feature build + epilogue
+constexpr int EPI_WARPS = 4 * MT;     // warp group m = warps 2+4m .. 5+4m drains accumulator m
+constexpr int THREADS = 32 * (2 + EPI_WARPS);  // warp 0 TMA producer, warp 1 MMA issuer, then feature build + epilogue
 constexpr int MAX_FB = 22;            // 2 + 22 + 100 pairs = 124 <= 128 columns
 constexpr int KEY_SHIFT = 17;         // key = E * 2^17 + column (D < 2^17, |E| < 2^13)
 constexpr int E_NONE = 16383;         // INT32_MAX >> KEY_SHIFT: "no energy yet"
+constexpr int E_PAD = 8191;           // energy of the pad structures D..n_tiles*128-1 (bias columns 127*64 + 63): above
+                                      // every real energy (|E| <= 8190 is checked in gp_check_hp), so a pad never wins
 
 struct Cols {        // column c of the folded contraction: A byte = val * h_i * h_j  (bit 31 of the row word is always 1)
     uint8_t i[ROWB], j[ROWB], val[ROWB];
@@ -184,7 +190,7 @@ __global__ void __launch_bounds__(THREADS, 1) scoring_kernel(const Args a, const
     if (threadIdx.x == 0) {
         for (int s = 0; s < NSTAGE; s++) { mbar_init(&bar->b_full[s], 1); mbar_init(&bar->b_empty[s], 1); }
         for (int m = 0; m < MT; m++) { mbar_init(&bar->acc_full[m], 1); mbar_init(&bar->acc_empty[m], 4); }
-        mbar_init(&bar->a_full, 128);
+        mbar_init(&bar->a_full, 32 * EPI_WARPS);
         mbar_init(&bar->a_empty, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -240,61 +246,45 @@ __global__ void __launch_bounds__(THREADS, 1) scoring_kernel(const Args a, const
             }
         }
     } else {
-        // ===== feature build + epilogue: 128 threads, thread = genotype row =====
-        const uint32_t quarter = warp & 3;              // TMEM lanes 32*quarter .. +31 belong to this warp
-        const uint32_t r = quarter * 32 + lane;         // row within each 128-row tile
-        const uint32_t t_lane = tmem + ((quarter * 32u) << 16);
+        // ===== feature build + epilogue: 16 warps; warp group m owns A tile m and accumulator m; thread = genotype row =====
+        const uint32_t m = (warp - 2) >> 2;             // accumulator / A tile of this warp group
+        const uint32_t quarter = warp & 3;              // TMEM lanes 32*quarter .. +31 are the ones this warp may read
+        const uint32_t r = quarter * 32 + lane;         // row within the 128-row tile
+        const uint32_t t_acc = tmem + ((quarter * 32u) << 16) + m * TN;
+        const uint32_t lowmask = a.fb >= 32 ? 0xFFFFFFFFu : ((1u << a.fb) - 1u);
         uint32_t it = 0, item_no = 0;
         for (uint32_t item = blockIdx.x; item < a.n_items; item += gridDim.x, item_no++) {
-            const uint64_t g0 = a.g_first + (uint64_t)item * SUPER;
+            const uint64_t g = a.g_first + (uint64_t)item * SUPER + m * TM + r;
             mbar_wait(&bar->a_empty, (item_no & 1) ^ 1);
-            const uint32_t lowmask = a.fb >= 32 ? 0xFFFFFFFFu : ((1u << a.fb) - 1u);
-#pragma unroll 1
-            for (int m = 0; m < MT; m++)
-                build_a_row(sA + m * TILE_BYTES, r, (uint32_t)(g0 + m * TM + r) & lowmask, *cols);
+            build_a_row(sA + m * TILE_BYTES, r, (uint32_t)g & lowmask, *cols);
             fence_proxy_async();
             mbar_arrive(&bar->a_full);
 
-            int32_t k1[MT], k2[MT], e2[MT];
-#pragma unroll
-            for (int m = 0; m < MT; m++) { k1[m] = INT32_MAX; k2[m] = INT32_MAX; e2[m] = E_NONE; }
+            int32_t k1 = INT32_MAX, k2 = INT32_MAX, e2 = E_NONE;
+#pragma unroll 1
             for (uint32_t n = 0; n < a.n_tiles; n++, it++) {
-                const bool last = (n + 1 == a.n_tiles);
-#pragma unroll
-                for (int m = 0; m < MT; m++) {
-                    mbar_wait(&bar->acc_full[m], it & 1);
-                    tc_fence_after();
-#pragma unroll
-                    for (int ch = 0; ch < TN / 32; ch++) {
-                        int32_t v[32];
-                        tmem_ld32(t_lane + m * TN + ch * 32, v);
-                        tmem_ld_wait();
-                        if (ch == TN / 32 - 1) {  // accumulator m fully read: hand it back to the MMA warp
-                            tc_fence_before();
-                            __syncwarp();
-                            if (lane == 0) mbar_arrive(&bar->acc_empty[m]);
-                        }
-                        const uint32_t col0 = n * TN + ch * 32;
-                        if (last) {
-#pragma unroll
-                            for (int j = 0; j < 32; j++)
-                                if (col0 + j >= a.D) v[j] = E_NONE;  // pad columns never win
-                        }
-                        fold_chunk(v, col0, k1[m], k2[m], e2[m]);
+                mbar_wait(&bar->acc_full[m], it & 1);
+                tc_fence_after();
+#pragma unroll 1
+                for (uint32_t ch = 0; ch < TN / 32; ch++) {
+                    int32_t v[32];
+                    tmem_ld32(t_acc + ch * 32, v);
+                    tmem_ld_wait();
+                    if (ch == TN / 32 - 1) {  // accumulator fully read: hand it back to the MMA warp
+                        tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(&bar->acc_empty[m]);
                     }
+                    fold_chunk(v, n * TN + ch * 32, k1, k2, e2);
                 }
             }
-#pragma unroll
-            for (int m = 0; m < MT; m++) {
-                const uint64_t g = g0 + (uint64_t)m * TM + r;
-                if (g < a.g_end && g >= a.out_base) {
-                    const int32_t e1 = k1[m] >> KEY_SHIFT, e2v = k2[m] >> KEY_SHIFT;
-                    const uint32_t col = (uint32_t)k1[m] & ((1u << KEY_SHIFT) - 1u);
-                    const bool single = (e2v == E_NONE);  // pad columns carry E_NONE too
-                    const bool folds = single || (e2v - e1 >= a.threshold);
-                    a.pheno[g - a.out_base] = folds ? a.class_of[col] : (uint16_t)GP_NULL_PHENO;
-                    if (a.gap) a.gap[g - a.out_base] = (int16_t)(single ? GP_GAP_NONE : max(e1 - e2v, -32768));
-                }
+            if (g < a.g_end && g >= a.out_base) {
+                const int32_t e1 = k1 >> KEY_SHIFT, e2v = k2 >> KEY_SHIFT;
+                const uint32_t col = (uint32_t)k1 & ((1u << KEY_SHIFT) - 1u);
+                const bool single = (e2v >= E_PAD);  // D = 1: the runner-up is a pad structure
+                const bool folds = single || (e2v - e1 >= a.threshold);
+                a.pheno[g - a.out_base] = folds ? a.class_of[col] : (uint16_t)GP_NULL_PHENO;
+                if (a.gap) a.gap[g - a.out_base] = (int16_t)(single ? GP_GAP_NONE : max(e1 - e2v, -32768));
             }
         }
     }
@@ -348,6 +338,9 @@ __global__ void __launch_bounds__(TN) build_image_kernel(const ImgArgs a, const 
         }
         tile[swz(r, 0)] = (int8_t)(bias >> 6);   // x 64
         tile[swz(r, 1)] = (int8_t)(bias & 63);   // x 1
+    } else {                                     // pad structure: energy E_PAD for every genotype
+        tile[swz(r, 0)] = 127;
+        tile[swz(r, 1)] = 63;
     }
     __syncthreads();
     uint4* dst = reinterpret_cast<uint4*>(a.img + ((uint64_t)blockIdx.y * a.n_tiles + n) * TILE_BYTES);
