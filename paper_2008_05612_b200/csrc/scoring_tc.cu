@@ -24,7 +24,9 @@
 namespace tc {
 
 constexpr int MT = 4;                 // genotype tiles per supertile
-constexpr int TM = 128, TN = 128;     // MMA tile: genotypes x structures
+constexpr int TM = 128, TN = 128;     // weight tile: 128 structures; genotype tile: 128 rows
+constexpr int HN = 64;                // the epilogue drains 64 columns at a time; with NH = 2 (template) one MMA also
+                                      // covers 64 structures, so accumulator m is two independent 64-column buffers
 constexpr int ROWB = 128;             // bytes per operand row = one 128-byte swizzle span = up to 128 int8 features
 constexpr int TILE_BYTES = TM * ROWB; // 16 KB, A tile and B stage alike
 constexpr int NSTAGE = 6;
@@ -81,6 +83,20 @@ __device__ __forceinline__ void mma_i8(uint32_t d_tmem, uint64_t adesc, uint64_t
         "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p;\n\t}" ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc),
         "r"(accumulate) : "memory");
 }
+template <bool ACC>
+__device__ __forceinline__ void mma_i8_c(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc) {
+    if (ACC)
+        asm volatile("{\n\t.reg .pred p;\n\tsetp.eq.u32 p, 1, 1;\n\t"
+                     "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p;\n\t}" ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc) : "memory");
+    else
+        asm volatile("{\n\t.reg .pred p;\n\tsetp.eq.u32 p, 1, 0;\n\t"
+                     "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p;\n\t}" ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc) : "memory");
+}
+__device__ __forceinline__ bool elect_one() {
+    uint32_t pred;
+    asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(pred));
+    return pred != 0;
+}
 __device__ __forceinline__ void tmem_ld32(uint32_t taddr, int32_t (&v)[32]) {
     asm volatile(
         "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
@@ -92,14 +108,26 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, int32_t (&v)[32]) {
           "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
         : "r"(taddr) : "memory");
 }
+// 128 accumulator columns as 64 registers: .pack::16b keeps the low 16 bits of each 32-bit column and packs two
+// adjacent columns per register (column 2i in the low half of v[i], column 2i+1 in the high half).  Energies are
+// |E| <= 8191, so the low 16 bits are the exact int16 value.
+__device__ __forceinline__ void tmem_ld64_pack16(uint32_t taddr, uint32_t (&v)[64]) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x64.pack::16b.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31, %32, %33, %34, %35, %36, %37, %38, %39, %40, %41, %42, %43, %44, %45, %46, %47, %48, %49, %50, %51, %52, %53, %54, %55, %56, %57, %58, %59, %60, %61, %62, %63}, [%64];"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]), "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]), "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31]), "=r"(v[32]), "=r"(v[33]), "=r"(v[34]), "=r"(v[35]), "=r"(v[36]), "=r"(v[37]), "=r"(v[38]), "=r"(v[39]), "=r"(v[40]), "=r"(v[41]), "=r"(v[42]), "=r"(v[43]), "=r"(v[44]), "=r"(v[45]), "=r"(v[46]), "=r"(v[47]), "=r"(v[48]), "=r"(v[49]), "=r"(v[50]), "=r"(v[51]), "=r"(v[52]), "=r"(v[53]), "=r"(v[54]), "=r"(v[55]), "=r"(v[56]), "=r"(v[57]), "=r"(v[58]), "=r"(v[59]), "=r"(v[60]), "=r"(v[61]), "=r"(v[62]), "=r"(v[63])
+        : "r"(taddr) : "memory");
+}
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
 // shared-memory matrix descriptor: K-major, 128-byte swizzle, 8-row groups 1024 B apart (rows are 128 B)
 __device__ __forceinline__ uint64_t smem_desc(uint32_t saddr) {
     return (uint64_t)((saddr & 0x3FFFFu) >> 4) | (1ULL << 16) | ((uint64_t)(1024 >> 4) << 32) | (1ULL << 46) | (2ULL << 61);
 }
-// instruction descriptor: D = s32, A = B = s8, both K-major, N = 128, M = 128
-constexpr uint32_t IDESC = (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(TN >> 3) << 17) | ((uint32_t)(TM >> 4) << 24);
+// instruction descriptor: D = s32, A = B = s8, both K-major, N = n, M = 128
+__host__ __device__ constexpr uint32_t idesc_for(int n) {
+    return (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(TM >> 4) << 24);
+}
 
 // byte offset of (row r, byte c) inside a 128-byte-swizzled tile with 128-byte rows
 __host__ __device__ __forceinline__ uint32_t swz(uint32_t r, uint32_t c) {
@@ -120,6 +148,7 @@ struct Args {
     int fb;                   // folded (varying) low bits
     int k_steps;              // 32-byte K steps actually used (1..4)
     int threshold;
+    int dbg;                  // measurement hook (gp_set_debug): 1 = skip the min/argmin fold, 2 = also skip the TMEM loads
 };
 
 // ---- a1: feature rows -----------------------------------------------------------------------------------------------
@@ -150,31 +179,76 @@ __device__ __forceinline__ void build_a_row(uint8_t* a_tile, uint32_t r, uint32_
 // Filter: eight columns are rescanned only if their minimum is strictly below the current second-smallest energy;
 // an energy equal to it cannot change (k1, k2) because columns arrive in increasing order.
 __device__ __forceinline__ int min3(int a, int b, int c) { return min(a, min(b, c)); }
+__device__ __forceinline__ int min8(const int32_t* u) {
+    return min3(min3(u[0], u[1], u[2]), min3(u[3], u[4], u[5]), min(u[6], u[7]));
+}
 
-__device__ __forceinline__ void fold_chunk(const int32_t (&v)[32], uint32_t col0, int32_t& k1, int32_t& k2, int32_t& e2) {
+// 64 columns at a time: one test on the minimum of all 64 (36 min ops, 0.56 per energy); only when some energy is
+// strictly below the running second-smallest are the eight 8-column groups tested and the hit ones rescanned.
+__device__ __forceinline__ void fold_half(const int32_t (&v)[HN], uint32_t col0, int32_t& k1, int32_t& k2, int32_t& e2) {
+    int32_t g[8];
 #pragma unroll
-    for (int s = 0; s < 4; s++) {
-        const int32_t* u = &v[8 * s];
-        const int32_t sm = min3(min3(u[0], u[1], u[2]), min3(u[3], u[4], u[5]), min(u[6], u[7]));
-        if (sm < e2) {
+    for (int s = 0; s < 8; s++) g[s] = min8(&v[8 * s]);
+    if (min8(g) < e2) {
 #pragma unroll
-            for (int j = 0; j < 8; j++) {
-                const int32_t key = u[j] * (1 << KEY_SHIFT) + (int32_t)(col0 + 8 * s + j);
-                k2 = min(k2, max(k1, key));
-                k1 = min(k1, key);
+        for (int s = 0; s < 8; s++) {
+            if (g[s] < e2) {
+#pragma unroll
+                for (int j = 0; j < 8; j++) {
+                    const int32_t key = v[8 * s + j] * (1 << KEY_SHIFT) + (int32_t)(col0 + 8 * s + j);
+                    k2 = min(k2, max(k1, key));
+                    k1 = min(k1, key);
+                }
+                e2 = k2 >> KEY_SHIFT;
             }
-            e2 = k2 >> KEY_SHIFT;
+        }
+    }
+}
+
+// The same filter on packed int16 pairs (two columns per register): per-halfword signed min (VIMNMX.S16X2-class DPX
+// instructions), 22 ALU ops per 64 columns instead of 37.  "some halfword of x is below e2" <=> min(x, E2) != E2 with
+// E2 = (e2, e2).
+__device__ __forceinline__ uint32_t pmin3(uint32_t a, uint32_t b, uint32_t c) { return __vimin3_s16x2(a, b, c); }
+__device__ __forceinline__ uint32_t pmin(uint32_t a, uint32_t b) { return __vmins2(a, b); }
+__device__ __forceinline__ uint32_t pack2(int32_t e) { return ((uint32_t)e & 0xFFFFu) * 0x10001u; }
+
+__device__ __forceinline__ void fold_half_packed(const uint32_t* w, uint32_t col0, int32_t& k1, int32_t& k2, uint32_t& E2) {
+    uint32_t g[8];
+#pragma unroll
+    for (int s = 0; s < 8; s++) g[s] = pmin3(w[4 * s], w[4 * s + 1], pmin(w[4 * s + 2], w[4 * s + 3]));
+    const uint32_t all = pmin3(pmin3(g[0], g[1], g[2]), pmin3(g[3], g[4], g[5]), pmin(g[6], g[7]));
+    if (pmin(all, E2) != E2) {
+#pragma unroll
+        for (int s = 0; s < 8; s++) {
+            if (pmin(g[s], E2) != E2) {
+#pragma unroll
+                for (int j = 0; j < 4; j++) {
+                    const uint32_t x = w[4 * s + j];
+                    const int32_t lo = (int32_t)(int16_t)(x & 0xFFFFu), hi = (int32_t)x >> 16;
+                    const int32_t c = (int32_t)(col0 + 8 * s + 2 * j);
+                    const int32_t key0 = lo * (1 << KEY_SHIFT) + c, key1 = hi * (1 << KEY_SHIFT) + c + 1;
+                    k2 = min(k2, max(k1, key0));
+                    k1 = min(k1, key0);
+                    k2 = min(k2, max(k1, key1));
+                    k1 = min(k1, key1);
+                }
+                E2 = pack2(k2 >> KEY_SHIFT);
+            }
         }
     }
 }
 
 struct __align__(8) Barriers {
     uint64_t b_full[NSTAGE], b_empty[NSTAGE];
-    uint64_t acc_full[MT], acc_empty[MT];
+    uint64_t acc_full[MT][2], acc_empty[MT][2];
     uint64_t a_full, a_empty;
     uint32_t tmem_base;
 };
 
+// KS = 32-byte K steps per MMA chain (1..4); NH = 1: one N=128 MMA chain per accumulator, NH = 2: two N=64 chains into
+// independent halves (the tensor pipe refills one half while the other is drained).  PACK (NH = 1 only): the epilogue
+// reads the whole accumulator as packed int16 pairs, releases it at once and folds with two-lane SIMD min.
+template <int KS, int NH, bool PACK>
 __global__ void __launch_bounds__(THREADS, 1) scoring_kernel(const Args a, const Cols cols_in) {
     extern __shared__ unsigned char smem_dyn[];
     unsigned char* smem = reinterpret_cast<unsigned char*>(((uintptr_t)smem_dyn + 1023) & ~(uintptr_t)1023);
@@ -182,6 +256,8 @@ __global__ void __launch_bounds__(THREADS, 1) scoring_kernel(const Args a, const
     uint8_t* sB = smem + MT * TILE_BYTES;                 // NSTAGE tiles
     Barriers* bar = reinterpret_cast<Barriers*>(sB + NSTAGE * TILE_BYTES);
     Cols* cols = reinterpret_cast<Cols*>(bar + 1);
+    constexpr int MN = TN / NH;                           // structures per MMA
+    constexpr uint32_t IDESC = idesc_for(MN);
 
     const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
@@ -189,7 +265,8 @@ __global__ void __launch_bounds__(THREADS, 1) scoring_kernel(const Args a, const
         reinterpret_cast<uint8_t*>(cols)[i] = reinterpret_cast<const uint8_t*>(&cols_in)[i];
     if (threadIdx.x == 0) {
         for (int s = 0; s < NSTAGE; s++) { mbar_init(&bar->b_full[s], 1); mbar_init(&bar->b_empty[s], 1); }
-        for (int m = 0; m < MT; m++) { mbar_init(&bar->acc_full[m], 1); mbar_init(&bar->acc_empty[m], 4); }
+        for (int m = 0; m < MT; m++)
+            for (int h = 0; h < 2; h++) { mbar_init(&bar->acc_full[m][h], 1); mbar_init(&bar->acc_empty[m][h], 4); }
         mbar_init(&bar->a_full, 32 * EPI_WARPS);
         mbar_init(&bar->a_empty, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -204,46 +281,59 @@ __global__ void __launch_bounds__(THREADS, 1) scoring_kernel(const Args a, const
     const uint32_t tmem = bar->tmem_base;
 
     if (warp == 0) {
-        // ===== producer: stream every weight tile of the item's batch image through the ring =====
-        if (lane == 0) {
-            uint32_t it = 0;
-            for (uint32_t item = blockIdx.x; item < a.n_items; item += gridDim.x) {
-                const uint64_t g0 = a.g_first + (uint64_t)item * SUPER;
-                const uint64_t batch = (g0 >> a.fb) - (a.g_first >> a.fb);
-                const int8_t* img = a.img + batch * (uint64_t)a.n_tiles * TILE_BYTES;
-                for (uint32_t n = 0; n < a.n_tiles; n++, it++) {
-                    const uint32_t s = it % NSTAGE, ph = (it / NSTAGE) & 1;
-                    mbar_wait(&bar->b_empty[s], ph ^ 1);
+        // ===== producer: stream every weight tile of the item's batch image through the ring.  The whole warp runs the
+        // loop (uniform control flow); one elected lane issues the copies. =====
+        uint32_t it = 0;
+        for (uint32_t item = blockIdx.x; item < a.n_items; item += gridDim.x) {
+            const uint64_t g0 = a.g_first + (uint64_t)item * SUPER;
+            const uint64_t batch = (g0 >> a.fb) - (a.g_first >> a.fb);
+            const int8_t* img = a.img + batch * (uint64_t)a.n_tiles * TILE_BYTES;
+            for (uint32_t n = 0; n < a.n_tiles; n++, it++) {
+                const uint32_t s = it % NSTAGE, ph = (it / NSTAGE) & 1;
+                mbar_wait(&bar->b_empty[s], ph ^ 1);
+                if (elect_one()) {
                     mbar_expect_tx(&bar->b_full[s], TILE_BYTES);
                     bulk_g2s(sB + s * TILE_BYTES, img + (uint64_t)n * TILE_BYTES, TILE_BYTES, &bar->b_full[s]);
                 }
+                __syncwarp();
             }
         }
     } else if (warp == 1) {
-        // ===== MMA issuer: one thread =====
-        if (lane == 0) {
-            uint32_t it = 0, item_no = 0;
-            for (uint32_t item = blockIdx.x; item < a.n_items; item += gridDim.x, item_no++) {
-                mbar_wait(&bar->a_full, item_no & 1);
+        // ===== MMA issuer: warp-uniform loop, one elected lane issues =====
+        const uint64_t a_desc0 = smem_desc(smem_u32(sA));
+        const uint64_t b_desc0 = smem_desc(smem_u32(sB));
+        uint32_t it = 0, item_no = 0;
+        for (uint32_t item = blockIdx.x; item < a.n_items; item += gridDim.x, item_no++) {
+            mbar_wait(&bar->a_full, item_no & 1);
+            tc_fence_after();
+            for (uint32_t n = 0; n < a.n_tiles; n++, it++) {
+                const uint32_t s = it % NSTAGE, ph = (it / NSTAGE) & 1;
+                mbar_wait(&bar->b_full[s], ph);
                 tc_fence_after();
-                for (uint32_t n = 0; n < a.n_tiles; n++, it++) {
-                    const uint32_t s = it % NSTAGE, ph = (it / NSTAGE) & 1;
-                    mbar_wait(&bar->b_full[s], ph);
-                    tc_fence_after();
-                    const uint32_t b_addr = smem_u32(sB + s * TILE_BYTES);
+                const uint64_t bd = b_desc0 + (uint64_t)(s * (TILE_BYTES >> 4));
+#pragma unroll
+                for (int h = 0; h < NH; h++) {
 #pragma unroll
                     for (int m = 0; m < MT; m++) {
-                        mbar_wait(&bar->acc_empty[m], (it & 1) ^ 1);
+                        mbar_wait(&bar->acc_empty[m][h], (it & 1) ^ 1);
                         tc_fence_after();
-                        const uint32_t a_addr = smem_u32(sA + m * TILE_BYTES);
-                        for (int k = 0; k < a.k_steps; k++)
-                            mma_i8(tmem + m * TN, smem_desc(a_addr + k * 32), smem_desc(b_addr + k * 32), IDESC, k > 0);
-                        tc_commit(&bar->acc_full[m]);
+                        if (elect_one()) {
+                            const uint32_t d = tmem + m * TN + h * MN;
+                            const uint64_t ad = a_desc0 + (uint64_t)((m * TILE_BYTES) >> 4);
+                            const uint64_t bdh = bd + (uint64_t)((h * MN * ROWB) >> 4);
+                            mma_i8_c<false>(d, ad, bdh, IDESC);
+#pragma unroll
+                            for (int k = 1; k < KS; k++) mma_i8_c<true>(d, ad + 2 * k, bdh + 2 * k, IDESC);
+                            tc_commit(&bar->acc_full[m][h]);
+                        }
+                        __syncwarp();
                     }
-                    tc_commit(&bar->b_empty[s]);
                 }
-                tc_commit(&bar->a_empty);
+                if (elect_one()) tc_commit(&bar->b_empty[s]);
+                __syncwarp();
             }
+            if (elect_one()) tc_commit(&bar->a_empty);
+            __syncwarp();
         }
     } else {
         // ===== feature build + epilogue: 16 warps; warp group m owns A tile m and accumulator m; thread = genotype row =====
@@ -260,22 +350,49 @@ __global__ void __launch_bounds__(THREADS, 1) scoring_kernel(const Args a, const
             fence_proxy_async();
             mbar_arrive(&bar->a_full);
 
-            int32_t k1 = INT32_MAX, k2 = INT32_MAX, e2 = E_NONE;
+            int32_t k1 = INT32_MAX, k2 = INT32_MAX;
+            if (PACK) {
+                uint32_t E2 = pack2(E_NONE);
 #pragma unroll 1
-            for (uint32_t n = 0; n < a.n_tiles; n++, it++) {
-                mbar_wait(&bar->acc_full[m], it & 1);
-                tc_fence_after();
-#pragma unroll 1
-                for (uint32_t ch = 0; ch < TN / 32; ch++) {
-                    int32_t v[32];
-                    tmem_ld32(t_acc + ch * 32, v);
-                    tmem_ld_wait();
-                    if (ch == TN / 32 - 1) {  // accumulator fully read: hand it back to the MMA warp
-                        tc_fence_before();
-                        __syncwarp();
-                        if (lane == 0) mbar_arrive(&bar->acc_empty[m]);
+                for (uint32_t n = 0; n < a.n_tiles; n++, it++) {
+                    mbar_wait(&bar->acc_full[m][0], it & 1);
+                    tc_fence_after();
+                    uint32_t w[2 * 32];
+                    if (!(a.dbg & 2)) {
+                        tmem_ld64_pack16(t_acc, w);
+                        tmem_ld_wait();
                     }
-                    fold_chunk(v, n * TN + ch * 32, k1, k2, e2);
+                    tc_fence_before();  // the accumulator is in registers: hand it back to the MMA warp
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(&bar->acc_empty[m][0]);
+                    if (!a.dbg) {
+                        fold_half_packed(&w[0], n * TN, k1, k2, E2);
+                        fold_half_packed(&w[32], n * TN + HN, k1, k2, E2);
+                    }
+                }
+            } else {
+                int32_t e2 = E_NONE;
+#pragma unroll 1
+                for (uint32_t n = 0; n < a.n_tiles; n++, it++) {
+#pragma unroll 1
+                    for (uint32_t h = 0; h < 2; h++) {
+                        if (NH == 2 || h == 0) {
+                            mbar_wait(&bar->acc_full[m][NH == 2 ? h : 0], it & 1);
+                            tc_fence_after();
+                        }
+                        int32_t v[HN];
+                        if (!(a.dbg & 2)) {
+                            tmem_ld32(t_acc + h * HN, *reinterpret_cast<int32_t(*)[32]>(&v[0]));
+                            tmem_ld32(t_acc + h * HN + 32, *reinterpret_cast<int32_t(*)[32]>(&v[32]));
+                            tmem_ld_wait();
+                        }
+                        if (NH == 2 || h == 1) {  // the buffer is in registers: hand it back to the MMA warp
+                            tc_fence_before();
+                            __syncwarp();
+                            if (lane == 0) mbar_arrive(&bar->acc_empty[m][NH == 2 ? h : 0]);
+                        }
+                        if (!a.dbg) fold_half(v, n * TN + h * HN, k1, k2, e2);
+                    }
                 }
             }
             if (g < a.g_end && g >= a.out_base) {
@@ -293,6 +410,17 @@ __global__ void __launch_bounds__(THREADS, 1) scoring_kernel(const Args a, const
     if (warp == 1) {
         tc_fence_after();
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem) : "memory");
+    }
+}
+
+typedef void (*scoring_fn)(const Args, const Cols);
+template <int NH, bool PACK>
+scoring_fn scoring_for(int ks) {
+    switch (ks) {
+        case 1: return scoring_kernel<1, NH, PACK>;
+        case 2: return scoring_kernel<2, NH, PACK>;
+        case 3: return scoring_kernel<3, NH, PACK>;
+        default: return scoring_kernel<4, NH, PACK>;
     }
 }
 
@@ -348,6 +476,9 @@ __global__ void __launch_bounds__(TN) build_image_kernel(const ImgArgs a, const 
 }
 
 int g_fold_bits = 19;  // 2 + 19 + 72 = 93 columns -> 3 K steps
+int g_halves = 1;      // NH of scoring_kernel
+int g_debug = 0;
+int g_pack = 1;        // PACK of scoring_kernel
 
 }  // namespace tc
 
@@ -355,6 +486,14 @@ int g_fold_bits = 19;  // 2 + 19 + 72 = 93 columns -> 3 K steps
 extern "C" int gp_set_fold_bits(int fb) {
     if (fb < 9 || fb > tc::MAX_FB) return -1;
     tc::g_fold_bits = fb;
+    return 0;
+}
+
+extern "C" int gp_set_debug(int d) { tc::g_debug = d; return 0; }  // measurement hook: results are garbage when non-zero
+extern "C" int gp_set_pack(int p) { tc::g_pack = p != 0; return 0; }
+extern "C" int gp_set_halves(int nh) {  // test / tuning hook
+    if (nh != 1 && nh != 2) return -1;
+    tc::g_halves = nh;
     return 0;
 }
 
@@ -387,7 +526,10 @@ gp_status gp_launch_scoring_tc(gp_structures_s* s, const gp_hp_params& hp, uint6
     GP_CUDA(cudaGetDevice(&dev));
     GP_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
     const size_t smem = (size_t)(MT + NSTAGE) * TILE_BYTES + sizeof(Barriers) + sizeof(Cols) + 1024 + 64;
-    GP_CUDA(cudaFuncSetAttribute(scoring_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const scoring_fn kernel = g_halves == 2 ? scoring_for<2, false>(k_steps)
+                              : g_pack      ? scoring_for<1, true>(k_steps)
+                                            : scoring_for<1, false>(k_steps);
+    GP_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
 
     // batches of 2^fb genotypes share a weight image; a launch covers up to `group` batches
     const uint64_t batch_len = 1ULL << fb;
@@ -419,10 +561,10 @@ gp_status gp_launch_scoring_tc(gp_structures_s* s, const gp_hp_params& hp, uint6
         a.img = (const int8_t*)s->d_scratch; a.class_of = s->d_class_of; a.pheno = d_pheno; a.gap = d_gap;
         a.g_first = g; a.g_end = stop; a.out_base = g_begin;
         a.n_items = (uint32_t)((stop - g + SUPER - 1) / SUPER);
-        a.n_tiles = n_tiles; a.D = s->D; a.fb = fb; a.k_steps = k_steps; a.threshold = hp.threshold;
+        a.n_tiles = n_tiles; a.D = s->D; a.fb = fb; a.k_steps = k_steps; a.threshold = hp.threshold; a.dbg = g_debug;
         const unsigned grid = a.n_items < (uint32_t)sms ? a.n_items : (uint32_t)sms;
         gp_time_begin(GP_KERNEL_SCORING, st);
-        scoring_kernel<<<grid, THREADS, smem, st>>>(a, cols);
+        kernel<<<grid, THREADS, smem, st>>>(a, cols);
         gp_time_end(GP_KERNEL_SCORING, st);
         GP_CUDA(cudaGetLastError());
         gp_count_launches(2);
