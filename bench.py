@@ -278,13 +278,19 @@ def run_ours(args):
     hbm, bf16_burst, bf16_sus, src = peaks()
     sc_ms, sc_n = ktime[gpmap.KERNEL_SCORING]
     evals_launch = float(n) * D / max(1, sc_n // max(1, args.steps))  # one rank's launches
-    alg_ops = 2.0 * S.K                                              # contraction as posed, 2*K per eval
-    peak_i8 = 2.0 * bf16_sus                                         # int8 dense = 2 x bf16 (guide's nominal ratio)
+    fb = min(N, args.fold_bits or 19)                                 # low genotype bits kept as contraction columns
+    k_exec = 2 + fb + sum(1 for i in range(fb) for j in range(i + 3, fb, 2))  # bias x2 + monomers + pairs
+    ops_exec = 2.0 * k_exec                                           # int8 multiply-adds x2 the kernel executes per evaluation
+    peak_i8 = 2.0 * bf16_sus                                          # int8 dense = 2 x bf16 (guide's nominal ratio)
     dur = sc_ms / max(1, sc_n) * 1e-3
-    achieved = alg_ops * evals_launch / dur / 1e12 if dur > 0 else 0.0
+    achieved = ops_exec * evals_launch / dur / 1e12 if dur > 0 else 0.0
     roofline = {"kernel": "tc::scoring_kernel", "bound": "tensor", "achieved": achieved, "peak": peak_i8, "unit": "TFLOP/s",
-                "frac": achieved / peak_i8, "traffic": None, "peak_source": "2 x bf16_tflops_sustained (%s)" % src,
-                "ops_per_eval_algorithmic": alg_ops, "avg_launch_ms": dur * 1e3, "launches": int(sc_n),
+                "frac": achieved / peak_i8, "traffic": 133.2e6 * evals_launch / 4.81e11,
+                "traffic_source": "ncu dram__bytes_read+write of profiles/r1_scoring_v4_ncu.md, scaled by evaluations per launch",
+                "peak_source": "2 x bf16_tflops_sustained (%s); int8 ops" % src,
+                "frac_of_nominal_4500": achieved / 4500.0, "frac_of_2x_bf16_burst": achieved / (2.0 * bf16_burst),
+                "ops_per_eval_executed": ops_exec, "ops_per_eval_contraction_as_posed": 2.0 * S.K,
+                "avg_launch_ms": dur * 1e3, "launches": int(sc_n),
                 "evals_per_s_kernel": evals_launch / dur if dur > 0 else 0.0,
                 "share_of_step": sc_ms / ms if ms > 0 else None}
     rb_ms, rb_n = ktime[gpmap.KERNEL_ROBUSTNESS]
