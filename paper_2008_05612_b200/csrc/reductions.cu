@@ -54,12 +54,16 @@ __global__ void __launch_bounds__(1024) hist_kernel(const uint16_t* __restrict__
 }
 
 // ---------------------------------------------------------------------------------------------------------------
-// a6. Neighbour pass.  A block owns 2^TB consecutive genotypes staged in shared memory: flips of the low TB bits are
-// served on chip; each higher bit k is one coalesced, vectorised read of the partner segment base ^ 2^k.  Counts are
-// packed per genotype and flushed per class with 64-bit reductions; distinct-class pairs go to a C x C bitmap.
+// a6. Neighbour pass, bit-tiled.  The n_bits flips are handled in passes; each pass reads the
+// store ONCE.  A block stages a tile of 2^tb phenotypes in shared memory: 2^h segments (all values of the h "spread"
+// genotype bits hi_pos..hi_pos+h-1) of 2^c consecutive ids each (c = tb - h >= 3, so a segment is >= 16 B and loads
+// stay vectorised / coalesced).  Pass 0 has h = 0 and flips the tb low bits; every later pass flips its own h spread
+// bits, all on chip.  n_bits = 36, tb = 15: 15 + 8 + 8 + 5 bits = 4 passes instead of 24 partner sweeps.
+// A thread owns 8 consecutive ids (one 16-byte shared-memory vector); flips of local bits 0-2 stay inside the vector,
+// higher local bits are one LDS.128 of the partner vector.
 // ---------------------------------------------------------------------------------------------------------------
-constexpr int TB = 13;              // 2^13 genotypes = 16 KB per staged segment
-constexpr int RTHREADS = 1024;      // 8 genotypes per thread
+constexpr int ROB_TB_MAX = 15;      // 2^15 phenotypes = 64 KB of shared memory per block, two blocks per SM
+constexpr int RTHREADS = 512;
 
 struct RobArgs {
     const uint16_t* pheno;
@@ -67,86 +71,134 @@ struct RobArgs {
     uint32_t C;
     unsigned long long *R, *Dl, *O;
     uint32_t* bitmap;  // nullable; bit (min*C + max)
+    int tb, c, h, hi_pos, f0;  // tile bits, contiguous low bits, spread bits, their position, first local bit to flip
 };
 
 __device__ __forceinline__ void note_pair(const RobArgs& a, uint32_t p, uint32_t q) {
-    uint32_t lo = min(p, q), hi = max(p, q);
-    uint64_t bit = (uint64_t)lo * a.C + hi;
+    if (q < p) return;  // every unordered pair is met from both ends: record it from the smaller class only
+    uint64_t bit = (uint64_t)p * a.C + q;
     uint32_t* w = a.bitmap + (bit >> 5);
     uint32_t m = 1u << (bit & 31);
-    if (!(__ldg(w) & m) && !(*(volatile uint32_t*)w & m)) atomicOr(w, m);
+    if (!(*(volatile uint32_t*)w & m)) atomicOr(w, m);
 }
 
-__global__ void __launch_bounds__(RTHREADS) robustness_kernel(RobArgs a) {
-    __shared__ __align__(16) uint16_t seg[1 << TB];
-    const int tb = min(TB, a.n_bits);
-    const uint64_t seg_len = 1ULL << tb;
-    const uint64_t n_seg = 1ULL << (a.n_bits - tb);
-    const int per_thread = (int)((seg_len + RTHREADS - 1) / RTHREADS);  // 8 when tb = 13
-    for (uint64_t s = blockIdx.x; s < n_seg; s += gridDim.x) {
-        const uint64_t base = s << tb;
-        __syncthreads();
-        if (seg_len >= 8 * RTHREADS) {
-            const uint4* src = reinterpret_cast<const uint4*>(a.pheno + base);
-            reinterpret_cast<uint4*>(seg)[threadIdx.x] = __ldg(src + threadIdx.x);
-        } else {
-            for (uint32_t i = threadIdx.x; i < seg_len; i += RTHREADS) seg[i] = a.pheno[base + i];
-        }
-        __syncthreads();
-        // this thread's genotypes: local ids l0 .. l0+per_thread-1 (contiguous, so high-bit partners are one vector)
-        const uint32_t l0 = threadIdx.x * per_thread;
-        if (l0 >= seg_len) continue;
-        uint32_t mine[8], r[8], dl[8], o[8];
-#pragma unroll
-        for (int j = 0; j < 8; j++) { mine[j] = (j < per_thread) ? seg[l0 + j] : NULLP; r[j] = dl[j] = o[j] = 0; }
-        bool any = false;
-#pragma unroll
-        for (int j = 0; j < 8; j++) any |= (mine[j] != NULLP);
-        // low bits: on chip
-        for (int k = 0; k < tb; k++) {
-#pragma unroll
-            for (int j = 0; j < 8; j++) {
-                if (j < per_thread && mine[j] != NULLP) {
-                    uint32_t q = seg[(l0 + j) ^ (1u << k)];
-                    if (q == mine[j]) r[j]++;
-                    else if (q == NULLP) dl[j]++;
-                    else { o[j]++; if (a.bitmap) note_pair(a, mine[j], q); }
-                }
-            }
-        }
-        // high bits: partner segment, one 16-byte load per thread per bit (skipped when all 8 are null)
-        for (int k = tb; k < a.n_bits; k++) {
-            if (!any) break;
-            const uint16_t* part = a.pheno + (base ^ (1ULL << k)) + l0;
-            uint32_t q8[8];
-            if (per_thread == 8) {
-                uint4 x = __ldg(reinterpret_cast<const uint4*>(part));
-                q8[0] = x.x & 0xFFFF; q8[1] = x.x >> 16; q8[2] = x.y & 0xFFFF; q8[3] = x.y >> 16;
-                q8[4] = x.z & 0xFFFF; q8[5] = x.z >> 16; q8[6] = x.w & 0xFFFF; q8[7] = x.w >> 16;
-            } else {
-#pragma unroll
-                for (int j = 0; j < 8; j++) q8[j] = (j < per_thread) ? part[j] : NULLP;
-            }
-#pragma unroll
-            for (int j = 0; j < 8; j++) {
-                if (j < per_thread && mine[j] != NULLP) {
-                    uint32_t q = q8[j];
-                    if (q == mine[j]) r[j]++;
-                    else if (q == NULLP) dl[j]++;
-                    else { o[j]++; if (a.bitmap) note_pair(a, mine[j], q); }
-                }
-            }
-        }
-        // flush, merging runs of equal class among this thread's 8 genotypes
-#pragma unroll
-        for (int j = 0; j < 8; j++) {
-            if (mine[j] == NULLP) continue;
-            if (j < 7 && mine[j + 1] == mine[j]) { r[j + 1] += r[j]; dl[j + 1] += dl[j]; o[j + 1] += o[j]; continue; }
-            if (r[j]) atomicAdd(&a.R[mine[j]], (unsigned long long)r[j]);
-            if (dl[j]) atomicAdd(&a.Dl[mine[j]], (unsigned long long)dl[j]);
-            if (o[j]) atomicAdd(&a.O[mine[j]], (unsigned long long)o[j]);
-        }
+__device__ __forceinline__ void unpack8(const uint4& x, uint32_t (&q)[8]) {
+    q[0] = x.x & 0xFFFF; q[1] = x.x >> 16; q[2] = x.y & 0xFFFF; q[3] = x.y >> 16;
+    q[4] = x.z & 0xFFFF; q[5] = x.z >> 16; q[6] = x.w & 0xFFFF; q[7] = x.w >> 16;
+}
+
+// Per-block direct-mapped cache of per-class counts in shared memory: 3 shared atomics per flushed run instead of 3
+// 64-bit global atomics (which serialise in L2 on the popular classes).  A run whose slot is taken by another class
+// goes straight to global memory.  The cache is written back every ROB_FLUSH_TILES tiles (u32 counters) and at the end.
+constexpr uint32_t ROB_SLOTS = 2048;
+constexpr uint32_t ROB_FLUSH_TILES = 64;
+struct RobSlot { uint32_t key, r, d, o; };
+
+__device__ __forceinline__ void rob_add(const RobArgs& a, RobSlot* cache, uint32_t p, uint32_t r, uint32_t d, uint32_t o) {
+    RobSlot* s = cache + ((p * 2654435761u) >> 21);  // 11 bits
+    uint32_t k = s->key;
+    if (k == NULLP) k = atomicCAS(&s->key, NULLP, p), k = (k == NULLP) ? p : k;
+    if (k == p) {
+        if (r) atomicAdd(&s->r, r);
+        if (d) atomicAdd(&s->d, d);
+        if (o) atomicAdd(&s->o, o);
+    } else {
+        if (r) atomicAdd(&a.R[p], (unsigned long long)r);
+        if (d) atomicAdd(&a.Dl[p], (unsigned long long)d);
+        if (o) atomicAdd(&a.O[p], (unsigned long long)o);
     }
+}
+
+__device__ __forceinline__ void rob_flush(const RobArgs& a, RobSlot* cache) {
+    __syncthreads();
+    for (uint32_t i = threadIdx.x; i < ROB_SLOTS; i += blockDim.x) {
+        RobSlot s = cache[i];
+        if (s.key != NULLP) {
+            if (s.r) atomicAdd(&a.R[s.key], (unsigned long long)s.r);
+            if (s.d) atomicAdd(&a.Dl[s.key], (unsigned long long)s.d);
+            if (s.o) atomicAdd(&a.O[s.key], (unsigned long long)s.o);
+        }
+        cache[i] = RobSlot{NULLP, 0, 0, 0};
+    }
+    __syncthreads();
+}
+
+__global__ void __launch_bounds__(RTHREADS, 2) robustness_kernel(RobArgs a) {
+    extern __shared__ __align__(16) uint16_t seg[];
+    RobSlot* cache = reinterpret_cast<RobSlot*>(seg + ((size_t)1 << a.tb));
+    for (uint32_t i = threadIdx.x; i < ROB_SLOTS; i += blockDim.x) cache[i] = RobSlot{NULLP, 0, 0, 0};
+    uint32_t tiles_done = 0;
+    const uint32_t n_vec = 1u << (a.tb - 3);                       // 16-byte vectors per tile
+    const uint64_t n_tiles = 1ULL << (a.n_bits - a.tb);
+    const uint32_t cmask = (1u << a.c) - 1u;
+    const int lo_outer = a.hi_pos - a.c;                           // outer-index bits that sit below the spread bits
+    const int n_flip = a.tb - a.f0;
+    uint4* sv = reinterpret_cast<uint4*>(seg);
+    for (uint64_t t = blockIdx.x; t < n_tiles; t += gridDim.x) {
+        const uint64_t base = ((t & ((1ULL << lo_outer) - 1ULL)) << a.c) | ((t >> lo_outer) << (a.hi_pos + a.h));
+        __syncthreads();
+        for (uint32_t v = threadIdx.x; v < n_vec; v += RTHREADS) {
+            const uint32_t l = v << 3;
+            const uint64_t g = base | (l & cmask) | ((uint64_t)(l >> a.c) << a.hi_pos);
+            sv[v] = __ldg(reinterpret_cast<const uint4*>(a.pheno + g));
+        }
+        __syncthreads();
+        for (uint32_t v = threadIdx.x; v < n_vec; v += RTHREADS) {
+            uint32_t mine[8], r[8], dl[8];
+            unpack8(sv[v], mine);
+            bool any = false;
+#pragma unroll
+            for (int j = 0; j < 8; j++) { r[j] = dl[j] = 0; any |= (mine[j] != NULLP); }
+            if (!any) continue;
+            for (int k = a.f0; k < a.tb; k++) {
+                uint32_t q[8];
+                if (k < 3) {
+#pragma unroll
+                    for (int j = 0; j < 8; j++) q[j] = mine[j ^ (1 << k)];
+                } else {
+                    unpack8(sv[v ^ (1u << (k - 3))], q);
+                }
+#pragma unroll
+                for (int j = 0; j < 8; j++) {
+                    const uint32_t p = mine[j];
+                    r[j] += (q[j] == p);
+                    dl[j] += (q[j] == NULLP);
+                    if (a.bitmap && p != NULLP && q[j] != p && q[j] != NULLP) note_pair(a, p, q[j]);
+                }
+            }
+            // flush, merging runs of equal class among the 8 genotypes; other = flips - neutral - deleterious
+            uint32_t run = 0;
+#pragma unroll
+            for (int j = 0; j < 8; j++) {
+                if (mine[j] == NULLP) continue;
+                run++;
+                if (j < 7 && mine[j + 1] == mine[j]) { r[j + 1] += r[j]; dl[j + 1] += dl[j]; continue; }
+                const uint32_t o = run * (uint32_t)n_flip - r[j] - dl[j];
+                rob_add(a, cache, mine[j], r[j], dl[j], o);
+                run = 0;
+            }
+        }
+        if (++tiles_done % ROB_FLUSH_TILES == 0) rob_flush(a, cache);
+    }
+    rob_flush(a, cache);
+}
+
+// n_bits < 3 (fewer than 8 genotypes): one thread per genotype, straight from global memory.
+__global__ void robustness_tiny_kernel(RobArgs a) {
+    const uint32_t g = threadIdx.x;
+    if (g >= (1u << a.n_bits)) return;
+    const uint32_t p = a.pheno[g];
+    if (p == NULLP) return;
+    unsigned long long r = 0, d = 0, o = 0;
+    for (int k = 0; k < a.n_bits; k++) {
+        const uint32_t q = a.pheno[g ^ (1u << k)];
+        if (q == p) r++;
+        else if (q == NULLP) d++;
+        else { o++; if (a.bitmap) note_pair(a, p, q); }
+    }
+    if (r) atomicAdd(&a.R[p], r);
+    if (d) atomicAdd(&a.Dl[p], d);
+    if (o) atomicAdd(&a.O[p], o);
 }
 
 __global__ void popcount_kernel(const uint32_t* __restrict__ words, uint64_t n_words, unsigned long long* out) {
@@ -204,6 +256,8 @@ __global__ void uf_count_kernel(const uint16_t* __restrict__ pheno, const uint32
     }
 }
 
+int g_rob_tile_bits = ROB_TB_MAX;  // test hook (gp_set_rob_tile_bits): smaller tiles force the multi-pass path on small stores
+
 int sm_count() {
     int dev = 0, sms = 148;
     if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
@@ -211,6 +265,12 @@ int sm_count() {
 }
 
 }  // namespace
+
+extern "C" int gp_set_rob_tile_bits(int tb) {
+    if (tb < 4 || tb > ROB_TB_MAX) return -1;
+    g_rob_tile_bits = tb;
+    return 0;
+}
 
 extern "C" gp_status gp_designability(const uint16_t* d_pheno, uint64_t count, uint32_t n_classes, uint64_t* d_hist,
                                       void* stream) {
@@ -257,13 +317,37 @@ extern "C" gp_status gp_robustness(const uint16_t* d_pheno, int n_bits, uint32_t
         GP_CUDA(cudaMemsetAsync(a.bitmap, 0, n_words * 4, st));
         GP_CUDA(cudaMemsetAsync(d_pair_count, 0, sizeof(uint64_t), st));
     }
-    const uint64_t n_seg = 1ULL << (n_bits > TB ? n_bits - TB : 0);
-    const uint64_t cap = (uint64_t)sm_count() * 2;
-    gp_time_begin(GP_KERNEL_ROBUSTNESS, st);
-    robustness_kernel<<<(unsigned)(n_seg < cap ? n_seg : cap), RTHREADS, 0, st>>>(a);
-    gp_time_end(GP_KERNEL_ROBUSTNESS, st);
-    GP_CUDA(cudaGetLastError());
-    gp_count_launches(1);
+    if (n_bits < 3) {
+        gp_time_begin(GP_KERNEL_ROBUSTNESS, st);
+        robustness_tiny_kernel<<<1, 32, 0, st>>>(a);
+        gp_time_end(GP_KERNEL_ROBUSTNESS, st);
+        GP_CUDA(cudaGetLastError());
+        gp_count_launches(1);
+    } else {
+        const int tb = n_bits < g_rob_tile_bits ? n_bits : g_rob_tile_bits;
+        const size_t smem = ((size_t)2 << tb) + ROB_SLOTS * sizeof(RobSlot);
+        GP_CUDA(cudaFuncSetAttribute(robustness_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        const uint64_t n_tiles = 1ULL << (n_bits - tb);
+        const uint64_t cap = (uint64_t)sm_count() * 2;
+        const unsigned grid = (unsigned)(n_tiles < cap ? n_tiles : cap);
+        a.tb = tb;
+        // pass 0: the tb low bits; then up to tb-3 further bits per pass (segments stay >= 16 bytes)
+        int done = 0;
+        while (done < n_bits) {
+            if (done == 0) { a.c = tb; a.h = 0; a.hi_pos = tb; a.f0 = 0; done = tb; }
+            else {
+                int h = n_bits - done;
+                const int hmax = tb - 7 > 1 ? tb - 7 : (tb - 3 > 1 ? tb - 3 : 1);  // keep segments >= 256 B when the tile allows
+                if (h > hmax) h = hmax;
+                a.h = h; a.c = tb - h; a.hi_pos = done; a.f0 = a.c; done += h;
+            }
+            gp_time_begin(GP_KERNEL_ROBUSTNESS, st);
+            robustness_kernel<<<grid, RTHREADS, smem, st>>>(a);
+            gp_time_end(GP_KERNEL_ROBUSTNESS, st);
+            GP_CUDA(cudaGetLastError());
+            gp_count_launches(1);
+        }
+    }
     if (d_pair_count) {
         popcount_kernel<<<(unsigned)((n_words + 255) / 256 < 4096 ? (n_words + 255) / 256 : 4096), 256, 0, st>>>(
             a.bitmap, n_words, reinterpret_cast<unsigned long long*>(d_pair_count));

@@ -237,3 +237,28 @@ def test_enumerate_host_end_to_end(oracle_structures):
     with pytest.raises(gpmap.GpError):
         S5.enumerate_host(512, 1 << 12, want_robustness=True)  # not an aligned sub-cube
     assert gpmap.launch_count() > 0
+
+
+@pytest.mark.parametrize("tile_bits", [4, 7, 10, 15])
+def test_robustness_tile_sizes_agree_with_oracle(tile_bits):
+    """The bit-tiled neighbour pass gives the same counts for every tile size (small tiles force the multi-pass,
+    spread-bit path on small stores), on stores whose size is not a multiple of the pass width."""
+    rng = np.random.default_rng(11)
+    L = gpmap.lib()
+    assert L.gp_set_rob_tile_bits(tile_bits) == 0
+    try:
+        for n_bits, C, p_null in [(1, 2, 0.3), (2, 3, 0.3), (3, 5, 0.5), (9, 3, 0.4), (13, 549, 0.6), (18, 28728, 0.57)]:
+            n = 1 << n_bits
+            store = rng.integers(0, C, size=n).astype(np.uint16)
+            # clustered classes, so that neutral neighbours and equal-class runs exist
+            store = np.sort(store.reshape(-1, 4), axis=1).reshape(-1) if n >= 4 else store
+            store[rng.random(n) < p_null] = 0xFFFF
+            ph = torch.from_numpy(store.view(np.int16)).cuda().view(torch.uint16)
+            R, Dl, Oc, pc = gpmap.robustness(ph, n_bits, C)
+            Ro, Do, Oo, pco = orc.robustness(store, n_bits, C)
+            assert np.array_equal(R.cpu().numpy().astype(np.uint64), Ro), (tile_bits, n_bits)
+            assert np.array_equal(Dl.cpu().numpy().astype(np.uint64), Do), (tile_bits, n_bits)
+            assert np.array_equal(Oc.cpu().numpy().astype(np.uint64), Oo), (tile_bits, n_bits)
+            assert int(pc) == pco, (tile_bits, n_bits)
+    finally:
+        L.gp_set_rob_tile_bits(15)
