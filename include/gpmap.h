@@ -79,6 +79,13 @@ uint64_t gp_tile(void);
 gp_status gp_enumerate(const gp_structures_t* s, const gp_energies* en, uint64_t g_begin, uint64_t g_count,
                        uint16_t* d_pheno, int16_t* d_gap, void* stream);
 
+/* a1-a4 for the WHOLE map (g = 0 .. 2^N-1, d_pheno and the nullable d_gap hold 2^N entries), same results as
+ * gp_enumerate(s, en, 0, 2^N, ...), at half the work: by the reversal identity E(g, rev S) = E(rev g, S) (:391) each
+ * genotype is scored on one representative structure per class, and a genotype's list is merged with its reversed
+ * genotype's list before the uniqueness test.  executed evaluations = 2^N * C, effective = 2^N * D. */
+gp_status gp_enumerate_map(const gp_structures_t* s, const gp_energies* en, uint16_t* d_pheno, int16_t* d_gap,
+                           void* stream);
+
 /* Same contract as gp_enumerate, computed by the plain CUDA-core kernel that walks the contact table like the paper's
  * listing (:530-570).  Kept as the in-library cross-check and timing strawman; no alignment requirement. */
 gp_status gp_enumerate_simple(const gp_structures_t* s, const gp_energies* en, uint64_t g_begin, uint64_t g_count,

@@ -104,6 +104,33 @@ gp_status gp_upload_tables(gp_structures_s* s) {
         }
     GP_CUDA(cudaMalloc(&s->d_pair_ij, ij.size()));
     GP_CUDA(cudaMemcpy(s->d_pair_ij, ij.data(), ij.size(), cudaMemcpyHostToDevice));
+    // one representative (smallest directed index) per class; classes with two members first
+    {
+        std::vector<uint32_t> members(s->C, 0), rep(s->C, 0xFFFFFFFFu);
+        for (uint32_t d = 0; d < s->D; d++) {
+            members[s->class_of[d]]++;
+            if (rep[s->class_of[d]] == 0xFFFFFFFFu) rep[s->class_of[d]] = d;
+        }
+        std::vector<uint32_t> order;
+        for (uint32_t c = 0; c < s->C; c++) if (members[c] == 2) order.push_back(rep[c]);
+        const uint32_t n_nsr = (uint32_t)order.size();
+        s->n_snap = (n_nsr + 127) / 128;
+        order.resize((size_t)s->n_snap * 128, 0xFFFFFFFFu);
+        for (uint32_t c = 0; c < s->C; c++) if (members[c] == 1) order.push_back(rep[c]);
+        s->D_sym = (uint32_t)order.size();
+        const size_t row = (size_t)s->NBP * 2;
+        std::vector<uint8_t> csym(order.size() * row, 0);
+        std::vector<uint16_t> ksym(order.size(), (uint16_t)GP_NULL_PHENO);
+        for (size_t k = 0; k < order.size(); k++)
+            if (order[k] != 0xFFFFFFFFu) {
+                memcpy(&csym[k * row], &s->contacts[order[k] * row], row);
+                ksym[k] = s->class_of[order[k]];
+            }
+        GP_CUDA(cudaMalloc(&s->d_contacts_sym, csym.size() ? csym.size() : 1));
+        GP_CUDA(cudaMemcpy(s->d_contacts_sym, csym.data(), csym.size(), cudaMemcpyHostToDevice));
+        GP_CUDA(cudaMalloc(&s->d_class_sym, ksym.size() * sizeof(uint16_t)));
+        GP_CUDA(cudaMemcpy(s->d_class_sym, ksym.data(), ksym.size() * sizeof(uint16_t), cudaMemcpyHostToDevice));
+    }
     return GP_OK;
 }
 
@@ -113,6 +140,9 @@ void gp_release_device(gp_structures_s* s) {
     cudaFree(s->d_class_of);
     cudaFree(s->d_pairidx);
     cudaFree(s->d_pair_ij);
+    cudaFree(s->d_contacts_sym);
+    cudaFree(s->d_class_sym);
+    s->d_contacts_sym = nullptr; s->d_class_sym = nullptr;
     cudaFree(s->wimg.d_img);
     cudaFree(s->d_scratch);
     s->d_contacts = nullptr; s->d_class_of = nullptr; s->d_pairidx = nullptr; s->d_pair_ij = nullptr; s->wimg.d_img = nullptr; s->d_scratch = nullptr;

@@ -30,6 +30,11 @@ struct gp_structures_s {
     uint16_t* d_class_of = nullptr;
     uint16_t* d_pairidx = nullptr;       // D * NBP: pair-feature index of each contact
     uint8_t* d_pair_ij = nullptr;        // P * 2: monomers (i, j) of each pair feature
+    // reversal-reduced structure list for gp_enumerate_map (one representative per class; scoring_tc.cu): first the
+    // classes that differ from their reversal, padded to a multiple of 128 columns, then the self-reverse classes
+    uint8_t* d_contacts_sym = nullptr;   // D_sym * NBP * 2 (pad entries zero)
+    uint16_t* d_class_sym = nullptr;     // D_sym: class id of the column, 0xFFFF = pad column
+    uint32_t D_sym = 0, n_snap = 0;      // columns incl. interior pads; weight tiles holding non-self-reverse classes
     gp_weight_image wimg;
     void* d_scratch = nullptr;           // private scratch, grown on demand
     size_t scratch_bytes = 0;

@@ -19,6 +19,8 @@
 // accumulator m, so every SM sub-partition has four warps whose TMEM loads and min/max work overlap, and the drain loop
 // is one small rolled body that stays in the instruction cache (the first version unrolled 16 copies of it, 100 KB of
 // SASS, and spent its time in instruction-fetch stalls: profiles/r1_scoring_v1_ncu.md).
+#include <vector>
+
 #include "device_common.cuh"
 
 namespace tc {
@@ -148,6 +150,9 @@ struct Args {
     int fb;                   // folded (varying) low bits
     int k_steps;              // 32-byte K steps actually used (1..4)
     int threshold;
+    int4* hrec;               // map mode (gp_enumerate_map): per genotype (k1, k2) over all columns and the snapshot of
+                              // (k1, k2) after the first n_snap weight tiles; indexed like pheno; pheno/gap unused
+    uint32_t n_snap;
     int dbg;                  // measurement hook (gp_set_debug): 1 = skip the min/argmin fold, 2 = also skip the TMEM loads
 };
 
@@ -350,11 +355,12 @@ __global__ void __launch_bounds__(THREADS, 1) scoring_kernel(const Args a, const
             fence_proxy_async();
             mbar_arrive(&bar->a_full);
 
-            int32_t k1 = INT32_MAX, k2 = INT32_MAX;
+            int32_t k1 = INT32_MAX, k2 = INT32_MAX, s1 = INT32_MAX, s2 = INT32_MAX;
             if (PACK) {
                 uint32_t E2 = pack2(E_NONE);
 #pragma unroll 1
                 for (uint32_t n = 0; n < a.n_tiles; n++, it++) {
+                    if (n == a.n_snap) { s1 = k1; s2 = k2; }
                     mbar_wait(&bar->acc_full[m][0], it & 1);
                     tc_fence_after();
                     uint32_t w[2 * 32];
@@ -374,6 +380,7 @@ __global__ void __launch_bounds__(THREADS, 1) scoring_kernel(const Args a, const
                 int32_t e2 = E_NONE;
 #pragma unroll 1
                 for (uint32_t n = 0; n < a.n_tiles; n++, it++) {
+                    if (n == a.n_snap) { s1 = k1; s2 = k2; }
 #pragma unroll 1
                     for (uint32_t h = 0; h < 2; h++) {
                         if (NH == 2 || h == 0) {
@@ -395,7 +402,10 @@ __global__ void __launch_bounds__(THREADS, 1) scoring_kernel(const Args a, const
                     }
                 }
             }
-            if (g < a.g_end && g >= a.out_base) {
+            if (a.n_snap >= a.n_tiles) { s1 = k1; s2 = k2; }
+            if (a.hrec) {
+                if (g < a.g_end) a.hrec[g] = make_int4(k1, k2, s1, s2);
+            } else if (g < a.g_end && g >= a.out_base) {
                 const int32_t e1 = k1 >> KEY_SHIFT, e2v = k2 >> KEY_SHIFT;
                 const uint32_t col = (uint32_t)k1 & ((1u << KEY_SHIFT) - 1u);
                 const bool single = (e2v >= E_PAD);  // D = 1: the runner-up is a pad structure
@@ -425,42 +435,50 @@ scoring_fn scoring_for(int ks) {
 }
 
 // ---- per-prefix weight image ----------------------------------------------------------------------------------------
-struct Slots {  // column of pair (i, j), i < j < fb, in the folded contraction; 0 = not a column
-    uint8_t pair[MAX_FB * MAX_FB];
+struct Slots {  // column of pair (li, lj) of LOCAL bits li < lj in the folded contraction (0 = not a column), and
+    uint8_t pair[MAX_FB * MAX_FB];  // the local bit of every monomer (-1 = the monomer is fixed within an image)
+    int8_t loc[64];
 };
 
 struct ImgArgs {
-    const uint8_t* contacts;  // D * NBP * 2
-    int8_t* img;              // [n_batches][n_tiles][TILE_BYTES]
-    uint64_t hi_first;        // prefix (g >> fb) of batch 0; batch y has prefix hi_first + y
+    const uint8_t* contacts;   // D * NBP * 2
+    const uint16_t* class_of;  // D; 0xFFFF marks a pad column inside the list
+    int8_t* img;               // [n_images][n_tiles][TILE_BYTES]
+    const uint32_t* tile_list; // nullable: fixed-bit value of image y is tile_list[list_first + y], else gfix_first + y
+    uint64_t gfix_first;
+    uint32_t list_first;
+    int gfix_shift;            // genotype with the fixed bits of image y in place = value << gfix_shift
     uint32_t D, n_tiles;
-    int NBP, fb, lin, quad;
+    int NBP, lin, quad;
 };
 
-// One block = one 128-structure tile of one prefix.  Thread = structure: it accumulates its 128-byte weight row in
+// One block = one 128-structure tile of one image.  Thread = structure: it accumulates its 128-byte weight row in
 // shared memory (already in the swizzled layout the MMA reads), then the block writes the 16 KB tile out coalesced.
 __global__ void __launch_bounds__(TN) build_image_kernel(const ImgArgs a, const Slots slots) {
     __shared__ __align__(16) int8_t tile[TILE_BYTES];
     const uint32_t r = threadIdx.x, n = blockIdx.x;
-    const uint64_t H = a.hi_first + blockIdx.y;
+    const uint64_t G = (a.tile_list ? (uint64_t)a.tile_list[a.list_first + blockIdx.y] : a.gfix_first + blockIdx.y) << a.gfix_shift;
     for (uint32_t i = threadIdx.x; i < TILE_BYTES / 16; i += TN) reinterpret_cast<uint4*>(tile)[i] = make_uint4(0, 0, 0, 0);
     __syncthreads();
     const uint32_t d = n * TN + r;
-    if (d < a.D) {
+    if (d < a.D && a.class_of[d] != GP_NULL_PHENO) {
         const uint8_t* c = a.contacts + (size_t)d * a.NBP * 2;
         int bias = 0;
         for (int k = 0; k < a.NBP; k++) {
             const int i = c[2 * k], j = c[2 * k + 1];  // i < j
-            if (j < a.fb) {
-                tile[swz(r, 2 + i)] += (int8_t)a.lin;
-                tile[swz(r, 2 + j)] += (int8_t)a.lin;
-                tile[swz(r, slots.pair[i * MAX_FB + j])] = (int8_t)a.quad;
-            } else if (i < a.fb) {
-                const int hj = (int)((H >> (j - a.fb)) & 1ULL);
-                tile[swz(r, 2 + i)] += (int8_t)(a.lin + a.quad * hj);
+            const int li = slots.loc[i], lj = slots.loc[j];
+            const int hi = (int)((G >> i) & 1ULL), hj = (int)((G >> j) & 1ULL);
+            if (li >= 0 && lj >= 0) {
+                tile[swz(r, 2 + li)] += (int8_t)a.lin;
+                tile[swz(r, 2 + lj)] += (int8_t)a.lin;
+                tile[swz(r, slots.pair[li * MAX_FB + lj])] = (int8_t)a.quad;
+            } else if (li >= 0) {
+                tile[swz(r, 2 + li)] += (int8_t)(a.lin + a.quad * hj);
                 bias += a.lin * hj;
+            } else if (lj >= 0) {
+                tile[swz(r, 2 + lj)] += (int8_t)(a.lin + a.quad * hi);
+                bias += a.lin * hi;
             } else {
-                const int hi = (int)((H >> (i - a.fb)) & 1ULL), hj = (int)((H >> (j - a.fb)) & 1ULL);
                 bias += a.lin * (hi + hj) + a.quad * hi * hj;
             }
         }
@@ -474,6 +492,69 @@ __global__ void __launch_bounds__(TN) build_image_kernel(const ImgArgs a, const 
     uint4* dst = reinterpret_cast<uint4*>(a.img + ((uint64_t)blockIdx.y * a.n_tiles + n) * TILE_BYTES);
     for (uint32_t i = threadIdx.x; i < TILE_BYTES / 16; i += TN) dst[i] = reinterpret_cast<const uint4*>(tile)[i];
 }
+
+// Columns of the folded contraction for a set of free monomers mon[0..fb-1] (increasing): 2 bias columns, fb monomer
+// columns, one column per pair of free monomers that can touch (j - i odd and >= 3).  Returns the column count.
+static int make_columns(const int* mon, int fb, int N, Cols& cols, Slots& slots) {
+    memset(&slots, 0, sizeof(slots));
+    for (int i = 0; i < 64; i++) slots.loc[i] = -1;
+    for (int l = 0; l < fb; l++) slots.loc[mon[l]] = (int8_t)l;
+    for (int c = 0; c < ROWB; c++) { cols.i[c] = 31; cols.j[c] = 31; cols.val[c] = 0; }
+    cols.val[0] = 64;
+    cols.val[1] = 1;
+    int nc = 2;
+    for (int l = 0; l < fb; l++, nc++) { cols.i[nc] = cols.j[nc] = (uint8_t)l; cols.val[nc] = 1; }
+    for (int li = 0; li < fb; li++)
+        for (int lj = li + 1; lj < fb; lj++) {
+            const int dist = mon[lj] - mon[li];
+            if (dist < 3 || (dist & 1) == 0) continue;
+            if (nc < ROWB) {
+                cols.i[nc] = (uint8_t)li; cols.j[nc] = (uint8_t)lj; cols.val[nc] = 1;
+                slots.pair[li * MAX_FB + lj] = (uint8_t)nc;
+            }
+            nc++;
+        }
+    (void)N;
+    return nc;
+}
+
+// ---- map mode: merge the two half-lists of a genotype and its reversal -------------------------
+struct CombArgs {
+    const int4* hrec;           // [n_images][2^fb]
+    const uint32_t* tile_list;  // middle-bit value of every image of the map
+    const uint32_t* partner;    // index (in tile_list) of the image holding the reversed genotypes
+    const uint16_t* class_sym;
+    uint16_t* pheno;
+    int16_t* gap;               // nullable
+    uint32_t list_first, n_images;
+    int fb, k, N, threshold;
+};
+
+__global__ void __launch_bounds__(256) combine_kernel(const CombArgs a) {
+    const uint64_t total = (uint64_t)a.n_images << a.fb;
+    const uint32_t tmask = (1u << a.fb) - 1u, kmask = (1u << a.k) - 1u;
+    for (uint64_t idx = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (uint64_t)gridDim.x * blockDim.x) {
+        const uint32_t y = (uint32_t)(idx >> a.fb), t = (uint32_t)idx & tmask;
+        const uint32_t yp = a.partner[a.list_first + y] - a.list_first;
+        const uint32_t tr = __brev(t) >> (32 - a.fb);
+        const int4 A = a.hrec[idx];
+        const int4 B = a.hrec[((uint64_t)yp << a.fb) + tr];
+        // own list: all class representatives; reversed genotype's list: the same structures read backwards, i.e. the
+        // other member of every two-member class (self-reverse classes are in the own list only)
+        const int32_t a1 = A.x >> KEY_SHIFT, a2 = A.y >> KEY_SHIFT, b1 = B.z >> KEY_SHIFT, b2 = B.w >> KEY_SHIFT;
+        const bool own = a1 <= b1;
+        const int32_t m1 = own ? a1 : b1;
+        const int32_t m2 = own ? min(a2, b1) : min(b2, a1);
+        const uint32_t col = (uint32_t)(own ? A.x : B.z) & ((1u << KEY_SHIFT) - 1u);
+        const bool single = (m2 >= E_PAD);
+        const bool folds = single || (m2 - m1 >= a.threshold);
+        const uint64_t g = ((uint64_t)(t >> a.k) << (a.N - a.k)) | ((uint64_t)a.tile_list[a.list_first + y] << a.k) | (t & kmask);
+        a.pheno[g] = folds ? a.class_sym[col] : (uint16_t)GP_NULL_PHENO;
+        if (a.gap) a.gap[g] = (int16_t)(single ? GP_GAP_NONE : max(m1 - m2, -32768));
+    }
+}
+
+int g_sym_bits = 9;    // k of map mode: the k first and k last monomers vary inside an image
 
 int g_fold_bits = 19;  // 2 + 19 + 72 = 93 columns -> 3 K steps
 int g_halves = 1;      // NH of scoring_kernel
@@ -490,6 +571,11 @@ extern "C" int gp_set_fold_bits(int fb) {
 }
 
 extern "C" int gp_set_debug(int d) { tc::g_debug = d; return 0; }  // measurement hook: results are garbage when non-zero
+extern "C" int gp_set_sym_bits(int k) {  // test / tuning hook
+    if (k < 5 || 2 * k > tc::MAX_FB) return -1;
+    tc::g_sym_bits = k;
+    return 0;
+}
 extern "C" int gp_set_pack(int p) { tc::g_pack = p != 0; return 0; }
 extern "C" int gp_set_halves(int nh) {  // test / tuning hook
     if (nh != 1 && nh != 2) return -1;
@@ -503,20 +589,11 @@ gp_status gp_launch_scoring_tc(gp_structures_s* s, const gp_hp_params& hp, uint6
     const int N = s->N;
     const int fb = N < g_fold_bits ? N : g_fold_bits;
     if (s->D >= (1u << KEY_SHIFT)) return GP_UNSUPPORTED_LATTICE;
-    // columns
     Cols cols;
     Slots slots;
-    memset(&slots, 0, sizeof(slots));
-    for (int c = 0; c < ROWB; c++) { cols.i[c] = 31; cols.j[c] = 31; cols.val[c] = 0; }
-    cols.val[0] = 64;
-    cols.val[1] = 1;
-    int nc = 2;
-    for (int i = 0; i < fb; i++, nc++) { cols.i[nc] = cols.j[nc] = (uint8_t)i; cols.val[nc] = 1; }
-    for (int i = 0; i < fb; i++)
-        for (int j = i + 3; j < fb; j += 2, nc++) {
-            cols.i[nc] = (uint8_t)i; cols.j[nc] = (uint8_t)j; cols.val[nc] = 1;
-            slots.pair[i * MAX_FB + j] = (uint8_t)nc;
-        }
+    int mon[MAX_FB];
+    for (int i = 0; i < fb; i++) mon[i] = i;
+    const int nc = make_columns(mon, fb, N, cols, slots);
     if (nc > ROWB) return GP_INVALID_ARG;
     const int k_steps = (nc + 31) / 32;
     const uint32_t n_tiles = (s->D + TN - 1) / TN;
@@ -551,8 +628,9 @@ gp_status gp_launch_scoring_tc(gp_structures_s* s, const gp_hp_params& hp, uint6
         if (stop > g_end) stop = g_end;
         const uint32_t n_batches = (uint32_t)(((stop - 1) >> fb) - b0 + 1);
         ImgArgs ia;
-        ia.contacts = s->d_contacts; ia.img = (int8_t*)s->d_scratch; ia.hi_first = b0; ia.D = s->D; ia.n_tiles = n_tiles;
-        ia.NBP = s->NBP; ia.fb = fb; ia.lin = hp.lin; ia.quad = hp.quad;
+        ia.contacts = s->d_contacts; ia.class_of = s->d_class_of; ia.img = (int8_t*)s->d_scratch; ia.tile_list = nullptr;
+        ia.gfix_first = b0; ia.list_first = 0; ia.gfix_shift = fb; ia.D = s->D; ia.n_tiles = n_tiles;
+        ia.NBP = s->NBP; ia.lin = hp.lin; ia.quad = hp.quad;
         gp_time_begin(GP_KERNEL_IMAGE, st);
         build_image_kernel<<<dim3(n_tiles, n_batches), TN, 0, st>>>(ia, slots);
         gp_time_end(GP_KERNEL_IMAGE, st);
@@ -562,6 +640,7 @@ gp_status gp_launch_scoring_tc(gp_structures_s* s, const gp_hp_params& hp, uint6
         a.g_first = g; a.g_end = stop; a.out_base = g_begin;
         a.n_items = (uint32_t)((stop - g + SUPER - 1) / SUPER);
         a.n_tiles = n_tiles; a.D = s->D; a.fb = fb; a.k_steps = k_steps; a.threshold = hp.threshold; a.dbg = g_debug;
+        a.hrec = nullptr; a.n_snap = n_tiles;
         const unsigned grid = a.n_items < (uint32_t)sms ? a.n_items : (uint32_t)sms;
         gp_time_begin(GP_KERNEL_SCORING, st);
         kernel<<<grid, THREADS, smem, st>>>(a, cols);
@@ -572,6 +651,117 @@ gp_status gp_launch_scoring_tc(gp_structures_s* s, const gp_hp_params& hp, uint6
     }
     (void)batch_len;
     return GP_OK;
+}
+
+// Whole map through the reversal identity E(g, rev S) = E(rev g, S): every genotype is
+// scored on ONE representative per class (C columns instead of D); the energies of the other class members are those
+// of the reversed genotype on the same representatives.  An image holds the 2^(2k) genotypes that share their middle
+// N - 2k bits, so the reversed genotypes of image m are exactly image rev(m), read in bit-reversed local order.
+gp_status gp_launch_map_tc(gp_structures_s* s, const gp_hp_params& hp, uint16_t* d_pheno, int16_t* d_gap, cudaStream_t st) {
+    using namespace tc;
+    const int N = s->N;
+    int k = g_sym_bits < N / 2 ? g_sym_bits : N / 2;
+    const int fb = 2 * k, mid = N - fb;
+    if (fb < 9 || s->D_sym >= (1u << KEY_SHIFT)) return GP_UNSUPPORTED_LATTICE;  // caller falls back to the prefix path
+    Cols cols;
+    Slots slots;
+    int mon[MAX_FB];
+    for (int l = 0; l < k; l++) { mon[l] = l; mon[k + l] = N - k + l; }
+    const int nc = make_columns(mon, fb, N, cols, slots);
+    if (nc > ROWB) return GP_UNSUPPORTED_LATTICE;
+    const int k_steps = (nc + 31) / 32;
+    const uint32_t n_tiles = (s->D_sym + TN - 1) / TN;
+    const size_t img_bytes = (size_t)n_tiles * TILE_BYTES;
+    const size_t rec_bytes = sizeof(int4) << fb;
+
+    // images of the map: m and rev(m) adjacent, each unordered pair once
+    const uint32_t n_mid = 1u << mid;
+    std::vector<uint32_t> tiles, partner, cuts;
+    tiles.reserve(n_mid); partner.reserve(n_mid);
+    size_t group = (192ULL << 20) / (img_bytes + rec_bytes);
+    if (group < 2) group = 2;
+    if (group > 64) group = 64;
+    cuts.push_back(0);
+    for (uint32_t m = 0; m < n_mid; m++) {
+        uint32_t r = 0;
+        for (int b = 0; b < mid; b++) r |= ((m >> b) & 1u) << (mid - 1 - b);
+        if (r < m) continue;
+        if (tiles.size() - cuts.back() + 2 > group) cuts.push_back((uint32_t)tiles.size());
+        const uint32_t at = (uint32_t)tiles.size();
+        if (r == m) { tiles.push_back(m); partner.push_back(at); }
+        else { tiles.push_back(m); tiles.push_back(r); partner.push_back(at + 1); partner.push_back(at); }
+    }
+    cuts.push_back((uint32_t)tiles.size());
+
+    int dev = 0, sms = 0;
+    GP_CUDA(cudaGetDevice(&dev));
+    GP_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    const size_t smem = (size_t)(MT + NSTAGE) * TILE_BYTES + sizeof(Barriers) + sizeof(Cols) + 1024 + 64;
+    const scoring_fn kernel = g_pack ? scoring_for<1, true>(k_steps) : scoring_for<1, false>(k_steps);
+    GP_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const size_t need = (img_bytes + rec_bytes) * group;
+    if (s->scratch_bytes < need) {
+        if (s->d_scratch) GP_CUDA(cudaFree(s->d_scratch));
+        s->d_scratch = nullptr; s->scratch_bytes = 0;
+        GP_CUDA(cudaMalloc(&s->d_scratch, need));
+        s->scratch_bytes = need;
+    }
+    int8_t* d_img = (int8_t*)s->d_scratch;
+    int4* d_rec = (int4*)((char*)s->d_scratch + img_bytes * group);
+    uint32_t* d_lists = nullptr;  // tiles | partner
+    GP_CUDA(cudaMallocAsync(&d_lists, tiles.size() * 2 * sizeof(uint32_t), st));
+    GP_CUDA(cudaMemcpyAsync(d_lists, tiles.data(), tiles.size() * sizeof(uint32_t), cudaMemcpyHostToDevice, st));
+    GP_CUDA(cudaMemcpyAsync(d_lists + tiles.size(), partner.data(), tiles.size() * sizeof(uint32_t), cudaMemcpyHostToDevice, st));
+    GP_CUDA(cudaStreamSynchronize(st));  // the host vectors go out of scope; pageable copies are staged, this is belt and braces
+
+    for (size_t c = 0; c + 1 < cuts.size(); c++) {
+        const uint32_t first = cuts[c], n_img = cuts[c + 1] - cuts[c];
+        if (!n_img) continue;
+        ImgArgs ia;
+        ia.contacts = s->d_contacts_sym; ia.class_of = s->d_class_sym; ia.img = d_img; ia.tile_list = d_lists;
+        ia.gfix_first = 0; ia.list_first = first; ia.gfix_shift = k; ia.D = s->D_sym; ia.n_tiles = n_tiles;
+        ia.NBP = s->NBP; ia.lin = hp.lin; ia.quad = hp.quad;
+        gp_time_begin(GP_KERNEL_IMAGE, st);
+        build_image_kernel<<<dim3(n_tiles, n_img), TN, 0, st>>>(ia, slots);
+        gp_time_end(GP_KERNEL_IMAGE, st);
+        GP_CUDA(cudaGetLastError());
+        Args a;
+        a.img = d_img; a.class_of = s->d_class_sym; a.pheno = nullptr; a.gap = nullptr;
+        a.g_first = 0; a.g_end = (uint64_t)n_img << fb; a.out_base = 0;
+        a.n_items = (uint32_t)((a.g_end + SUPER - 1) / SUPER);
+        a.n_tiles = n_tiles; a.D = s->D_sym; a.fb = fb; a.k_steps = k_steps; a.threshold = hp.threshold; a.dbg = g_debug;
+        a.hrec = d_rec; a.n_snap = s->n_snap;
+        const unsigned grid = a.n_items < (uint32_t)sms ? a.n_items : (uint32_t)sms;
+        gp_time_begin(GP_KERNEL_SCORING, st);
+        kernel<<<grid, THREADS, smem, st>>>(a, cols);
+        gp_time_end(GP_KERNEL_SCORING, st);
+        GP_CUDA(cudaGetLastError());
+        CombArgs ca;
+        ca.hrec = d_rec; ca.tile_list = d_lists; ca.partner = d_lists + tiles.size(); ca.class_sym = s->d_class_sym;
+        ca.pheno = d_pheno; ca.gap = d_gap; ca.list_first = first; ca.n_images = n_img;
+        ca.fb = fb; ca.k = k; ca.N = N; ca.threshold = hp.threshold;
+        const uint64_t work = ((uint64_t)n_img << fb) / 256;
+        combine_kernel<<<(unsigned)(work < (uint64_t)sms * 8 ? (work ? work : 1) : (uint64_t)sms * 8), 256, 0, st>>>(ca);
+        GP_CUDA(cudaGetLastError());
+        gp_count_launches(3);
+    }
+    GP_CUDA(cudaFreeAsync(d_lists, st));
+    return GP_OK;
+}
+
+extern "C" gp_status gp_enumerate_map(const gp_structures_t* s_, const gp_energies* en, uint16_t* d_pheno, int16_t* d_gap,
+                                      void* stream) {
+    gp_structures_s* s = const_cast<gp_structures_s*>(s_);
+    gp_hp_params hp;
+    gp_status stt = gp_check_hp(s, en, &hp);
+    if (stt != GP_OK) return stt;
+    if (!d_pheno) return GP_INVALID_ARG;
+    if (s->device < 0) { gp_set_cuda_error(cudaErrorNoDevice, "handle has no device tables"); return GP_CUDA_ERROR; }
+    if (s->N >= 64) return GP_UNSUPPORTED_LATTICE;
+    stt = gp_launch_map_tc(s, hp, d_pheno, d_gap, (cudaStream_t)stream);
+    if (stt == GP_UNSUPPORTED_LATTICE)  // chains shorter than 10 monomers: the prefix path covers the map in one image
+        return gp_launch_scoring_tc(s, hp, 0, 1ULL << s->N, d_pheno, d_gap, (cudaStream_t)stream);
+    return stt;
 }
 
 extern "C" uint64_t gp_tile(void) { return tc::SUPER; }

@@ -36,6 +36,7 @@ SIGNATURES = {
     "gp_structures_get": (ctypes.c_int, [_vp, ctypes.c_uint32, _u8p, _u8p, _u16p]),
     "gp_tile": (ctypes.c_uint64, []),
     "gp_enumerate": (ctypes.c_int, [_vp, ctypes.POINTER(_Energies), ctypes.c_uint64, ctypes.c_uint64, _vp, _vp, _vp]),
+    "gp_enumerate_map": (ctypes.c_int, [_vp, ctypes.POINTER(_Energies), _vp, _vp, _vp]),
     "gp_enumerate_simple": (ctypes.c_int, [_vp, ctypes.POINTER(_Energies), ctypes.c_uint64, ctypes.c_uint64, _vp, _vp, _vp]),
     "gp_enumerate_seqs": (ctypes.c_int, [_vp, ctypes.POINTER(_Energies), _vp, ctypes.c_uint64, _vp, _vp, _vp]),
     "gp_enumerate_seeded": (ctypes.c_int, [_vp, ctypes.POINTER(_Energies), ctypes.c_uint64, ctypes.c_uint64,
@@ -69,7 +70,7 @@ def lib():
             f.argtypes = args
         L.gp_set_fold_bits.restype = ctypes.c_int
         L.gp_set_fold_bits.argtypes = [ctypes.c_int]
-        for hook in ("gp_set_rob_tile_bits", "gp_set_pack", "gp_set_halves", "gp_set_debug"):  # test / tuning hooks
+        for hook in ("gp_set_sym_bits", "gp_set_rob_tile_bits", "gp_set_pack", "gp_set_halves", "gp_set_debug"):  # test / tuning hooks
             getattr(L, hook).restype = ctypes.c_int
             getattr(L, hook).argtypes = [ctypes.c_int]
         _lib = L
@@ -198,6 +199,15 @@ class Structures:
             raise ValueError("output tensor too small")
         _check(f(self._h, ctypes.byref(en), g_begin, g_count, _dptr(pheno, torch.uint16), _dptr(gap, torch.int16),
                  _stream(stream)), "gp_enumerate")
+
+    def enumerate_map(self, pheno, gap=None, e=HP_ENERGIES, threshold=1, stream=None):
+        """gp_enumerate_map: the whole map (2^N entries) through the reversal identity, half the evaluations."""
+        import torch
+        en = _energies(e, 2, threshold)
+        if pheno.numel() != 1 << self.N or (gap is not None and gap.numel() != 1 << self.N):
+            raise ValueError("gp_enumerate_map needs 2^N entries")
+        _check(lib().gp_enumerate_map(self._h, ctypes.byref(en), _dptr(pheno, torch.uint16), _dptr(gap, torch.int16),
+                                      _stream(stream)), "gp_enumerate_map")
 
     def enumerate_seqs(self, seqs, pheno, gap=None, e=None, alphabet=20, threshold=1, stream=None):
         import torch

@@ -262,3 +262,36 @@ def test_robustness_tile_sizes_agree_with_oracle(tile_bits):
             assert int(pc) == pco, (tile_bits, n_bits)
     finally:
         L.gp_set_rob_tile_bits(15)
+
+
+@pytest.mark.parametrize("dims,k", [((2, 2, 1), 9), ((3, 3, 1), 9), ((4, 4, 1), 5), ((4, 4, 1), 6), ((4, 4, 1), 8),
+                                    ((4, 3, 1), 5), ((2, 2, 2), 9)])
+def test_enumerate_map_whole_small_maps(oracle_structures, dims, k):
+    """gp_enumerate_map (reversal identity, one representative per class) equals the oracle on whole maps, for image
+    sizes that give many image pairs, palindromic images and a single image; chains under 10 monomers fall back."""
+    S, O = lib_structures(dims), oracle_structures(*dims)
+    n = 1 << S.N
+    assert gpmap.lib().gp_set_sym_bits(k) == 0
+    try:
+        ph = torch.full((n,), 0x7777, dtype=torch.int32, device="cuda").to(torch.uint16)
+        gap = torch.zeros(n, dtype=torch.int16, device="cuda")
+        S.enumerate_map(ph, gap)
+        torch.cuda.synchronize()
+    finally:
+        gpmap.lib().gp_set_sym_bits(9)
+    ph_o, gap_o = O.enumerate(0, n)
+    assert np.array_equal(ph.cpu().numpy(), ph_o), dims
+    assert np.array_equal(gap.cpu().numpy().astype(np.int32), np.maximum(gap_o, -32768)), dims
+
+
+def test_enumerate_map_other_energies_and_threshold(oracle_structures):
+    S, O = lib_structures((4, 4, 1)), oracle_structures(4, 4)
+    n = 1 << 16
+    assert gpmap.lib().gp_set_sym_bits(6) == 0
+    try:
+        for e, thr in [((0, -10, -10, -23), 4), ((-3, 2, 2, -17), 1), ((5, -1, -1, 0), 2)]:
+            ph = torch.empty(n, dtype=torch.uint16, device="cuda")
+            S.enumerate_map(ph, None, e=e, threshold=thr)
+            assert np.array_equal(ph.cpu().numpy(), O.enumerate(0, n, e=e, threshold=thr, want_gap=False)), (e, thr)
+    finally:
+        gpmap.lib().gp_set_sym_bits(9)
