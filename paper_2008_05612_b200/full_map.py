@@ -23,7 +23,7 @@ def bit_reverse(g, n):
     return r
 
 
-def run(lattice, out, chunk_bits=30, sample=1 << 20, seed=200805612, keep_store=False):
+def run(lattice, out, chunk_bits=30, sample=1 << 20, seed=200805612, keep_store=False, prefix_path=False):
     import torch
     from . import gpmap
 
@@ -43,11 +43,14 @@ def run(lattice, out, chunk_bits=30, sample=1 << 20, seed=200805612, keep_store=
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
     torch.cuda.synchronize()
     ev[0].record()
-    for b in range(0, total, chunk):
-        S.enumerate(b, chunk, pheno[b:b + chunk])
-        if (b // chunk) % 8 == 7:
-            torch.cuda.synchronize()
-            say("scored %d / %d chunks" % (b // chunk + 1, total // chunk))
+    if prefix_path:   # gp_enumerate on consecutive ranges: every genotype on all D directed structures
+        for b in range(0, total, chunk):
+            S.enumerate(b, chunk, pheno[b:b + chunk])
+            if (b // chunk) % 8 == 7:
+                torch.cuda.synchronize()
+                say("scored %d / %d chunks" % (b // chunk + 1, total // chunk))
+    else:             # gp_enumerate_map: reversal identity, one representative per class (C columns)
+        S.enumerate_map(pheno)
     ev[1].record()
     hist = gpmap.designability(pheno, C)
     ev[2].record()
@@ -76,6 +79,8 @@ def run(lattice, out, chunk_bits=30, sample=1 << 20, seed=200805612, keep_store=
     order = np.argsort(hist[:C])[::-1]
     summary = {
         "lattice": lattice, "N": N, "D": D, "C": C, "genotypes": total, "evaluations": float(total) * D,
+        "path": "gp_enumerate (prefix tiles, D columns)" if prefix_path else "gp_enumerate_map (reversal identity, C columns)",
+        "evaluations_executed": float(total) * (D if prefix_path else C),
         "seconds": {"scoring": t_score, "designability": t_hist, "neighbour_pass": t_rob,
                     "total": t_score + t_hist + t_rob},
         "evals_per_s_scoring": float(total) * D / t_score,
@@ -98,8 +103,9 @@ def main():
     ap.add_argument("--lattice", default="6x6", choices=sorted(LATTICES))
     ap.add_argument("--out", default="gpurun_out/map")
     ap.add_argument("--chunk-bits", type=int, default=30)
+    ap.add_argument("--prefix-path", action="store_true", help="score with gp_enumerate instead of gp_enumerate_map")
     a = ap.parse_args()
-    print(json.dumps(run(a.lattice, a.out, a.chunk_bits)))
+    print(json.dumps(run(a.lattice, a.out, a.chunk_bits, prefix_path=a.prefix_path)))
 
 
 if __name__ == "__main__":

@@ -25,8 +25,9 @@ def main():
     ap.add_argument("--out", default="gpurun_out/map")
     ap.add_argument("--ranges", type=int, default=8)
     ap.add_argument("--length", type=int, default=2048)
+    ap.add_argument("--prefix-path", action="store_true")
     a = ap.parse_args()
-    summary, pheno, S = full_map.run(a.lattice, a.out, keep_store=True)
+    summary, pheno, S = full_map.run(a.lattice, a.out, keep_store=True, prefix_path=a.prefix_path)
     O = orc.Structures(*full_map.LATTICES[a.lattice])
     bad = 0
     for b, c in workloads.sample_ranges(S.N, a.ranges, a.length, 512):
