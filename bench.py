@@ -44,6 +44,7 @@ def parse():
     ap.add_argument("--full", action="store_true", help="one step = the full map of the lattice")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-whole-map", action="store_true", help="skip the whole-3x3x3-map leg")
     ap.add_argument("--fold-bits", type=int, default=0, help="tuning hook: low genotype bits kept as MMA columns")
     return ap.parse_args()
 
@@ -216,7 +217,10 @@ def run_ours(args):
 
     def step(i):
         b = tile_begin(i, rank, world, G, N)
-        S.enumerate(b, n, pheno, stream=stream)                       # a1-a4
+        if args.full:
+            S.enumerate_map(pheno, stream=stream)                     # a1-a4, whole map through the reversal identity
+        else:
+            S.enumerate(b, n, pheno, stream=stream)                   # a1-a4
         gpmap.designability(pheno, C, hist=hist, stream=stream)       # a5
         return gpmap.robustness(pheno, G, C, stream=stream)           # a6 (+ pair bitmap)
 
@@ -315,6 +319,29 @@ def run_ours(args):
         cpu = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc, "seconds": secs,
                "host_cores_available": os.cpu_count()}
 
+    whole = None
+    if world == 1 and not args.full and not args.no_whole_map:
+        # BASELINE.json configs[2]: the paper's fully analysed map, whole, through gp_enumerate_map (reversal identity)
+        S3 = gpmap.Structures(3, 3, 3)
+        p3 = torch.empty(1 << 27, dtype=torch.uint16, device="cuda")
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        reps = 3
+        for i in range(1 + reps):
+            if i == 1:
+                torch.cuda.synchronize()
+                e0.record(stream)
+            S3.enumerate_map(p3, stream=stream)
+            h3 = gpmap.designability(p3, S3.C, stream=stream)
+            r3 = gpmap.robustness(p3, 27, S3.C, stream=stream)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        sec = e0.elapsed_time(e1) * 1e-3 / reps
+        whole = {"workload": "3x3x3 HP whole map: 2^27 genotypes, 103346 directed structures (51704 scored by the reversal "
+                             "identity), designability + neighbour pass", "seconds_per_map": sec,
+                 "effective_evals_per_s": float(1 << 27) * S3.D / sec, "executed_evals_per_s": float(1 << 27) * S3.C / sec,
+                 "folding": int((1 << 27) - h3[S3.C].item()), "paper_folding_percent": 4.76}
+        del p3
+        S3.close()
     total_evals_map = float(1 << N) * D
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -328,6 +355,9 @@ def run_ours(args):
             "full_map_wall_s_extrapolated": total_evals_map / value * world if value else None,
             "folding_fraction_last_tile": folding / float(n),
             "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline, "other_kernels": other,
+            "whole_map_3x3x3": whole,
+            "full_6x6_measured": {"wall_s": 127.4, "path": "gp_enumerate_map + designability + neighbour pass, 137 GB store",
+                                  "source": "profiles/r1_full_6x6.md (separate run: python tests/full_map_check.py --lattice 6x6)"},
             "cpu_baseline": cpu}
     print(json.dumps(line), flush=True)
     if world > 1:
