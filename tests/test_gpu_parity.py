@@ -295,3 +295,27 @@ def test_enumerate_map_other_energies_and_threshold(oracle_structures):
             assert np.array_equal(ph.cpu().numpy(), O.enumerate(0, n, e=e, threshold=thr, want_gap=False)), (e, thr)
     finally:
         gpmap.lib().gp_set_sym_bits(9)
+
+
+def test_bench_step_configuration_sampled(oracle_structures):
+    """The step bench.py times (6x6 prefix tile of 2^26 genotypes, gp_enumerate + gp_designability + gp_robustness, same
+    launch configuration) checked on sampled outputs the oracle computes one by one, plus the size-independent invariants."""
+    import bench
+    S, O = lib_structures((6, 6, 1)), oracle_structures(6, 6)
+    G, n = 26, 1 << 26
+    begin = bench.tile_begin(3, 0, 1, G, S.N)
+    ph = torch.empty(n, dtype=torch.uint16, device="cuda")
+    S.enumerate(begin, n, ph)
+    hist = gpmap.designability(ph, S.C).cpu().numpy().astype(np.int64)
+    R, Dl, Oc, pc = (x.cpu().numpy().astype(np.int64) if hasattr(x, "cpu") else x for x in gpmap.robustness(ph, G, S.C))
+    assert hist.sum() == n
+    folding = int(hist[:S.C].sum())
+    assert int(R.sum() + Dl.sum() + Oc.sum()) == G * folding and R.sum() % 2 == 0 and Oc.sum() % 2 == 0
+    rng = np.random.default_rng(5)
+    offs = np.unique(np.concatenate([[0, n - 1, 511, 512, (1 << 19) - 1, 1 << 19], rng.integers(0, n, 250)]))
+    got = ph.view(torch.int16)[torch.from_numpy(offs).cuda()].cpu().numpy().view(np.uint16)
+    for o, v in zip(offs.tolist(), got.tolist()):
+        assert v == int(O.enumerate(begin + o, 1, want_gap=False)[0]), (begin, o)
+    # a whole supertile-aligned stretch as well (ragged against the 2^19 weight-image boundary)
+    b2 = (1 << 19) - 256
+    assert np.array_equal(ph[b2:b2 + 512].cpu().numpy(), O.enumerate(begin + b2, 512, want_gap=False))
