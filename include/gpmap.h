@@ -112,6 +112,12 @@ gp_status gp_designability(const uint16_t* d_pheno, uint64_t count, uint32_t n_c
 gp_status gp_robustness(const uint16_t* d_pheno, int n_bits, uint32_t n_classes, uint64_t* d_neutral,
                         uint64_t* d_deleterious, uint64_t* d_other, uint64_t* d_pair_count, void* stream);
 
+/* phi row of target class q (:138-147 Eq. 2 numerators, Figs. 9-12): d_row[p] = number of
+ * (genotype, flip) pairs that lead from a genotype of class p to a genotype of class q, p < n_classes (p = q: the
+ * neutral count of q); d_row[n_classes] = the same from null genotypes.  phi_pq = d_row[p] / (n_bits * hist[p]).  Full
+ * store of 2^n_bits entries. */
+gp_status gp_phi_row(const uint16_t* d_pheno, int n_bits, uint32_t n_classes, uint32_t q, uint64_t* d_row, void* stream);
+
 /* a7. Neutral-network components (:19, R12): d_ncomp[p] = number of connected components of {g : pheno = p} under
  * single-bit flips.  Needs 4 bytes of private scratch per genotype; n_bits <= 30.  Synchronises the stream. */
 gp_status gp_nn_components(const uint16_t* d_pheno, int n_bits, uint32_t n_classes, uint32_t* d_ncomp, void* stream);

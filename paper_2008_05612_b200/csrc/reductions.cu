@@ -201,6 +201,35 @@ __global__ void robustness_tiny_kernel(RobArgs a) {
     if (o) atomicAdd(&a.O[p], o);
 }
 
+// phi row (Figs. 9-12): for a target class q, row[p] = number of (genotype, flip) pairs that lead from
+// class p into q; row[C] = the same from null genotypes.  Adjacency is symmetric, so the kernel walks the genotypes OF
+// class q (one streaming read, 16-byte vectors) and histograms their neighbours' classes.
+__global__ void __launch_bounds__(256) phi_row_kernel(const uint16_t* __restrict__ pheno, int n_bits, uint32_t C, uint32_t q,
+                                                      unsigned long long* __restrict__ row) {
+    const uint64_t n = 1ULL << n_bits;
+    const uint64_t n_vec = n >> 3;
+    const uint32_t qq = q * 0x10001u;
+    for (uint64_t v = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; v < (n_vec ? n_vec : 1);
+         v += (uint64_t)gridDim.x * blockDim.x) {
+        uint32_t mine[8];
+        if (n_vec) {
+            const uint4 x = __ldg(reinterpret_cast<const uint4*>(pheno) + v);
+            if (!__vcmpeq2(x.x, qq) && !__vcmpeq2(x.y, qq) && !__vcmpeq2(x.z, qq) && !__vcmpeq2(x.w, qq)) continue;
+            unpack8(x, mine);
+        } else {
+            for (int j = 0; j < 8; j++) mine[j] = (uint64_t)j < n ? pheno[j] : NULLP;
+        }
+        for (int j = 0; j < 8; j++) {
+            if (mine[j] != q) continue;
+            const uint64_t g = v * 8 + j;
+            for (int k = 0; k < n_bits; k++) {
+                const uint32_t p = pheno[g ^ (1ULL << k)];
+                atomicAdd(&row[p == NULLP ? C : p], 1ULL);
+            }
+        }
+    }
+}
+
 __global__ void popcount_kernel(const uint32_t* __restrict__ words, uint64_t n_words, unsigned long long* out) {
     unsigned long long c = 0;
     for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_words; i += (uint64_t)gridDim.x * blockDim.x)
@@ -355,6 +384,21 @@ extern "C" gp_status gp_robustness(const uint16_t* d_pheno, int n_bits, uint32_t
         gp_count_launches(1);
         GP_CUDA(cudaFreeAsync(a.bitmap, st));
     }
+    return GP_OK;
+}
+
+extern "C" gp_status gp_phi_row(const uint16_t* d_pheno, int n_bits, uint32_t n_classes, uint32_t q, uint64_t* d_row,
+                                void* stream) {
+    if (!d_pheno || !d_row || n_classes == 0 || n_classes >= NULLP || q >= n_classes) return GP_INVALID_ARG;
+    if (n_bits < 1 || n_bits > 40 || ((uintptr_t)d_pheno & 15) != 0) return GP_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    GP_CUDA(cudaMemsetAsync(d_row, 0, ((size_t)n_classes + 1) * sizeof(uint64_t), st));
+    const uint64_t n_vec = (1ULL << n_bits) >> 3;
+    const uint64_t want = (n_vec + 255) / 256, cap = (uint64_t)sm_count() * 8;
+    phi_row_kernel<<<(unsigned)(want < cap ? (want ? want : 1) : cap), 256, 0, st>>>(
+        d_pheno, n_bits, n_classes, q, reinterpret_cast<unsigned long long*>(d_row));
+    GP_CUDA(cudaGetLastError());
+    gp_count_launches(1);
     return GP_OK;
 }
 

@@ -45,6 +45,7 @@ SIGNATURES = {
     "gp_seeded_sequences": (ctypes.c_int, [ctypes.c_uint64, ctypes.c_uint64, ctypes.c_uint64, ctypes.c_int, _u8p]),
     "gp_designability": (ctypes.c_int, [_vp, ctypes.c_uint64, ctypes.c_uint32, _vp, _vp]),
     "gp_robustness": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_uint32, _vp, _vp, _vp, _vp, _vp]),
+    "gp_phi_row": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_uint32, ctypes.c_uint32, _vp, _vp]),
     "gp_nn_components": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_uint32, _vp, _vp]),
     "gp_enumerate_host": (ctypes.c_int, [_vp, ctypes.POINTER(_Energies), ctypes.c_uint64, ctypes.c_uint64, _vp, _u64p,
                                          _u64p, _u64p]),
@@ -276,6 +277,17 @@ def robustness(pheno, n_bits, n_classes, want_pairs=True, stream=None):
     _check(lib().gp_robustness(_dptr(pheno, torch.uint16), n_bits, n_classes, _dptr(out[0]), _dptr(out[1]), _dptr(out[2]),
                                _dptr(pc), _stream(stream)), "gp_robustness")
     return out[0], out[1], out[2], pc
+
+
+def phi_row(pheno, n_bits, n_classes, q, stream=None):
+    """gp_phi_row: int64[n_classes+1] counts of single mutations leading from each class (last: from null) into q."""
+    import torch
+    if pheno.numel() != 1 << n_bits:
+        raise ValueError("gp_phi_row needs the full store of 2^n_bits entries")
+    row = torch.empty(n_classes + 1, dtype=torch.int64, device=pheno.device)
+    _check(lib().gp_phi_row(_dptr(pheno, torch.uint16), n_bits, n_classes, q, _dptr(row, torch.int64), _stream(stream)),
+           "gp_phi_row")
+    return row
 
 
 def nn_components(pheno, n_bits, n_classes, stream=None):

@@ -64,3 +64,16 @@ def test_map_path_equals_prefix_path_and_oracle_on_ranges(map_3x3x3, oracle_stru
         assert torch.equal(buf.view(torch.int16), ph[begin:begin + (1 << 16)].view(torch.int16)), begin
         want = O.enumerate(begin + 1024, 512, want_gap=False)
         assert np.array_equal(ph[begin + 1024:begin + 1536].cpu().numpy(), want), begin
+
+
+def test_classes_connected_to_the_top_fold(map_3x3x3):
+    """'0.86 % of phenotypes are connected to the most designable fold': 406 of 47 449."""
+    S, ph, hist, R, Dl, Oc, pairs = map_3x3x3
+    pins = read_pins()
+    des = hist[:S.C]
+    top = int(np.argmax(des))
+    row = gpmap.phi_row(ph, S.N, S.C, top).cpu().numpy()
+    assert int(row[top]) == int(R[top])                       # the diagonal entry is the neutral count
+    connected = int(((row[:S.C] > 0) & (np.arange(S.C) != top)).sum())
+    assert connected == 406
+    assert round(100.0 * connected / int((des > 0).sum()), 2) == pins["connected_to_top_percent"]

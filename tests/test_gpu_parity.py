@@ -319,3 +319,26 @@ def test_bench_step_configuration_sampled(oracle_structures):
     # a whole supertile-aligned stretch as well (ragged against the 2^19 weight-image boundary)
     b2 = (1 << 19) - 256
     assert np.array_equal(ph[b2:b2 + 512].cpu().numpy(), O.enumerate(begin + b2, 512, want_gap=False))
+
+
+def test_phi_row_against_oracle_transitions(oracle_structures):
+    """gp_phi_row(q) equals column q of the oracle's ordered transition matrix (and its null-source entry), on the
+    4x4 map, on synthetic stores and on tiny stores."""
+    S, O = lib_structures((4, 4, 1)), oracle_structures(4, 4)
+    store = O.enumerate(0, 1 << 16, want_gap=False)
+    cases = [(store, 16, S.C)]
+    rng = np.random.default_rng(3)
+    for n_bits, C, p_null in [(1, 2, 0.0), (2, 2, 0.3), (5, 3, 0.4), (13, 40, 0.6)]:
+        st = rng.integers(0, C, size=1 << n_bits).astype(np.uint16)
+        st[rng.random(1 << n_bits) < p_null] = 0xFFFF
+        cases.append((st, n_bits, C))
+    for st, n_bits, C in cases:
+        T = orc.transitions(st, n_bits, C)
+        ph = torch.from_numpy(st.view(np.int16)).cuda().view(torch.uint16)
+        n = 1 << n_bits
+        idx = np.arange(n, dtype=np.uint64)
+        for q in sorted(set([0, C - 1, int(np.argmax(np.bincount(st[st != 0xFFFF], minlength=C)))])):
+            row = gpmap.phi_row(ph, n_bits, C, q).cpu().numpy().astype(np.uint64)
+            assert np.array_equal(row[:C], T[:, q]), (n_bits, q)
+            from_null = sum(int(((st == 0xFFFF) & (st[idx ^ np.uint64(1 << k)] == q)).sum()) for k in range(n_bits))
+            assert int(row[C]) == from_null, (n_bits, q)
