@@ -74,12 +74,25 @@ struct RobArgs {
     int tb, c, h, hi_pos, f0;  // tile bits, contiguous low bits, spread bits, their position, first local bit to flip
 };
 
-__device__ __forceinline__ void note_pair(const RobArgs& a, uint32_t p, uint32_t q) {
-    if (q < p) return;  // every unordered pair is met from both ends: record it from the smaller class only
+constexpr uint32_t ROB_PF_SLOTS = 1024;  // per-block filter of recently recorded class pairs (shared memory)
+
+__device__ __forceinline__ void note_pair(const RobArgs& a, uint32_t* pf, uint32_t p, uint32_t q) {
+    if (q < p) { const uint32_t t = p; p = q; q = t; }
+    if (pf) {
+        const uint32_t key = (p << 16) | q;
+        uint32_t* slot = pf + ((key * 2654435761u) >> 22);
+        if (*(volatile uint32_t*)slot == key) return;  // seen by this block already (racy update is harmless: the bitmap is the truth)
+        *(volatile uint32_t*)slot = key;
+    }
     uint64_t bit = (uint64_t)p * a.C + q;
     uint32_t* w = a.bitmap + (bit >> 5);
     uint32_t m = 1u << (bit & 31);
     if (!(*(volatile uint32_t*)w & m)) atomicOr(w, m);
+}
+
+// bit 15 / bit 31 of the result are set iff the low / high 16-bit half of x is zero (exact: no carry crosses the halves)
+__device__ __forceinline__ uint32_t zero_halves(uint32_t x) {
+    return ~(((x & 0x7FFF7FFFu) + 0x7FFF7FFFu) | x) & 0x80008000u;
 }
 
 __device__ __forceinline__ void unpack8(const uint4& x, uint32_t (&q)[8]) {
@@ -126,7 +139,9 @@ __device__ __forceinline__ void rob_flush(const RobArgs& a, RobSlot* cache) {
 __global__ void __launch_bounds__(RTHREADS, 2) robustness_kernel(RobArgs a) {
     extern __shared__ __align__(16) uint16_t seg[];
     RobSlot* cache = reinterpret_cast<RobSlot*>(seg + ((size_t)1 << a.tb));
+    uint32_t* pf = reinterpret_cast<uint32_t*>(cache + ROB_SLOTS);
     for (uint32_t i = threadIdx.x; i < ROB_SLOTS; i += blockDim.x) cache[i] = RobSlot{NULLP, 0, 0, 0};
+    for (uint32_t i = threadIdx.x; i < ROB_PF_SLOTS; i += blockDim.x) pf[i] = 0xFFFFFFFFu;
     uint32_t tiles_done = 0;
     const uint32_t n_vec = 1u << (a.tb - 3);                       // 16-byte vectors per tile
     const uint64_t n_tiles = 1ULL << (a.n_bits - a.tb);
@@ -144,38 +159,65 @@ __global__ void __launch_bounds__(RTHREADS, 2) robustness_kernel(RobArgs a) {
         }
         __syncthreads();
         for (uint32_t v = threadIdx.x; v < n_vec; v += RTHREADS) {
-            uint32_t mine[8], r[8], dl[8];
-            unpack8(sv[v], mine);
-            bool any = false;
+            // 8 genotypes as 4 words of two 16-bit class ids; counters packed the same way (a count is at most 36)
+            const uint4 mv = sv[v];
+            const uint32_t m[4] = {mv.x, mv.y, mv.z, mv.w};
+            uint32_t mnz[4], rc[4] = {0, 0, 0, 0}, dc[4] = {0, 0, 0, 0};
 #pragma unroll
-            for (int j = 0; j < 8; j++) { r[j] = dl[j] = 0; any |= (mine[j] != NULLP); }
-            if (!any) continue;
+            for (int w = 0; w < 4; w++) mnz[w] = zero_halves(~m[w]);          // which of mine are null
+            if ((mnz[0] & mnz[1] & mnz[2] & mnz[3]) == 0x80008000u) continue;  // all 8 null
             for (int k = a.f0; k < a.tb; k++) {
-                uint32_t q[8];
-                if (k < 3) {
+                uint32_t q[4];
+                if (k == 0) {
 #pragma unroll
-                    for (int j = 0; j < 8; j++) q[j] = mine[j ^ (1 << k)];
+                    for (int w = 0; w < 4; w++) q[w] = __funnelshift_l(m[w], m[w], 16);
+                } else if (k == 1) {
+                    q[0] = m[1]; q[1] = m[0]; q[2] = m[3]; q[3] = m[2];
+                } else if (k == 2) {
+                    q[0] = m[2]; q[1] = m[3]; q[2] = m[0]; q[3] = m[1];
                 } else {
-                    unpack8(sv[v ^ (1u << (k - 3))], q);
+                    const uint4 x = sv[v ^ (1u << (k - 3))];
+                    q[0] = x.x; q[1] = x.y; q[2] = x.z; q[3] = x.w;
                 }
+                uint32_t other = 0, ez[4], nz[4];
 #pragma unroll
-                for (int j = 0; j < 8; j++) {
-                    const uint32_t p = mine[j];
-                    r[j] += (q[j] == p);
-                    dl[j] += (q[j] == NULLP);
-                    if (a.bitmap && p != NULLP && q[j] != p && q[j] != NULLP) note_pair(a, p, q[j]);
+                for (int w = 0; w < 4; w++) {
+                    ez[w] = zero_halves(q[w] ^ m[w]);     // neighbour in the same class
+                    nz[w] = zero_halves(~q[w]);           // neighbour null
+                    rc[w] += ez[w] >> 15;
+                    dc[w] += nz[w] >> 15;
+                    other |= ~(ez[w] | nz[w] | mnz[w]) & 0x80008000u;
+                }
+                if (a.bitmap && other) {
+                    // every edge between two different non-null classes is met from both ends: keep the end whose
+                    // flipped bit is 0, gather the flagged genotypes into one 8-bit mask and walk it
+                    uint32_t ob = 0;
+#pragma unroll
+                    for (int w = 0; w < 4; w++) {
+                        const uint32_t o = ~(ez[w] | nz[w] | mnz[w]);
+                        ob |= (((o >> 15) & 1u) | ((o >> 30) & 2u)) << (2 * w);
+                    }
+                    ob &= k == 0 ? 0x55u : k == 1 ? 0x33u : k == 2 ? 0x0Fu : (((v >> (k - 3)) & 1u) ? 0u : 0xFFu);
+                    while (ob) {
+                        const uint32_t l = (v << 3) + (__ffs(ob) - 1);
+                        ob &= ob - 1;
+                        note_pair(a, pf, seg[l], seg[l ^ (1u << k)]);
+                    }
                 }
             }
             // flush, merging runs of equal class among the 8 genotypes; other = flips - neutral - deleterious
-            uint32_t run = 0;
+            uint32_t run = 0, r_acc = 0, d_acc = 0;
 #pragma unroll
             for (int j = 0; j < 8; j++) {
-                if (mine[j] == NULLP) continue;
+                const uint32_t p = (m[j >> 1] >> (16 * (j & 1))) & 0xFFFFu;
+                if (p == NULLP) continue;
                 run++;
-                if (j < 7 && mine[j + 1] == mine[j]) { r[j + 1] += r[j]; dl[j + 1] += dl[j]; continue; }
-                const uint32_t o = run * (uint32_t)n_flip - r[j] - dl[j];
-                rob_add(a, cache, mine[j], r[j], dl[j], o);
-                run = 0;
+                r_acc += (rc[j >> 1] >> (16 * (j & 1))) & 0xFFFFu;
+                d_acc += (dc[j >> 1] >> (16 * (j & 1))) & 0xFFFFu;
+                const uint32_t nxt = j < 7 ? (m[(j + 1) >> 1] >> (16 * ((j + 1) & 1))) & 0xFFFFu : NULLP;
+                if (nxt == p) continue;
+                rob_add(a, cache, p, r_acc, d_acc, run * (uint32_t)n_flip - r_acc - d_acc);
+                run = 0; r_acc = 0; d_acc = 0;
             }
         }
         if (++tiles_done % ROB_FLUSH_TILES == 0) rob_flush(a, cache);
@@ -194,7 +236,7 @@ __global__ void robustness_tiny_kernel(RobArgs a) {
         const uint32_t q = a.pheno[g ^ (1u << k)];
         if (q == p) r++;
         else if (q == NULLP) d++;
-        else { o++; if (a.bitmap) note_pair(a, p, q); }
+        else { o++; if (a.bitmap) note_pair(a, nullptr, p, q); }
     }
     if (r) atomicAdd(&a.R[p], r);
     if (d) atomicAdd(&a.Dl[p], d);
@@ -354,7 +396,7 @@ extern "C" gp_status gp_robustness(const uint16_t* d_pheno, int n_bits, uint32_t
         gp_count_launches(1);
     } else {
         const int tb = n_bits < g_rob_tile_bits ? n_bits : g_rob_tile_bits;
-        const size_t smem = ((size_t)2 << tb) + ROB_SLOTS * sizeof(RobSlot);
+        const size_t smem = ((size_t)2 << tb) + ROB_SLOTS * sizeof(RobSlot) + ROB_PF_SLOTS * sizeof(uint32_t);
         GP_CUDA(cudaFuncSetAttribute(robustness_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         const uint64_t n_tiles = 1ULL << (n_bits - tb);
         const uint64_t cap = (uint64_t)sm_count() * 2;
