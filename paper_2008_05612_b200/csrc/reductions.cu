@@ -19,18 +19,25 @@ __global__ void __launch_bounds__(1024) hist_kernel(const uint16_t* __restrict__
     unsigned long long nulls = 0;
     const uint64_t nvec = count / 8;
     const uint4* v = reinterpret_cast<const uint4*>(pheno);
-    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += (uint64_t)gridDim.x * blockDim.x) {
-        uint4 x = __ldg(v + i);
-        uint32_t w[4] = {x.x, x.y, x.z, x.w};
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += 4 * stride) {
+        uint4 xs[4];  // four independent 16-byte loads in flight per thread
 #pragma unroll
-        for (int j = 0; j < 4; j++) {
+        for (int u = 0; u < 4; u++) xs[u] = (i + u * stride < nvec) ? __ldg(v + i + u * stride) : make_uint4(~0u, ~0u, ~0u, ~0u);
 #pragma unroll
-            for (int h = 0; h < 2; h++) {
-                uint32_t p = h ? (w[j] >> 16) : (w[j] & 0xFFFFu);
-                if (p == NULLP) nulls++;
-                else if (p < C) {
-                    if (use_smem) atomicAdd(&sh[p], 1u);
-                    else atomicAdd(&hist[p], 1ULL);
+        for (int u = 0; u < 4; u++) {
+            if (i + u * stride >= nvec) break;
+            const uint32_t w[4] = {xs[u].x, xs[u].y, xs[u].z, xs[u].w};
+#pragma unroll
+            for (int j = 0; j < 4; j++) {
+#pragma unroll
+                for (int h = 0; h < 2; h++) {
+                    const uint32_t p = h ? (w[j] >> 16) : (w[j] & 0xFFFFu);
+                    if (p == NULLP) nulls++;
+                    else if (p < C) {
+                        if (use_smem) atomicAdd(&sh[p], 1u);
+                        else atomicAdd(&hist[p], 1ULL);
+                    }
                 }
             }
         }
