@@ -45,3 +45,5 @@ __host__ __device__ inline uint32_t gp_letter20(uint64_t seed, uint64_t seq, int
 // scoring_tc.cu
 gp_status gp_launch_scoring_tc(gp_structures_s* s, const gp_hp_params& hp, uint64_t g_begin, uint64_t g_count,
                                uint16_t* d_pheno, int16_t* d_gap, cudaStream_t st);
+gp_status gp_launch_sequences_tc(gp_structures_s* s, const gp_hp_params& hp, const uint8_t* d_seqs, uint64_t count,
+                                 uint16_t* d_pheno, int16_t* d_gap, cudaStream_t st);

@@ -561,6 +561,226 @@ int g_halves = 1;      // NH of scoring_kernel
 int g_debug = 0;
 int g_pack = 1;        // PACK of scoring_kernel
 
+// =====================================================================================================================
+// Explicit sequences on the tensor cores (the paper's sampling runs, Table 3).
+// Random sequences share no prefix, so the contraction keeps all K = 2 + N + P columns (two constant columns that give
+// pad structures the energy E_PAD, N monomer columns with weight lin*c_i(S), P pair columns with weight quad):
+// 327 columns for 6x6 = three 128-byte column blocks, eleven K steps per chain.  The weight image is built once per
+// (lattice, energies) and cached in the handle.  Chains are long (11 x 64 clk), so two genotype tiles with
+// double-buffered accumulators (2 x 2 x 128 TMEM columns) keep the tensor pipe busy.
+constexpr int SQ_KB = 3;                       // 128-byte column blocks per operand row
+constexpr int SQ_MT = 2;                       // sequence tiles per CTA
+constexpr int SQ_ROWS = SQ_MT * TM;            // 256 sequences per item
+constexpr int SQ_STAGES = 2;
+constexpr int SQ_TILE = SQ_KB * TILE_BYTES;    // 48 KB: one operand tile, all column blocks
+constexpr int SQ_EPI_WARPS = 4 * SQ_MT;
+constexpr int SQ_THREADS = 32 * (2 + SQ_EPI_WARPS);
+constexpr int SQ_MAXCOL = SQ_KB * ROWB;        // 384
+
+struct SqCols {  // column c of the full contraction: feature = val * h_i * h_j; i = j for monomers; bit 63 is always 1
+    uint8_t i[SQ_MAXCOL], j[SQ_MAXCOL];
+};
+
+struct SqImgArgs {
+    const uint8_t* contacts;   // D * NBP * 2
+    const uint16_t* pairidx;   // D * NBP: pair-feature index of each contact
+    int8_t* img;               // [n_tiles][SQ_KB][TILE_BYTES]
+    uint32_t D;
+    int N, NBP, lin, quad;
+};
+
+// One block = one 128-structure tile; thread = structure; the three column blocks are built one after the other.
+__global__ void __launch_bounds__(TN) build_full_image_kernel(const SqImgArgs a) {
+    __shared__ __align__(16) int8_t tile[TILE_BYTES];
+    const uint32_t r = threadIdx.x, n = blockIdx.x;
+    const uint32_t d = n * TN + r;
+    for (int kb = 0; kb < SQ_KB; kb++) {
+        __syncthreads();
+        for (uint32_t i = threadIdx.x; i < TILE_BYTES / 16; i += TN) reinterpret_cast<uint4*>(tile)[i] = make_uint4(0, 0, 0, 0);
+        __syncthreads();
+        const int c0 = kb * ROWB;
+        if (d < a.D) {
+            const uint8_t* c = a.contacts + (size_t)d * a.NBP * 2;
+            const uint16_t* px = a.pairidx + (size_t)d * a.NBP;
+            for (int k = 0; k < a.NBP; k++) {
+                const int ci = 2 + c[2 * k] - c0, cj = 2 + c[2 * k + 1] - c0, cp = 2 + a.N + px[k] - c0;
+                if (ci >= 0 && ci < ROWB) tile[swz(r, ci)] += (int8_t)a.lin;
+                if (cj >= 0 && cj < ROWB) tile[swz(r, cj)] += (int8_t)a.lin;
+                if (cp >= 0 && cp < ROWB) tile[swz(r, cp)] = (int8_t)a.quad;
+            }
+        } else if (kb == 0) {  // pad structure: energy E_PAD for every sequence
+            tile[swz(r, 0)] = 127;
+            tile[swz(r, 1)] = 63;
+        }
+        __syncthreads();
+        uint4* dst = reinterpret_cast<uint4*>(a.img + ((uint64_t)n * SQ_KB + kb) * TILE_BYTES);
+        for (uint32_t i = threadIdx.x; i < TILE_BYTES / 16; i += TN) dst[i] = reinterpret_cast<const uint4*>(tile)[i];
+    }
+}
+
+struct SqArgs {
+    const int8_t* img;        // [n_tiles][SQ_KB][TILE_BYTES]
+    const uint16_t* class_of;
+    const uint8_t* seqs;      // count x N letters (0 / 1)
+    uint16_t* pheno;
+    int16_t* gap;             // nullable
+    uint64_t count;
+    uint32_t n_items, n_tiles;
+    int N, ksteps, threshold;
+};
+
+struct __align__(8) SqBarriers {
+    uint64_t b_full[SQ_STAGES], b_empty[SQ_STAGES];
+    uint64_t acc_full[SQ_MT][2], acc_empty[SQ_MT][2];
+    uint64_t a_full, a_empty;
+    uint32_t tmem_base;
+};
+
+__global__ void __launch_bounds__(SQ_THREADS, 1) sequence_kernel(const SqArgs a, const SqCols cols_in) {
+    extern __shared__ unsigned char smem_dyn[];
+    unsigned char* smem = reinterpret_cast<unsigned char*>(((uintptr_t)smem_dyn + 1023) & ~(uintptr_t)1023);
+    uint8_t* sA = smem;                                    // SQ_MT tiles x SQ_KB blocks
+    uint8_t* sB = smem + SQ_MT * SQ_TILE;                  // SQ_STAGES tiles x SQ_KB blocks
+    SqBarriers* bar = reinterpret_cast<SqBarriers*>(sB + SQ_STAGES * SQ_TILE);
+    SqCols* cols = reinterpret_cast<SqCols*>(bar + 1);
+    constexpr uint32_t IDESC = idesc_for(TN);
+
+    const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    for (uint32_t i = threadIdx.x; i < sizeof(SqCols); i += SQ_THREADS)
+        reinterpret_cast<uint8_t*>(cols)[i] = reinterpret_cast<const uint8_t*>(&cols_in)[i];
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < SQ_STAGES; s++) { mbar_init(&bar->b_full[s], 1); mbar_init(&bar->b_empty[s], 1); }
+        for (int m = 0; m < SQ_MT; m++)
+            for (int h = 0; h < 2; h++) { mbar_init(&bar->acc_full[m][h], 1); mbar_init(&bar->acc_empty[m][h], 4); }
+        mbar_init(&bar->a_full, 32 * SQ_EPI_WARPS);
+        mbar_init(&bar->a_empty, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 1) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(&bar->tmem_base)) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = bar->tmem_base;
+
+    if (warp == 0) {
+        // ===== producer: whole 48 KB weight tiles =====
+        uint32_t it = 0;
+        for (uint32_t item = blockIdx.x; item < a.n_items; item += gridDim.x) {
+            for (uint32_t n = 0; n < a.n_tiles; n++, it++) {
+                const uint32_t s = it % SQ_STAGES, ph = (it / SQ_STAGES) & 1;
+                mbar_wait(&bar->b_empty[s], ph ^ 1);
+                if (elect_one()) {
+                    mbar_expect_tx(&bar->b_full[s], SQ_TILE);
+                    bulk_g2s(sB + s * SQ_TILE, a.img + (uint64_t)n * SQ_TILE, SQ_TILE, &bar->b_full[s]);
+                }
+                __syncwarp();
+            }
+        }
+    } else if (warp == 1) {
+        // ===== MMA issuer: chains of a.ksteps K steps over the column blocks, accumulators double-buffered =====
+        const uint64_t a_desc0 = smem_desc(smem_u32(sA));
+        const uint64_t b_desc0 = smem_desc(smem_u32(sB));
+        uint32_t it = 0, item_no = 0;
+        for (uint32_t item = blockIdx.x; item < a.n_items; item += gridDim.x, item_no++) {
+            mbar_wait(&bar->a_full, item_no & 1);
+            tc_fence_after();
+            for (uint32_t n = 0; n < a.n_tiles; n++, it++) {
+                const uint32_t s = it % SQ_STAGES, ph = (it / SQ_STAGES) & 1;
+                const uint32_t buf = it & 1;
+                mbar_wait(&bar->b_full[s], ph);
+                tc_fence_after();
+                const uint64_t bd = b_desc0 + (uint64_t)(s * (SQ_TILE >> 4));
+#pragma unroll
+                for (int m = 0; m < SQ_MT; m++) {
+                    mbar_wait(&bar->acc_empty[m][buf], ((it >> 1) & 1) ^ 1);
+                    tc_fence_after();
+                    if (elect_one()) {
+                        const uint32_t d = tmem + (m * 2 + buf) * TN;
+                        const uint64_t ad = a_desc0 + (uint64_t)((m * SQ_TILE) >> 4);
+                        for (int ks = 0; ks < a.ksteps; ks++) {
+                            const uint64_t off = (uint64_t)(((ks >> 2) * TILE_BYTES + (ks & 3) * 32) >> 4);
+                            mma_i8(d, ad + off, bd + off, IDESC, ks > 0);
+                        }
+                        tc_commit(&bar->acc_full[m][buf]);
+                    }
+                    __syncwarp();
+                }
+                if (elect_one()) tc_commit(&bar->b_empty[s]);
+                __syncwarp();
+            }
+            if (elect_one()) tc_commit(&bar->a_empty);
+            __syncwarp();
+        }
+    } else {
+        // ===== feature rows + epilogue: warp group m owns sequence tile m; thread = sequence =====
+        const uint32_t m = (warp - 2) >> 2;
+        const uint32_t quarter = warp & 3;
+        const uint32_t r = quarter * 32 + lane;
+        const uint32_t t_lane = tmem + ((quarter * 32u) << 16) + m * 2 * TN;
+        uint32_t it = 0, item_no = 0;
+        for (uint32_t item = blockIdx.x; item < a.n_items; item += gridDim.x, item_no++) {
+            const uint64_t q = (uint64_t)item * SQ_ROWS + m * TM + r;
+            unsigned long long h = 1ULL << 63;  // bit 63: the constant-1 feature; bit 62 stays 0 for unused columns
+            if (q < a.count)
+                for (int i = 0; i < a.N; i++) h |= (unsigned long long)(a.seqs[q * a.N + i] & 1) << i;
+            mbar_wait(&bar->a_empty, (item_no & 1) ^ 1);
+#pragma unroll 1
+            for (uint32_t c16 = 0; c16 < SQ_MAXCOL / 16; c16++) {
+                uint32_t w4[4];
+#pragma unroll
+                for (int wd = 0; wd < 4; wd++) {
+                    uint32_t x = 0;
+#pragma unroll
+                    for (int b = 0; b < 4; b++) {
+                        const uint32_t c = c16 * 16 + wd * 4 + b;
+                        const uint32_t bit = (uint32_t)((h >> cols->i[c]) & (h >> cols->j[c]) & 1ULL);
+                        x |= (bit * (c == 0 ? 64u : 1u)) << (8 * b);
+                    }
+                    w4[wd] = x;
+                }
+                uint8_t* blk = sA + (m * SQ_KB + (c16 >> 3)) * TILE_BYTES;
+                *reinterpret_cast<uint4*>(blk + r * ROWB + (((c16 & 7) ^ (r & 7u)) << 4)) = make_uint4(w4[0], w4[1], w4[2], w4[3]);
+            }
+            fence_proxy_async();
+            mbar_arrive(&bar->a_full);
+
+            int32_t k1 = INT32_MAX, k2 = INT32_MAX;
+            uint32_t E2 = pack2(E_NONE);
+#pragma unroll 1
+            for (uint32_t n = 0; n < a.n_tiles; n++, it++) {
+                const uint32_t buf = it & 1;
+                mbar_wait(&bar->acc_full[m][buf], (it >> 1) & 1);
+                tc_fence_after();
+                uint32_t w[2 * 32];
+                tmem_ld64_pack16(t_lane + buf * TN, w);
+                tmem_ld_wait();
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&bar->acc_empty[m][buf]);
+                fold_half_packed(&w[0], n * TN, k1, k2, E2);
+                fold_half_packed(&w[32], n * TN + HN, k1, k2, E2);
+            }
+            if (q < a.count) {
+                const int32_t e1 = k1 >> KEY_SHIFT, e2v = k2 >> KEY_SHIFT;
+                const uint32_t col = (uint32_t)k1 & ((1u << KEY_SHIFT) - 1u);
+                const bool single = (e2v >= E_PAD);
+                const bool folds = single || (e2v - e1 >= a.threshold);
+                a.pheno[q] = folds ? a.class_of[col] : (uint16_t)GP_NULL_PHENO;
+                if (a.gap) a.gap[q] = (int16_t)(single ? GP_GAP_NONE : max(e1 - e2v, -32768));
+            }
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 1) {
+        tc_fence_after();
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem) : "memory");
+    }
+}
+
 }  // namespace tc
 
 // test / tuning hook (not part of the public header): number of low genotype bits kept as contraction columns
@@ -762,6 +982,51 @@ extern "C" gp_status gp_enumerate_map(const gp_structures_t* s_, const gp_energi
     if (stt == GP_UNSUPPORTED_LATTICE)  // chains shorter than 10 monomers: the prefix path covers the map in one image
         return gp_launch_scoring_tc(s, hp, 0, 1ULL << s->N, d_pheno, d_gap, (cudaStream_t)stream);
     return stt;
+}
+
+// Explicit HP sequences on the tensor cores (sequence_kernel).  GP_UNSUPPORTED_LATTICE = this lattice needs more than
+// 384 columns or is too small to be worth it: the caller falls back to the CUDA-core kernel.
+gp_status gp_launch_sequences_tc(gp_structures_s* s, const gp_hp_params& hp, const uint8_t* d_seqs, uint64_t count,
+                                 uint16_t* d_pheno, int16_t* d_gap, cudaStream_t st) {
+    using namespace tc;
+    const int ncol = 2 + s->N + s->P;
+    if (ncol > SQ_MAXCOL || s->N > 62 || s->D >= (1u << KEY_SHIFT)) return GP_UNSUPPORTED_LATTICE;
+    const uint32_t n_tiles = (s->D + TN - 1) / TN;
+    if (!s->wimg.valid || s->wimg.lin != hp.lin || s->wimg.quad != hp.quad) {
+        if (!s->wimg.d_img) GP_CUDA(cudaMalloc(&s->wimg.d_img, (size_t)n_tiles * SQ_TILE));
+        SqImgArgs ia;
+        ia.contacts = s->d_contacts; ia.pairidx = s->d_pairidx; ia.img = s->wimg.d_img; ia.D = s->D;
+        ia.N = s->N; ia.NBP = s->NBP; ia.lin = hp.lin; ia.quad = hp.quad;
+        build_full_image_kernel<<<n_tiles, TN, 0, st>>>(ia);
+        GP_CUDA(cudaGetLastError());
+        gp_count_launches(1);
+        s->wimg.lin = hp.lin; s->wimg.quad = hp.quad; s->wimg.valid = true; s->wimg.n_tiles = n_tiles; s->wimg.k_blocks = SQ_KB;
+    }
+    SqCols cols;
+    for (int c = 0; c < SQ_MAXCOL; c++) cols.i[c] = cols.j[c] = 62;  // bit 62 of the letter word is always 0
+    cols.i[0] = cols.j[0] = cols.i[1] = cols.j[1] = 63;             // constant 1 (x64 and x1)
+    for (int i = 0; i < s->N; i++) cols.i[2 + i] = cols.j[2 + i] = (uint8_t)i;
+    for (int i = 0; i < s->N; i++)
+        for (int j = 0; j < s->N; j++) {
+            const int p = s->pair_index[(size_t)i * s->N + j];
+            if (p >= 0 && i < j) { cols.i[2 + s->N + p] = (uint8_t)i; cols.j[2 + s->N + p] = (uint8_t)j; }
+        }
+    int dev = 0, sms = 0;
+    GP_CUDA(cudaGetDevice(&dev));
+    GP_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    const size_t smem = (size_t)(SQ_MT + SQ_STAGES) * SQ_TILE + sizeof(SqBarriers) + sizeof(SqCols) + 1024 + 64;
+    GP_CUDA(cudaFuncSetAttribute(sequence_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    SqArgs a;
+    a.img = s->wimg.d_img; a.class_of = s->d_class_of; a.seqs = d_seqs; a.pheno = d_pheno; a.gap = d_gap; a.count = count;
+    a.n_items = (uint32_t)((count + SQ_ROWS - 1) / SQ_ROWS); a.n_tiles = n_tiles;
+    a.N = s->N; a.ksteps = (ncol + 31) / 32; a.threshold = hp.threshold;
+    const unsigned grid = a.n_items < (uint32_t)sms ? a.n_items : (uint32_t)sms;
+    gp_time_begin(GP_KERNEL_SCORING, st);
+    sequence_kernel<<<grid, SQ_THREADS, smem, st>>>(a, cols);
+    gp_time_end(GP_KERNEL_SCORING, st);
+    GP_CUDA(cudaGetLastError());
+    gp_count_launches(1);
+    return GP_OK;
 }
 
 extern "C" uint64_t gp_tile(void) { return tc::SUPER; }

@@ -342,3 +342,35 @@ def test_phi_row_against_oracle_transitions(oracle_structures):
             assert np.array_equal(row[:C], T[:, q]), (n_bits, q)
             from_null = sum(int(((st == 0xFFFF) & (st[idx ^ np.uint64(1 << k)] == q)).sum()) for k in range(n_bits))
             assert int(row[C]) == from_null, (n_bits, q)
+
+
+@pytest.mark.parametrize("dims,count", [((6, 6, 1), 2049), ((3, 3, 3), 1000), ((5, 5, 1), 4096), ((4, 4, 1), 777)])
+def test_explicit_hp_sequences_on_tensor_cores(oracle_structures, dims, count):
+    """The paper's sampling runs: seeded random H/P sequences, every one against all directed
+    structures, through gp_enumerate_seqs (tensor-core sequence_kernel for alphabet 2), against the oracle's explicit
+    sequence path, element by element with gaps; ragged counts; then the CUDA-core kernel on a larger batch."""
+    import workloads
+    S, O = lib_structures(dims), oracle_structures(*dims)
+    seqs = workloads.random_sequences(count, S.N, 2)
+    seqs[0, :] = 1; seqs[1, :] = 0; seqs[2, :] = np.arange(S.N) % 2          # all-H, all-P, alternating: all null
+    e = np.array(gpmap.HP_ENERGIES, np.int32)
+    d_seqs = torch.from_numpy(seqs).cuda()
+    ph = torch.empty(count, dtype=torch.uint16, device="cuda")
+    gap = torch.empty(count, dtype=torch.int16, device="cuda")
+    S.enumerate_seqs(d_seqs, ph, gap, e=e, alphabet=2)
+    ph_o, gap_o = O.enumerate_seqs(seqs, e, 2)
+    assert np.array_equal(ph.cpu().numpy(), ph_o), dims
+    assert np.array_equal(gap.cpu().numpy().astype(np.int32), gap_o), dims
+    if S.D > 1:
+        assert (ph_o[:3] == 0xFFFF).all()
+    big = workloads.random_sequences(1 << 15, S.N, 2, seed=11)
+    d_big = torch.from_numpy(big).cuda()
+    a = torch.empty(1 << 15, dtype=torch.uint16, device="cuda")
+    b = torch.empty_like(a)
+    S.enumerate_seqs(d_big, a, None, e=e, alphabet=2, threshold=3)
+    gpmap.lib().gp_set_seq_tc(0)
+    try:
+        S.enumerate_seqs(d_big, b, None, e=e, alphabet=2, threshold=3)
+    finally:
+        gpmap.lib().gp_set_seq_tc(1)
+    assert torch.equal(a.view(torch.int16), b.view(torch.int16)), dims
