@@ -58,6 +58,22 @@ def main():
             t, _ = dev_time(lambda: gpmap.nn_components(ph, S.N, S.C), reps=1)
             rows.append(dict(row="a7 gp_nn_components", config=name, seconds=t))
         del ph
+    # the paper's sampling runs (Table 3): random H/P sequences, each against every fold
+    import numpy as np
+    for name, paper_s in (("6x6", 1.35e-4), ("3x3x3", 2.6e-4)):
+        S = structs[name]
+        cnt = 1 << 21
+        seqs = torch.from_numpy(np.random.default_rng(SEED).integers(0, 2, size=(cnt, S.N), dtype=np.uint8)).cuda()
+        ph = torch.empty(cnt, dtype=torch.uint16, device="cuda")
+        e = np.array(gpmap.HP_ENERGIES, np.int32)
+        for label, on, c in (("tensor-core sequence_kernel", 1, cnt), ("CUDA-core kernel", 0, 1 << 17)):
+            gpmap.lib().gp_set_seq_tc(on)
+            t, _ = dev_time(lambda: S.enumerate_seqs(seqs[:c], ph[:c], None, e=e, alphabet=2), reps=1)
+            rows.append(dict(row="sampling: gp_enumerate_seqs, random HP sequences (%s)" % label, config="%s, %d sequences" % (name, c),
+                             seconds=t, evals_per_s=c * S.D / t, seconds_per_sequence=t / c,
+                             paper_gpu_seconds_per_sequence=paper_s))
+        gpmap.lib().gp_set_seq_tc(1)
+        del seqs, ph
     S = structs["4x4"]
     M = gpmap.seeded_matrix(SEED)
     n = 1 << a.mj_log2
