@@ -91,7 +91,9 @@ gp_status gp_enumerate_map(const gp_structures_t* s, const gp_energies* en, uint
 gp_status gp_enumerate_simple(const gp_structures_t* s, const gp_energies* en, uint64_t g_begin, uint64_t g_count,
                               uint16_t* d_pheno, int16_t* d_gap, void* stream);
 
-/* a8. Explicit sequences (the paper's SeqRnd path, :510-516, :762-775): d_seqs[count][N] letters < alphabet (2 or 20). */
+/* a8. Explicit sequences (the paper's SeqRnd path, :510-516, :762-775; its sampling runs :195-204): d_seqs[count][N]
+ * letters < alphabet (2 or 20).  Two-letter sequences whose energies fit the int8 weights (same bound as gp_enumerate)
+ * run on the tensor cores with the full 2 + N + P feature columns; everything else on the CUDA-core kernel. */
 gp_status gp_enumerate_seqs(const gp_structures_t* s, const gp_energies* en, const uint8_t* d_seqs, uint64_t count,
                             uint16_t* d_pheno, int16_t* d_gap, void* stream);
 /* a8. Sequences first..first+count-1 of the counter-based 20-letter generator of DESIGN.md section 4, drawn on chip. */
