@@ -158,19 +158,23 @@ struct Args {
 
 // ---- a1: feature rows -----------------------------------------------------------------------------------------------
 // Row r of A tile m holds genotype g0 + m*128 + r: byte c = val[c] * h_{i[c]} * h_{j[c]} on its low `fb` bits.
-__device__ __forceinline__ void build_a_row(uint8_t* a_tile, uint32_t r, uint32_t glow, const Cols& cols) {
+// `pk` = the column table in shared memory, one word per column (i | j << 8 | val << 16), read four columns per LDS.128:
+// with one byte-load per field the 384 loads per row went through the SM's single LSU pipe and the build took 12 000
+// clocks per supertile (clock64 timeline, profiles/r1_scoring_v4_ncu.md).
+__device__ __forceinline__ void build_a_row(uint8_t* a_tile, uint32_t r, uint32_t glow, const uint32_t* pk) {
     const uint32_t w = glow | 0x80000000u;  // bit 31: the constant-1 "monomer" used by the bias columns
 #pragma unroll 1
     for (uint32_t c16 = 0; c16 < ROWB / 16; c16++) {
         uint32_t q[4];
 #pragma unroll
         for (int wd = 0; wd < 4; wd++) {
+            const uint4 t4 = *reinterpret_cast<const uint4*>(pk + c16 * 16 + wd * 4);
+            const uint32_t t[4] = {t4.x, t4.y, t4.z, t4.w};
             uint32_t x = 0;
 #pragma unroll
             for (int b = 0; b < 4; b++) {
-                const uint32_t c = c16 * 16 + wd * 4 + b;
-                const uint32_t bit = (w >> cols.i[c]) & (w >> cols.j[c]) & 1u;
-                x |= (bit * cols.val[c]) << (8 * b);
+                const uint32_t bit = (w >> (t[b] & 31u)) & (w >> ((t[b] >> 8) & 31u)) & 1u;
+                x |= (bit * (t[b] >> 16)) << (8 * b);
             }
             q[wd] = x;
         }
@@ -243,7 +247,7 @@ __device__ __forceinline__ void fold_half_packed(const uint32_t* w, uint32_t col
     }
 }
 
-struct __align__(8) Barriers {
+struct __align__(16) Barriers {
     uint64_t b_full[NSTAGE], b_empty[NSTAGE];
     uint64_t acc_full[MT][2], acc_empty[MT][2];
     uint64_t a_full, a_empty;
@@ -260,14 +264,14 @@ __global__ void __launch_bounds__(THREADS, 1) scoring_kernel(const Args a, const
     uint8_t* sA = smem;                                   // MT tiles
     uint8_t* sB = smem + MT * TILE_BYTES;                 // NSTAGE tiles
     Barriers* bar = reinterpret_cast<Barriers*>(sB + NSTAGE * TILE_BYTES);
-    Cols* cols = reinterpret_cast<Cols*>(bar + 1);
+    uint32_t* pk = reinterpret_cast<uint32_t*>(bar + 1);  // packed column table, ROWB words
     constexpr int MN = TN / NH;                           // structures per MMA
     constexpr uint32_t IDESC = idesc_for(MN);
 
     const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
-    for (uint32_t i = threadIdx.x; i < sizeof(Cols); i += THREADS)
-        reinterpret_cast<uint8_t*>(cols)[i] = reinterpret_cast<const uint8_t*>(&cols_in)[i];
+    for (uint32_t c = threadIdx.x; c < ROWB; c += THREADS)
+        pk[c] = (uint32_t)cols_in.i[c] | ((uint32_t)cols_in.j[c] << 8) | ((uint32_t)cols_in.val[c] << 16);
     if (threadIdx.x == 0) {
         for (int s = 0; s < NSTAGE; s++) { mbar_init(&bar->b_full[s], 1); mbar_init(&bar->b_empty[s], 1); }
         for (int m = 0; m < MT; m++)
@@ -351,7 +355,7 @@ __global__ void __launch_bounds__(THREADS, 1) scoring_kernel(const Args a, const
         for (uint32_t item = blockIdx.x; item < a.n_items; item += gridDim.x, item_no++) {
             const uint64_t g = a.g_first + (uint64_t)item * SUPER + m * TM + r;
             mbar_wait(&bar->a_empty, (item_no & 1) ^ 1);
-            build_a_row(sA + m * TILE_BYTES, r, (uint32_t)g & lowmask, *cols);
+            build_a_row(sA + m * TILE_BYTES, r, (uint32_t)g & lowmask, pk);
             fence_proxy_async();
             mbar_arrive(&bar->a_full);
 
@@ -822,7 +826,7 @@ gp_status gp_launch_scoring_tc(gp_structures_s* s, const gp_hp_params& hp, uint6
     int dev = 0, sms = 0;
     GP_CUDA(cudaGetDevice(&dev));
     GP_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    const size_t smem = (size_t)(MT + NSTAGE) * TILE_BYTES + sizeof(Barriers) + sizeof(Cols) + 1024 + 64;
+    const size_t smem = (size_t)(MT + NSTAGE) * TILE_BYTES + sizeof(Barriers) + ROWB * sizeof(uint32_t) + 1024 + 64;
     const scoring_fn kernel = g_halves == 2 ? scoring_for<2, false>(k_steps)
                               : g_pack      ? scoring_for<1, true>(k_steps)
                                             : scoring_for<1, false>(k_steps);
@@ -916,7 +920,7 @@ gp_status gp_launch_map_tc(gp_structures_s* s, const gp_hp_params& hp, uint16_t*
     int dev = 0, sms = 0;
     GP_CUDA(cudaGetDevice(&dev));
     GP_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    const size_t smem = (size_t)(MT + NSTAGE) * TILE_BYTES + sizeof(Barriers) + sizeof(Cols) + 1024 + 64;
+    const size_t smem = (size_t)(MT + NSTAGE) * TILE_BYTES + sizeof(Barriers) + ROWB * sizeof(uint32_t) + 1024 + 64;
     const scoring_fn kernel = g_pack ? scoring_for<1, true>(k_steps) : scoring_for<1, false>(k_steps);
     GP_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const size_t need = (img_bytes + rec_bytes) * group;
