@@ -158,9 +158,9 @@ struct Args {
 
 // ---- a1: feature rows -----------------------------------------------------------------------------------------------
 // Row r of A tile m holds genotype g0 + m*128 + r: byte c = val[c] * h_{i[c]} * h_{j[c]} on its low `fb` bits.
-// `pk` = the column table in shared memory, one word per column (i | j << 8 | val << 16), read four columns per LDS.128:
-// with one byte-load per field the 384 loads per row went through the SM's single LSU pipe and the build took 12 000
-// clocks per supertile (clock64 timeline, profiles/r1_scoring_v4_ncu.md).
+// `pk` = the column table in shared memory, one word per column: the mask (1 << i) | (1 << j); the feature is 1 iff the
+// row word has all mask bits set (3 ALU operations per byte instead of 10; the build is ALU-bound: clock64 timeline in
+// profiles/r1_scoring_v4_ncu.md).  Column 0 (the x64 bias column) is the only one whose value is not 1.
 __device__ __forceinline__ void build_a_row(uint8_t* a_tile, uint32_t r, uint32_t glow, const uint32_t* pk) {
     const uint32_t w = glow | 0x80000000u;  // bit 31: the constant-1 "monomer" used by the bias columns
 #pragma unroll 1
@@ -172,12 +172,10 @@ __device__ __forceinline__ void build_a_row(uint8_t* a_tile, uint32_t r, uint32_
             const uint32_t t[4] = {t4.x, t4.y, t4.z, t4.w};
             uint32_t x = 0;
 #pragma unroll
-            for (int b = 0; b < 4; b++) {
-                const uint32_t bit = (w >> (t[b] & 31u)) & (w >> ((t[b] >> 8) & 31u)) & 1u;
-                x |= (bit * (t[b] >> 16)) << (8 * b);
-            }
+            for (int b = 0; b < 4; b++) x |= ((w & t[b]) == t[b] ? 1u : 0u) << (8 * b);
             q[wd] = x;
         }
+        if (c16 == 0) q[0] = (q[0] & ~0xFFu) | 64u;
         *reinterpret_cast<uint4*>(a_tile + r * ROWB + ((c16 ^ (r & 7u)) << 4)) = make_uint4(q[0], q[1], q[2], q[3]);
     }
 }
@@ -271,7 +269,7 @@ __global__ void __launch_bounds__(THREADS, 1) scoring_kernel(const Args a, const
     const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
     for (uint32_t c = threadIdx.x; c < ROWB; c += THREADS)
-        pk[c] = (uint32_t)cols_in.i[c] | ((uint32_t)cols_in.j[c] << 8) | ((uint32_t)cols_in.val[c] << 16);
+        pk[c] = cols_in.val[c] ? ((1u << cols_in.i[c]) | (1u << cols_in.j[c])) : 0xFFFFFFFFu;  // unused column: never all set
     if (threadIdx.x == 0) {
         for (int s = 0; s < NSTAGE; s++) { mbar_init(&bar->b_full[s], 1); mbar_init(&bar->b_empty[s], 1); }
         for (int m = 0; m < MT; m++)
