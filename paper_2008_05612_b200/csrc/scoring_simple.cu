@@ -23,65 +23,74 @@ struct SimpleArgs {
     int16_t* gap;
     uint64_t first, count, seed;
     uint32_t D;
-    int N, NBP, P, alphabet, threshold;
+    int N, NBP, P, alphabet, threshold, emax;
 };
 
+// Two sequences per thread: the pair energies are stored as non-negative 16-bit costs (emax - e) packed two to a word,
+// so one shared-memory load and one integer add serve both sequences, with no carry between the halves
+// (NBP * (emax - emin) < 2^16 is checked by the launcher).  The minimum energy is the maximum cost.
 template <int SRC>
 __global__ void __launch_bounds__(128) score_simple_kernel(SimpleArgs a, const int16_t* __restrict__ e_dev) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int BD = blockDim.x, tid = threadIdx.x;
-    int16_t* pe = reinterpret_cast<int16_t*>(smem_raw);                  // [P][BD]
-    uint16_t* sidx = reinterpret_cast<uint16_t*>(pe + (size_t)a.P * BD);  // [CHUNK][NBP]
+    uint32_t* pe = reinterpret_cast<uint32_t*>(smem_raw);                 // [P][BD] packed costs of the thread's two sequences
+    uint16_t* sidx = reinterpret_cast<uint16_t*>(pe + (size_t)a.P * BD);  // [CHUNK][NBP] pair index * BD
     int16_t* em = reinterpret_cast<int16_t*>(sidx + (size_t)CHUNK * a.NBP);  // [alphabet^2]
-    uint8_t* let = reinterpret_cast<uint8_t*>(em + 400);                 // [N][BD]
-    uint8_t* pij = let + (size_t)a.N * BD;                               // [P][2]
+    uint8_t* let = reinterpret_cast<uint8_t*>(em + 400);                  // [N][2 BD]
+    uint8_t* pij = let + (size_t)a.N * 2 * BD;                            // [P][2]
 
     for (int i = tid; i < a.alphabet * a.alphabet; i += BD) em[i] = e_dev[i];
     for (int i = tid; i < 2 * a.P; i += BD) pij[i] = a.pair_ij[i];
 
-    const uint64_t n_tiles = (a.count + BD - 1) / BD;
+    const uint64_t n_tiles = (a.count + 2 * BD - 1) / (2 * BD);
     for (uint64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-        const uint64_t q = tile * BD + tid;  // sequence number within the call
-        const bool live = q < a.count;
+        const uint64_t q[2] = {tile * 2 * BD + tid, tile * 2 * BD + BD + tid};  // sequence numbers within the call
+        const bool live[2] = {q[0] < a.count, q[1] < a.count};
         __syncthreads();
-        if (live) {
+#pragma unroll
+        for (int h = 0; h < 2; h++)
             for (int k = 0; k < a.N; k++) {
-                uint32_t l;
-                if (SRC == SRC_BITS) l = (uint32_t)(((a.first + q) >> k) & 1ULL);
-                else if (SRC == SRC_SEQS) l = a.seqs[q * a.N + k];
-                else l = gp_letter20(a.seed, a.first + q, k);
-                let[k * BD + tid] = (uint8_t)l;
+                uint32_t l = 0;
+                if (live[h]) {
+                    if (SRC == SRC_BITS) l = (uint32_t)(((a.first + q[h]) >> k) & 1ULL);
+                    else if (SRC == SRC_SEQS) l = a.seqs[q[h] * a.N + k];
+                    else l = gp_letter20(a.seed, a.first + q[h], k);
+                }
+                let[(k * 2 + h) * BD + tid] = (uint8_t)l;
             }
-            for (int p = 0; p < a.P; p++) {
-                int li = let[pij[2 * p] * BD + tid], lj = let[pij[2 * p + 1] * BD + tid];
-                pe[p * BD + tid] = em[li * a.alphabet + lj];
-            }
+        for (int p = 0; p < a.P; p++) {
+            const int i = pij[2 * p], j = pij[2 * p + 1];
+            const uint32_t c0 = (uint32_t)(a.emax - em[let[(i * 2) * BD + tid] * a.alphabet + let[(j * 2) * BD + tid]]);
+            const uint32_t c1 = (uint32_t)(a.emax - em[let[(i * 2 + 1) * BD + tid] * a.alphabet + let[(j * 2 + 1) * BD + tid]]);
+            pe[p * BD + tid] = c0 | (c1 << 16);
         }
-        int32_t m1 = INT32_MAX, m2 = INT32_MAX;
-        uint32_t arg = 0;
+        int32_t M1[2] = {-1, -1}, M2[2] = {-1, -1};  // largest and second-largest cost (with multiplicity)
+        uint32_t arg[2] = {0, 0};
         for (uint32_t d0 = 0; d0 < a.D; d0 += CHUNK) {
             const uint32_t nd = min((uint32_t)CHUNK, a.D - d0);
             __syncthreads();
-            for (uint32_t i = tid; i < nd * a.NBP; i += BD) sidx[i] = a.pairidx[(size_t)d0 * a.NBP + i];
+            for (uint32_t i = tid; i < nd * a.NBP; i += BD) sidx[i] = (uint16_t)(a.pairidx[(size_t)d0 * a.NBP + i] * BD);
             __syncthreads();
-            if (live) {
-                for (uint32_t c = 0; c < nd; c++) {
-                    const uint16_t* ix = sidx + c * a.NBP;
-                    int32_t E = 0;
-                    for (int k = 0; k < a.NBP; k++) E += pe[ix[k] * BD + tid];
-                    if (E < m1) { m2 = m1; m1 = E; arg = d0 + c; }
-                    else if (E < m2) { m2 = E; }
+            const uint32_t* mine = pe + tid;
+            for (uint32_t c = 0; c < nd; c++) {
+                const uint16_t* ix = sidx + c * a.NBP;
+                uint32_t S = 0;
+                for (int k = 0; k < a.NBP; k++) S += mine[ix[k]];
+#pragma unroll
+                for (int h = 0; h < 2; h++) {
+                    const int32_t cost = (int32_t)(h ? (S >> 16) : (S & 0xFFFFu));
+                    if (cost > M1[h]) { M2[h] = M1[h]; M1[h] = cost; arg[h] = d0 + c; }
+                    else if (cost > M2[h]) { M2[h] = cost; }
                 }
             }
         }
-        if (live) {
-            const bool folds = (m2 == INT32_MAX) || (m2 - m1 >= a.threshold);
-            a.pheno[q] = folds ? a.class_of[arg] : (uint16_t)GP_NULL_PHENO;
-            if (a.gap) {
-                int32_t g = (m2 == INT32_MAX) ? GP_GAP_NONE : max(m1 - m2, -32768);
-                a.gap[q] = (int16_t)g;
+#pragma unroll
+        for (int h = 0; h < 2; h++)
+            if (live[h]) {
+                const bool folds = (M2[h] < 0) || (M1[h] - M2[h] >= a.threshold);
+                a.pheno[q[h]] = folds ? a.class_of[arg[h]] : (uint16_t)GP_NULL_PHENO;
+                if (a.gap) a.gap[q[h]] = (int16_t)((M2[h] < 0) ? GP_GAP_NONE : max(M2[h] - M1[h], -32768));
             }
-        }
     }
 }
 
@@ -94,13 +103,17 @@ gp_status launch_simple(const gp_structures_s* s, const gp_energies* en, int src
     if (s->device < 0) { gp_set_cuda_error(cudaErrorNoDevice, "handle has no device tables"); return GP_CUDA_ERROR; }
     const int A = en->alphabet;
     int16_t h_e[400];
+    int32_t emax = INT32_MIN, emin = INT32_MAX;
     for (int i = 0; i < A; i++)
         for (int j = 0; j < A; j++) {
             int32_t v = en->e[i * A + j];
             if (v != en->e[j * A + i]) return GP_INVALID_ARG;
             if ((long long)v * s->NBP > 32767 || (long long)v * s->NBP < -32767) return GP_INVALID_ARG;
             h_e[i * A + j] = (int16_t)v;
+            emax = v > emax ? v : emax;
+            emin = v < emin ? v : emin;
         }
+    if ((long long)(emax - emin) * s->NBP > 65535 || (size_t)s->P * 128 > 65535) return GP_INVALID_ARG;  // packed 16-bit costs / offsets
     if (count == 0) return GP_OK;
     int16_t* d_e = nullptr;
     GP_CUDA(cudaMallocAsync(&d_e, sizeof(h_e), st));
@@ -109,13 +122,13 @@ gp_status launch_simple(const gp_structures_s* s, const gp_energies* en, int src
     SimpleArgs a;
     a.pairidx = s->d_pairidx; a.pair_ij = s->d_pair_ij; a.class_of = s->d_class_of; a.seqs = d_seqs;
     a.pheno = d_pheno; a.gap = d_gap; a.first = first; a.count = count; a.seed = seed;
-    a.D = s->D; a.N = s->N; a.NBP = s->NBP; a.P = s->P; a.alphabet = A; a.threshold = en->threshold;
+    a.D = s->D; a.N = s->N; a.NBP = s->NBP; a.P = s->P; a.alphabet = A; a.threshold = en->threshold; a.emax = emax;
     const int BD = 128;
-    size_t smem = (size_t)s->P * BD * 2 + (size_t)CHUNK * s->NBP * 2 + 800 + (size_t)s->N * BD + (size_t)s->P * 2 + 16;
+    size_t smem = (size_t)s->P * BD * 4 + (size_t)CHUNK * s->NBP * 2 + 800 + (size_t)s->N * 2 * BD + (size_t)s->P * 2 + 16;
     int dev = 0, sms = 0;
     GP_CUDA(cudaGetDevice(&dev));
     GP_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    uint64_t tiles = (count + BD - 1) / BD;
+    uint64_t tiles = (count + 2 * BD - 1) / (2 * BD);
     int per_sm = (int)(200 * 1024 / smem);
     if (per_sm < 1) per_sm = 1;
     if (per_sm > 8) per_sm = 8;
