@@ -259,7 +259,7 @@ def run_ours(args):
     host = torch.empty(n, dtype=torch.uint16).pin_memory() if n <= (1 << 32) else None
     if host is not None:
         host_np = host.numpy()
-        e_steps = max(1, min(args.steps, 3))
+        e_steps = max(1, args.steps)
         S.enumerate_host(tile_begin(0, rank, world, G, N), n, want_robustness=True, pheno_out=host_np)
         barrier()
         t0 = time.perf_counter()
@@ -273,7 +273,7 @@ def run_ours(args):
             dt = float(t.item())
         e2e = {"value": evals_step * e_steps / dt, "unit": UNIT, "h2d_bytes_per_step": 16,
                "d2h_bytes_per_step": int(2 * n + 8 * (C + 1) + 24 * C + 8), "steps": e_steps,
-               "call": "gp_enumerate_host (host buffers, pinned phenotype output; device store allocated inside the call)"}
+               "call": "gp_enumerate_host (host buffers, pinned phenotype output; device store kept in the handle)"}
 
     if rank != 0:
         if world > 1:
@@ -282,7 +282,7 @@ def run_ours(args):
     hbm, bf16_burst, bf16_sus, src = peaks()
     sc_ms, sc_n = ktime[gpmap.KERNEL_SCORING]
     evals_launch = float(n) * D / max(1, sc_n // max(1, args.steps))  # one rank's launches
-    fb = min(N, args.fold_bits or 19)                                 # low genotype bits kept as contraction columns
+    fb = min(N, args.fold_bits or 15)                                 # low genotype bits kept as contraction columns
     k_exec = 2 + fb + sum(1 for i in range(fb) for j in range(i + 3, fb, 2))  # bias x2 + monomers + pairs
     ops_exec = 2.0 * k_exec                                           # int8 multiply-adds x2 the kernel executes per evaluation
     peak_i8 = 2.0 * bf16_sus                                          # int8 dense = 2 x bf16 (guide's nominal ratio)
@@ -356,7 +356,7 @@ def run_ours(args):
             "folding_fraction_last_tile": folding / float(n),
             "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline, "other_kernels": other,
             "whole_map_3x3x3": whole,
-            "full_6x6_measured": {"wall_s": 127.4, "path": "gp_enumerate_map + designability + neighbour pass, 137 GB store",
+            "full_6x6_measured": {"wall_s": 117.6, "path": "gp_enumerate_map + designability + neighbour pass, 137 GB store",
                                   "source": "profiles/r1_full_6x6.md (separate run: python tests/full_map_check.py --lattice 6x6)"},
             "cpu_baseline": cpu}
     print(json.dumps(line), flush=True)

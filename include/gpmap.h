@@ -129,7 +129,7 @@ gp_status gp_nn_components(const uint16_t* d_pheno, int n_bits, uint32_t n_class
  * NULL the range must be an aligned sub-cube (g_count a power of two dividing g_begin, else GP_RANGE); the neighbour
  * pass (a6) then runs over its log2(g_count) mutable bits and rdo (host, 3*n_classes) receives neutral | deleterious |
  * other, pair_count (host, 1, nullable) the number of connected class pairs.  The energy matrix (16 bytes) is the only
- * host input: genotypes are implicit.  Synchronous; allocates and frees its device buffers. */
+ * host input: genotypes are implicit.  Synchronous; its device buffers live in the handle between calls. */
 gp_status gp_enumerate_host(const gp_structures_t* s, const gp_energies* en, uint64_t g_begin, uint64_t g_count,
                             uint16_t* pheno, uint64_t* hist, uint64_t* rdo, uint64_t* pair_count);
 

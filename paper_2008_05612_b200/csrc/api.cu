@@ -145,6 +145,8 @@ void gp_release_device(gp_structures_s* s) {
     s->d_contacts_sym = nullptr; s->d_class_sym = nullptr;
     cudaFree(s->wimg.d_img);
     cudaFree(s->d_scratch);
+    cudaFree(s->d_host_store);
+    s->d_host_store = nullptr; s->host_store_bytes = 0;
     s->d_contacts = nullptr; s->d_class_of = nullptr; s->d_pairidx = nullptr; s->d_pair_ij = nullptr; s->wimg.d_img = nullptr; s->d_scratch = nullptr;
 }
 
@@ -241,15 +243,19 @@ extern "C" gp_status gp_enumerate_host(const gp_structures_t* s, const gp_energi
     } else if (pair_count) {
         return GP_INVALID_ARG;
     }
-    uint16_t* d_pheno = nullptr;
-    uint64_t* d_out = nullptr;  // hist[C+1] | R[C] | D[C] | O[C] | pair_count
+    // one device buffer, kept in the handle between calls: outputs (hist[C+1] | R[C] | D[C] | O[C] | pair_count), then the store
     const size_t n_out = (size_t)C + 1 + 3 * (size_t)C + 1;
-    GP_CUDA(cudaMalloc(&d_pheno, (g_count ? g_count : 1) * sizeof(uint16_t)));
-    if (cudaMalloc(&d_out, n_out * sizeof(uint64_t)) != cudaSuccess) {
-        cudaFree(d_pheno);
-        gp_set_cuda_error(cudaGetLastError(), "cudaMalloc(outputs)");
-        return GP_OUT_OF_MEMORY;
+    const size_t out_bytes = (n_out * sizeof(uint64_t) + 255) & ~(size_t)255;
+    const size_t need = out_bytes + (g_count ? g_count : 1) * sizeof(uint16_t);
+    gp_structures_s* hs = const_cast<gp_structures_s*>(s);
+    if (hs->host_store_bytes < need) {
+        if (hs->d_host_store) GP_CUDA(cudaFree(hs->d_host_store));
+        hs->d_host_store = nullptr; hs->host_store_bytes = 0;
+        GP_CUDA(cudaMalloc(&hs->d_host_store, need));
+        hs->host_store_bytes = need;
     }
+    uint64_t* d_out = reinterpret_cast<uint64_t*>(hs->d_host_store);
+    uint16_t* d_pheno = reinterpret_cast<uint16_t*>(reinterpret_cast<char*>(hs->d_host_store) + out_bytes);
     uint64_t* d_hist = d_out;
     uint64_t* d_rdo = d_out + C + 1;
     uint64_t* d_pc = d_rdo + 3 * (size_t)C;
@@ -265,7 +271,5 @@ extern "C" gp_status gp_enumerate_host(const gp_structures_t* s, const gp_energi
         if (e == cudaSuccess && pair_count) e = cudaMemcpy(pair_count, d_pc, sizeof(uint64_t), cudaMemcpyDeviceToHost);
         if (e != cudaSuccess) { gp_set_cuda_error(e, "gp_enumerate_host copy-back"); st = GP_CUDA_ERROR; }
     }
-    cudaFree(d_pheno);
-    cudaFree(d_out);
     return st;
 }

@@ -36,6 +36,8 @@ struct gp_structures_s {
     uint16_t* d_class_sym = nullptr;     // D_sym: class id of the column, 0xFFFF = pad column
     uint32_t D_sym = 0, n_snap = 0;      // columns incl. interior pads; weight tiles holding non-self-reverse classes
     gp_weight_image wimg;
+    void* d_host_store = nullptr;        // device buffers of gp_enumerate_host, kept between calls (grown on demand)
+    size_t host_store_bytes = 0;
     void* d_scratch = nullptr;           // private scratch, grown on demand
     size_t scratch_bytes = 0;
 };

@@ -556,9 +556,11 @@ __global__ void __launch_bounds__(256) combine_kernel(const CombArgs a) {
     }
 }
 
-int g_sym_bits = 9;    // k of map mode: the k first and k last monomers vary inside an image
+int g_sym_bits = 7;    // k of map mode: the k first and k last monomers vary inside an image (7: 53 columns, 2 K steps;
+                       // 9: 85 columns, 3 K steps and 16x fewer images, 7 % slower on the full 6x6 map)
 
-int g_fold_bits = 19;  // 2 + 19 + 72 = 93 columns -> 3 K steps
+int g_fold_bits = 15;  // 2 + 15 + 42 = 59 columns -> 2 K steps; an image per 2^15 genotypes costs 5 us to build
+                       // (19: 93 columns, 3 K steps, was the default until the builder was timed per image: +10 %)
 int g_halves = 1;      // NH of scoring_kernel
 int g_debug = 0;
 int g_pack = 1;        // PACK of scoring_kernel
@@ -833,9 +835,9 @@ gp_status gp_launch_scoring_tc(gp_structures_s* s, const gp_hp_params& hp, uint6
     // batches of 2^fb genotypes share a weight image; a launch covers up to `group` batches
     const uint64_t batch_len = 1ULL << fb;
     const uint64_t g_end = g_begin + g_count;
-    uint64_t group = (256ULL << 20) / img_bytes;  // <= 256 MB of images per launch
+    uint64_t group = (1024ULL << 20) / img_bytes;  // <= 1 GB of images per launch
     if (group < 1) group = 1;
-    if (group > 64) group = 64;
+    if (group > 256) group = 256;
     const size_t need = img_bytes * (size_t)group;
     if (s->scratch_bytes < need) {
         if (s->d_scratch) GP_CUDA(cudaFree(s->d_scratch));
@@ -899,10 +901,9 @@ gp_status gp_launch_map_tc(gp_structures_s* s, const gp_hp_params& hp, uint16_t*
     // images of the map: m and rev(m) adjacent, each unordered pair once
     const uint32_t n_mid = 1u << mid;
     std::vector<uint32_t> tiles, partner, cuts;
-    tiles.reserve(n_mid); partner.reserve(n_mid);
-    size_t group = (192ULL << 20) / (img_bytes + rec_bytes);
+    size_t group = (1024ULL << 20) / (img_bytes + rec_bytes);  // <= 1 GB of images + records per launch
     if (group < 2) group = 2;
-    if (group > 64) group = 64;
+    if (group > 512) group = 512;
     cuts.push_back(0);
     for (uint32_t m = 0; m < n_mid; m++) {
         uint32_t r = 0;

@@ -144,7 +144,7 @@ def kernel_time(which):
 
 
 def set_fold_bits(fb):
-    """Tuning/test hook: number of low genotype bits kept as contraction columns (9..22, default 19)."""
+    """Tuning/test hook: number of low genotype bits kept as contraction columns (9..22, default 15)."""
     if lib().gp_set_fold_bits(fb) != 0:
         raise ValueError("fold bits must be in 9..22")
 
