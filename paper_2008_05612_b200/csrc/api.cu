@@ -87,6 +87,15 @@ gp_status gp_upload_tables(gp_structures_s* s) {
         return GP_OK;
     }
     GP_CUDA(cudaGetDevice(&s->device));
+    {   // the reductions take their scratch (pair bitmap, union-find parents) from the stream-ordered pool: keep freed
+        // blocks in the pool instead of handing them back to the driver at every synchronisation
+        cudaMemPool_t pool;
+        if (cudaDeviceGetDefaultMemPool(&pool, s->device) == cudaSuccess) {
+            uint64_t keep = ~0ULL;
+            cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+        }
+        cudaGetLastError();
+    }
     GP_CUDA(cudaMalloc(&s->d_contacts, s->contacts.size()));
     GP_CUDA(cudaMemcpy(s->d_contacts, s->contacts.data(), s->contacts.size(), cudaMemcpyHostToDevice));
     GP_CUDA(cudaMalloc(&s->d_class_of, s->class_of.size() * sizeof(uint16_t)));
