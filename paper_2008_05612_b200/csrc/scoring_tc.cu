@@ -135,6 +135,17 @@ __host__ __device__ constexpr uint32_t idesc_for(int n) {
 __host__ __device__ __forceinline__ uint32_t swz(uint32_t r, uint32_t c) {
     return r * ROWB + ((((c >> 4) ^ (r & 7u)) << 4) | (c & 15u));
 }
+// the same for rows of RB = 64 bytes (64-byte swizzle: 16-byte chunk index ^ bits 1-2 of the row) or 128 bytes
+template <int RB>
+__host__ __device__ __forceinline__ uint32_t swz_rb(uint32_t r, uint32_t c) {
+    return RB == 128 ? swz(r, c) : r * 64u + ((((c >> 4) ^ ((r >> 1) & 3u)) << 4) | (c & 15u));
+}
+// K-major shared-memory descriptor for rows of RB bytes: 8-row groups RB*8 bytes apart, 128- or 64-byte swizzle
+template <int RB>
+__device__ __forceinline__ uint64_t smem_desc_rb(uint32_t saddr) {
+    return (uint64_t)((saddr & 0x3FFFFu) >> 4) | (1ULL << 16) | ((uint64_t)((RB * 8) >> 4) << 32) | (1ULL << 46) |
+           ((RB == 128 ? 2ULL : 4ULL) << 61);
+}
 
 struct Args {
     const int8_t* img;        // [n_batches][n_tiles][TILE_BYTES]
@@ -161,10 +172,12 @@ struct Args {
 // `pk` = the column table in shared memory, one word per column: the mask (1 << i) | (1 << j); the feature is 1 iff the
 // row word has all mask bits set (3 ALU operations per byte instead of 10; the build is ALU-bound: clock64 timeline in
 // profiles/r1_scoring_v4_ncu.md).  Column 0 (the x64 bias column) is the only one whose value is not 1.
+template <int RB>
 __device__ __forceinline__ void build_a_row(uint8_t* a_tile, uint32_t r, uint32_t glow, const uint32_t* pk) {
     const uint32_t w = glow | 0x80000000u;  // bit 31: the constant-1 "monomer" used by the bias columns
+    const uint32_t sw = RB == 128 ? (r & 7u) : ((r >> 1) & 3u);
 #pragma unroll 1
-    for (uint32_t c16 = 0; c16 < ROWB / 16; c16++) {
+    for (uint32_t c16 = 0; c16 < RB / 16; c16++) {
         uint32_t q[4];
 #pragma unroll
         for (int wd = 0; wd < 4; wd++) {
@@ -176,7 +189,7 @@ __device__ __forceinline__ void build_a_row(uint8_t* a_tile, uint32_t r, uint32_
             q[wd] = x;
         }
         if (c16 == 0) q[0] = (q[0] & ~0xFFu) | 64u;
-        *reinterpret_cast<uint4*>(a_tile + r * ROWB + ((c16 ^ (r & 7u)) << 4)) = make_uint4(q[0], q[1], q[2], q[3]);
+        *reinterpret_cast<uint4*>(a_tile + r * RB + ((c16 ^ sw) << 4)) = make_uint4(q[0], q[1], q[2], q[3]);
     }
 }
 
@@ -255,13 +268,15 @@ struct __align__(16) Barriers {
 // KS = 32-byte K steps per MMA chain (1..4); NH = 1: one N=128 MMA chain per accumulator, NH = 2: two N=64 chains into
 // independent halves (the tensor pipe refills one half while the other is drained).  PACK (NH = 1 only): the epilogue
 // reads the whole accumulator as packed int16 pairs, releases it at once and folds with two-lane SIMD min.
-template <int KS, int NH, bool PACK>
+// RB = bytes per operand row: 64 when the contraction has at most 64 columns (half the weight-tile and feature-row traffic)
+template <int KS, int NH, bool PACK, int RB>
 __global__ void __launch_bounds__(THREADS, 1) scoring_kernel(const Args a, const Cols cols_in) {
+    constexpr int TB = TM * RB;                           // bytes of an A tile / a weight tile
     extern __shared__ unsigned char smem_dyn[];
     unsigned char* smem = reinterpret_cast<unsigned char*>(((uintptr_t)smem_dyn + 1023) & ~(uintptr_t)1023);
     uint8_t* sA = smem;                                   // MT tiles
-    uint8_t* sB = smem + MT * TILE_BYTES;                 // NSTAGE tiles
-    Barriers* bar = reinterpret_cast<Barriers*>(sB + NSTAGE * TILE_BYTES);
+    uint8_t* sB = smem + MT * TB;                         // NSTAGE tiles
+    Barriers* bar = reinterpret_cast<Barriers*>(sB + NSTAGE * TB);
     uint32_t* pk = reinterpret_cast<uint32_t*>(bar + 1);  // packed column table, ROWB words
     constexpr int MN = TN / NH;                           // structures per MMA
     constexpr uint32_t IDESC = idesc_for(MN);
@@ -294,21 +309,21 @@ __global__ void __launch_bounds__(THREADS, 1) scoring_kernel(const Args a, const
         for (uint32_t item = blockIdx.x; item < a.n_items; item += gridDim.x) {
             const uint64_t g0 = a.g_first + (uint64_t)item * SUPER;
             const uint64_t batch = (g0 >> a.fb) - (a.g_first >> a.fb);
-            const int8_t* img = a.img + batch * (uint64_t)a.n_tiles * TILE_BYTES;
+            const int8_t* img = a.img + batch * (uint64_t)a.n_tiles * TB;
             for (uint32_t n = 0; n < a.n_tiles; n++, it++) {
                 const uint32_t s = it % NSTAGE, ph = (it / NSTAGE) & 1;
                 mbar_wait(&bar->b_empty[s], ph ^ 1);
                 if (elect_one()) {
-                    mbar_expect_tx(&bar->b_full[s], TILE_BYTES);
-                    bulk_g2s(sB + s * TILE_BYTES, img + (uint64_t)n * TILE_BYTES, TILE_BYTES, &bar->b_full[s]);
+                    mbar_expect_tx(&bar->b_full[s], TB);
+                    bulk_g2s(sB + s * TB, img + (uint64_t)n * TB, TB, &bar->b_full[s]);
                 }
                 __syncwarp();
             }
         }
     } else if (warp == 1) {
         // ===== MMA issuer: warp-uniform loop, one elected lane issues =====
-        const uint64_t a_desc0 = smem_desc(smem_u32(sA));
-        const uint64_t b_desc0 = smem_desc(smem_u32(sB));
+        const uint64_t a_desc0 = smem_desc_rb<RB>(smem_u32(sA));
+        const uint64_t b_desc0 = smem_desc_rb<RB>(smem_u32(sB));
         uint32_t it = 0, item_no = 0;
         for (uint32_t item = blockIdx.x; item < a.n_items; item += gridDim.x, item_no++) {
             mbar_wait(&bar->a_full, item_no & 1);
@@ -317,7 +332,7 @@ __global__ void __launch_bounds__(THREADS, 1) scoring_kernel(const Args a, const
                 const uint32_t s = it % NSTAGE, ph = (it / NSTAGE) & 1;
                 mbar_wait(&bar->b_full[s], ph);
                 tc_fence_after();
-                const uint64_t bd = b_desc0 + (uint64_t)(s * (TILE_BYTES >> 4));
+                const uint64_t bd = b_desc0 + (uint64_t)(s * (TB >> 4));
 #pragma unroll
                 for (int h = 0; h < NH; h++) {
 #pragma unroll
@@ -326,8 +341,8 @@ __global__ void __launch_bounds__(THREADS, 1) scoring_kernel(const Args a, const
                         tc_fence_after();
                         if (elect_one()) {
                             const uint32_t d = tmem + m * TN + h * MN;
-                            const uint64_t ad = a_desc0 + (uint64_t)((m * TILE_BYTES) >> 4);
-                            const uint64_t bdh = bd + (uint64_t)((h * MN * ROWB) >> 4);
+                            const uint64_t ad = a_desc0 + (uint64_t)((m * TB) >> 4);
+                            const uint64_t bdh = bd + (uint64_t)((h * MN * RB) >> 4);
                             mma_i8_c<false>(d, ad, bdh, IDESC);
 #pragma unroll
                             for (int k = 1; k < KS; k++) mma_i8_c<true>(d, ad + 2 * k, bdh + 2 * k, IDESC);
@@ -353,7 +368,7 @@ __global__ void __launch_bounds__(THREADS, 1) scoring_kernel(const Args a, const
         for (uint32_t item = blockIdx.x; item < a.n_items; item += gridDim.x, item_no++) {
             const uint64_t g = a.g_first + (uint64_t)item * SUPER + m * TM + r;
             mbar_wait(&bar->a_empty, (item_no & 1) ^ 1);
-            build_a_row(sA + m * TILE_BYTES, r, (uint32_t)g & lowmask, pk);
+            build_a_row<RB>(sA + m * TB, r, (uint32_t)g & lowmask, pk);
             fence_proxy_async();
             mbar_arrive(&bar->a_full);
 
@@ -426,13 +441,13 @@ __global__ void __launch_bounds__(THREADS, 1) scoring_kernel(const Args a, const
 }
 
 typedef void (*scoring_fn)(const Args, const Cols);
-template <int NH, bool PACK>
+template <int NH, bool PACK, int RB>
 scoring_fn scoring_for(int ks) {
     switch (ks) {
-        case 1: return scoring_kernel<1, NH, PACK>;
-        case 2: return scoring_kernel<2, NH, PACK>;
-        case 3: return scoring_kernel<3, NH, PACK>;
-        default: return scoring_kernel<4, NH, PACK>;
+        case 1: return scoring_kernel<1, NH, PACK, RB>;
+        case 2: return scoring_kernel<2, NH, PACK, RB>;
+        case 3: return scoring_kernel<3, NH, PACK, RB>;
+        default: return scoring_kernel<4, NH, PACK, RB>;
     }
 }
 
@@ -456,11 +471,13 @@ struct ImgArgs {
 
 // One block = one 128-structure tile of one image.  Thread = structure: it accumulates its 128-byte weight row in
 // shared memory (already in the swizzled layout the MMA reads), then the block writes the 16 KB tile out coalesced.
+template <int RB>
 __global__ void __launch_bounds__(TN) build_image_kernel(const ImgArgs a, const Slots slots) {
-    __shared__ __align__(16) int8_t tile[TILE_BYTES];
+    constexpr int TB = TM * RB;
+    __shared__ __align__(16) int8_t tile[TB];
     const uint32_t r = threadIdx.x, n = blockIdx.x;
     const uint64_t G = (a.tile_list ? (uint64_t)a.tile_list[a.list_first + blockIdx.y] : a.gfix_first + blockIdx.y) << a.gfix_shift;
-    for (uint32_t i = threadIdx.x; i < TILE_BYTES / 16; i += TN) reinterpret_cast<uint4*>(tile)[i] = make_uint4(0, 0, 0, 0);
+    for (uint32_t i = threadIdx.x; i < TB / 16; i += TN) reinterpret_cast<uint4*>(tile)[i] = make_uint4(0, 0, 0, 0);
     __syncthreads();
     const uint32_t d = n * TN + r;
     if (d < a.D && a.class_of[d] != GP_NULL_PHENO) {
@@ -471,28 +488,28 @@ __global__ void __launch_bounds__(TN) build_image_kernel(const ImgArgs a, const 
             const int li = slots.loc[i], lj = slots.loc[j];
             const int hi = (int)((G >> i) & 1ULL), hj = (int)((G >> j) & 1ULL);
             if (li >= 0 && lj >= 0) {
-                tile[swz(r, 2 + li)] += (int8_t)a.lin;
-                tile[swz(r, 2 + lj)] += (int8_t)a.lin;
-                tile[swz(r, slots.pair[li * MAX_FB + lj])] = (int8_t)a.quad;
+                tile[swz_rb<RB>(r, 2 + li)] += (int8_t)a.lin;
+                tile[swz_rb<RB>(r, 2 + lj)] += (int8_t)a.lin;
+                tile[swz_rb<RB>(r, slots.pair[li * MAX_FB + lj])] = (int8_t)a.quad;
             } else if (li >= 0) {
-                tile[swz(r, 2 + li)] += (int8_t)(a.lin + a.quad * hj);
+                tile[swz_rb<RB>(r, 2 + li)] += (int8_t)(a.lin + a.quad * hj);
                 bias += a.lin * hj;
             } else if (lj >= 0) {
-                tile[swz(r, 2 + lj)] += (int8_t)(a.lin + a.quad * hi);
+                tile[swz_rb<RB>(r, 2 + lj)] += (int8_t)(a.lin + a.quad * hi);
                 bias += a.lin * hi;
             } else {
                 bias += a.lin * (hi + hj) + a.quad * hi * hj;
             }
         }
-        tile[swz(r, 0)] = (int8_t)(bias >> 6);   // x 64
-        tile[swz(r, 1)] = (int8_t)(bias & 63);   // x 1
+        tile[swz_rb<RB>(r, 0)] = (int8_t)(bias >> 6);   // x 64
+        tile[swz_rb<RB>(r, 1)] = (int8_t)(bias & 63);   // x 1
     } else {                                     // pad structure: energy E_PAD for every genotype
-        tile[swz(r, 0)] = 127;
-        tile[swz(r, 1)] = 63;
+        tile[swz_rb<RB>(r, 0)] = 127;
+        tile[swz_rb<RB>(r, 1)] = 63;
     }
     __syncthreads();
-    uint4* dst = reinterpret_cast<uint4*>(a.img + ((uint64_t)blockIdx.y * a.n_tiles + n) * TILE_BYTES);
-    for (uint32_t i = threadIdx.x; i < TILE_BYTES / 16; i += TN) dst[i] = reinterpret_cast<const uint4*>(tile)[i];
+    uint4* dst = reinterpret_cast<uint4*>(a.img + ((uint64_t)blockIdx.y * a.n_tiles + n) * TB);
+    for (uint32_t i = threadIdx.x; i < TB / 16; i += TN) dst[i] = reinterpret_cast<const uint4*>(tile)[i];
 }
 
 // Columns of the folded contraction for a set of free monomers mon[0..fb-1] (increasing): 2 bias columns, fb monomer
@@ -563,6 +580,7 @@ int g_fold_bits = 15;  // 2 + 15 + 42 = 59 columns -> 2 K steps; an image per 2^
                        // (19: 93 columns, 3 K steps, was the default until the builder was timed per image: +10 %)
 int g_halves = 1;      // NH of scoring_kernel
 int g_debug = 0;
+int g_narrow = 1;      // 64-byte operand rows when the contraction has at most 64 columns
 int g_pack = 1;        // PACK of scoring_kernel
 
 // =====================================================================================================================
@@ -800,6 +818,7 @@ extern "C" int gp_set_sym_bits(int k) {  // test / tuning hook
     tc::g_sym_bits = k;
     return 0;
 }
+extern "C" int gp_set_narrow(int on) { tc::g_narrow = on != 0; return 0; }  // test / tuning hook
 extern "C" int gp_set_pack(int p) { tc::g_pack = p != 0; return 0; }
 extern "C" int gp_set_halves(int nh) {  // test / tuning hook
     if (nh != 1 && nh != 2) return -1;
@@ -821,15 +840,19 @@ gp_status gp_launch_scoring_tc(gp_structures_s* s, const gp_hp_params& hp, uint6
     if (nc > ROWB) return GP_INVALID_ARG;
     const int k_steps = (nc + 31) / 32;
     const uint32_t n_tiles = (s->D + TN - 1) / TN;
-    const size_t img_bytes = (size_t)n_tiles * TILE_BYTES;
+    // at most 64 columns: 64-byte operand rows (half the image, weight-tile and feature-row traffic)
+    const bool narrow = nc <= 64 && g_narrow && g_halves == 1 && g_pack;
+    const size_t tile_bytes = (size_t)TM * (narrow ? 64 : 128);
+    const size_t img_bytes = (size_t)n_tiles * tile_bytes;
 
     int dev = 0, sms = 0;
     GP_CUDA(cudaGetDevice(&dev));
     GP_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    const size_t smem = (size_t)(MT + NSTAGE) * TILE_BYTES + sizeof(Barriers) + ROWB * sizeof(uint32_t) + 1024 + 64;
-    const scoring_fn kernel = g_halves == 2 ? scoring_for<2, false>(k_steps)
-                              : g_pack      ? scoring_for<1, true>(k_steps)
-                                            : scoring_for<1, false>(k_steps);
+    const size_t smem = (size_t)(MT + NSTAGE) * tile_bytes + sizeof(Barriers) + ROWB * sizeof(uint32_t) + 1024 + 64;
+    const scoring_fn kernel = narrow         ? scoring_for<1, true, 64>(k_steps)
+                              : g_halves == 2 ? scoring_for<2, false, 128>(k_steps)
+                              : g_pack        ? scoring_for<1, true, 128>(k_steps)
+                                              : scoring_for<1, false, 128>(k_steps);
     GP_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
 
     // batches of 2^fb genotypes share a weight image; a launch covers up to `group` batches
@@ -856,7 +879,8 @@ gp_status gp_launch_scoring_tc(gp_structures_s* s, const gp_hp_params& hp, uint6
         ia.gfix_first = b0; ia.list_first = 0; ia.gfix_shift = fb; ia.D = s->D; ia.n_tiles = n_tiles;
         ia.NBP = s->NBP; ia.lin = hp.lin; ia.quad = hp.quad;
         gp_time_begin(GP_KERNEL_IMAGE, st);
-        build_image_kernel<<<dim3(n_tiles, n_batches), TN, 0, st>>>(ia, slots);
+        if (narrow) build_image_kernel<64><<<dim3(n_tiles, n_batches), TN, 0, st>>>(ia, slots);
+        else build_image_kernel<128><<<dim3(n_tiles, n_batches), TN, 0, st>>>(ia, slots);
         gp_time_end(GP_KERNEL_IMAGE, st);
         GP_CUDA(cudaGetLastError());
         Args a;
@@ -895,7 +919,9 @@ gp_status gp_launch_map_tc(gp_structures_s* s, const gp_hp_params& hp, uint16_t*
     if (nc > ROWB) return GP_UNSUPPORTED_LATTICE;
     const int k_steps = (nc + 31) / 32;
     const uint32_t n_tiles = (s->D_sym + TN - 1) / TN;
-    const size_t img_bytes = (size_t)n_tiles * TILE_BYTES;
+    const bool narrow = nc <= 64 && g_narrow && g_pack;
+    const size_t tile_bytes = (size_t)TM * (narrow ? 64 : 128);
+    const size_t img_bytes = (size_t)n_tiles * tile_bytes;
     const size_t rec_bytes = sizeof(int4) << fb;
 
     // images of the map: m and rev(m) adjacent, each unordered pair once
@@ -919,8 +945,9 @@ gp_status gp_launch_map_tc(gp_structures_s* s, const gp_hp_params& hp, uint16_t*
     int dev = 0, sms = 0;
     GP_CUDA(cudaGetDevice(&dev));
     GP_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    const size_t smem = (size_t)(MT + NSTAGE) * TILE_BYTES + sizeof(Barriers) + ROWB * sizeof(uint32_t) + 1024 + 64;
-    const scoring_fn kernel = g_pack ? scoring_for<1, true>(k_steps) : scoring_for<1, false>(k_steps);
+    const size_t smem = (size_t)(MT + NSTAGE) * tile_bytes + sizeof(Barriers) + ROWB * sizeof(uint32_t) + 1024 + 64;
+    const scoring_fn kernel = narrow ? scoring_for<1, true, 64>(k_steps)
+                              : g_pack ? scoring_for<1, true, 128>(k_steps) : scoring_for<1, false, 128>(k_steps);
     GP_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const size_t need = (img_bytes + rec_bytes) * group;
     if (s->scratch_bytes < need) {
@@ -945,7 +972,8 @@ gp_status gp_launch_map_tc(gp_structures_s* s, const gp_hp_params& hp, uint16_t*
         ia.gfix_first = 0; ia.list_first = first; ia.gfix_shift = k; ia.D = s->D_sym; ia.n_tiles = n_tiles;
         ia.NBP = s->NBP; ia.lin = hp.lin; ia.quad = hp.quad;
         gp_time_begin(GP_KERNEL_IMAGE, st);
-        build_image_kernel<<<dim3(n_tiles, n_img), TN, 0, st>>>(ia, slots);
+        if (narrow) build_image_kernel<64><<<dim3(n_tiles, n_img), TN, 0, st>>>(ia, slots);
+        else build_image_kernel<128><<<dim3(n_tiles, n_img), TN, 0, st>>>(ia, slots);
         gp_time_end(GP_KERNEL_IMAGE, st);
         GP_CUDA(cudaGetLastError());
         Args a;

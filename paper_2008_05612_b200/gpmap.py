@@ -71,7 +71,7 @@ def lib():
             f.argtypes = args
         L.gp_set_fold_bits.restype = ctypes.c_int
         L.gp_set_fold_bits.argtypes = [ctypes.c_int]
-        for hook in ("gp_set_seq_tc", "gp_set_sym_bits", "gp_set_rob_tile_bits", "gp_set_pack", "gp_set_halves", "gp_set_debug"):  # test / tuning hooks
+        for hook in ("gp_set_narrow", "gp_set_seq_tc", "gp_set_sym_bits", "gp_set_rob_tile_bits", "gp_set_pack", "gp_set_halves", "gp_set_debug"):  # test / tuning hooks
             getattr(L, hook).restype = ctypes.c_int
             getattr(L, hook).argtypes = [ctypes.c_int]
         _lib = L
