@@ -356,7 +356,7 @@ def run_ours(args):
             "folding_fraction_last_tile": folding / float(n),
             "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline, "other_kernels": other,
             "whole_map_3x3x3": whole,
-            "full_6x6_measured": {"wall_s": 117.6, "path": "gp_enumerate_map + designability + neighbour pass, 137 GB store",
+            "full_6x6_measured": {"wall_s": 114.3, "path": "gp_enumerate_map + designability + neighbour pass, 137 GB store",
                                   "source": "profiles/r1_full_6x6.md (separate run: python tests/full_map_check.py --lattice 6x6)"},
             "cpu_baseline": cpu}
     print(json.dumps(line), flush=True)
