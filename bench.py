@@ -289,7 +289,7 @@ def run_ours(args):
     dur = sc_ms / max(1, sc_n) * 1e-3
     achieved = ops_exec * evals_launch / dur / 1e12 if dur > 0 else 0.0
     roofline = {"kernel": "tc::scoring_kernel", "bound": "tensor", "achieved": achieved, "peak": peak_i8, "unit": "TFLOP/s",
-                "frac": achieved / peak_i8, "traffic": 553.98e6 * evals_launch / 1.3903e11,
+                "frac": achieved / peak_i8, "traffic": 965.68e6 * evals_launch / 4.8098e11,
                 "traffic_source": "ncu dram__bytes_read+write of profiles/r1_scoring_final_ncu.md, scaled by evaluations per launch",
                 "peak_source": "2 x bf16_tflops_sustained (%s); int8 ops" % src,
                 "frac_of_nominal_4500": achieved / 4500.0, "frac_of_2x_bf16_burst": achieved / (2.0 * bf16_burst),
