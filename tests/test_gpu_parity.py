@@ -265,7 +265,7 @@ def test_robustness_tile_sizes_agree_with_oracle(tile_bits):
 
 
 @pytest.mark.parametrize("dims,k", [((2, 2, 1), 9), ((3, 3, 1), 9), ((4, 4, 1), 5), ((4, 4, 1), 6), ((4, 4, 1), 8),
-                                    ((4, 3, 1), 5), ((2, 2, 2), 9)])
+                                    ((4, 3, 1), 5), ((4, 3, 1), 7), ((4, 4, 1), 7), ((2, 2, 2), 9)])
 def test_enumerate_map_whole_small_maps(oracle_structures, dims, k):
     """gp_enumerate_map (reversal identity, one representative per class) equals the oracle on whole maps, for image
     sizes that give many image pairs, palindromic images and a single image; chains under 10 monomers fall back."""
