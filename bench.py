@@ -11,6 +11,9 @@ store (2^G x 2 B = 134 MB at G = 26) and its weight images (0.9 GB) are larger t
   python bench.py [--gpus N] [--steps K] [--warmup W] [--log2-genotypes G] [--lattice 6x6|5x5|3x3x3|4x4]
   python bench.py --impl reference ...     # the CPU oracle, as it stands, on a bounded sample of the same workload
   python bench.py --full                   # one step = the whole 2^36 map (137 GB store); long
+  python bench.py --rows                   # every row of SURVEY.md section 8(a) on its own configuration
+The default run also enumerates the WHOLE 6x6 map once (gp_enumerate_map_range in chunks + designability + neighbour
+pass over the resident 137 GB store, about 2 minutes; --no-full-map skips it) and prints its measured wall time.
 
 N > 1 (torchrun): each rank takes its own prefix tiles (genotype ranges are independent); no
 data-path collective; value = evaluations of all ranks / max-over-ranks device time ("weak" scaling).
@@ -27,7 +30,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-METRIC = "genotype x structure energy evals/s (6x6 HP prefix tile; full-enumeration wall time extrapolated)"
+METRIC = "genotype x structure energy evals/s (6x6 HP prefix tile; the full 2^36 enumeration is timed live beside it)"
 UNIT = "evals/s"
 LATTICES = {"4x4": (4, 4, 1), "5x5": (5, 5, 1), "3x3x3": (3, 3, 3), "6x6": (6, 6, 1)}
 SEED = 200805612
@@ -42,10 +45,13 @@ def parse():
     ap.add_argument("--lattice", default="6x6", choices=sorted(LATTICES))
     ap.add_argument("--log2-genotypes", type=int, default=26, help="genotypes per step = 2^G (clamped to the map)")
     ap.add_argument("--full", action="store_true", help="one step = the full map of the lattice")
-    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
+    ap.add_argument("--cpu-seconds", type=float, default=10.0, help="target CPU time of the oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-whole-map", action="store_true", help="skip the whole-3x3x3-map leg")
-    ap.add_argument("--fold-bits", type=int, default=0, help="tuning hook: low genotype bits kept as MMA columns")
+    ap.add_argument("--no-full-map", action="store_true", help="skip the live full 2^36 6x6 enumeration leg (about 2 minutes)")
+    ap.add_argument("--fold-bits", type=int, default=0, help="gp_tuning.fold_bits: low genotype bits kept as MMA columns")
+    ap.add_argument("--rows", action="store_true", help="time every row of the hot path on its BASELINE.json config instead")
+    ap.add_argument("--out", default="", help="--rows: also write the rows to this JSON file")
     return ap.parse_args()
 
 
@@ -121,28 +127,137 @@ def peaks():
         return 6650.0, 1590.0, 1400.0, "fallback"
 
 
-def oracle_sample(dims, begins, count_each, cpu_seconds):
-    """Time the CPU oracle (single thread, as it stands) on genotype ranges of the same workload.
-    Returns (evals/s, seconds, description).  The sample grows until it costs about cpu_seconds."""
+
+
+PROFILE_CSV = os.path.join(ROOT, "profiles", "r2_scoring_ncu_raw.csv")
+
+
+def ncu_profile():
+    """Tensor-pipe activity and DRAM bytes of one scoring_kernel launch from the committed `ncu --page raw --csv` export
+    (profiles/r2_scoring_ncu_raw.csv; the command is in profiles/r2_scoring_ncu.md): taken under the profiler in a
+    separate run of the same configuration, read here by file parse only.  None if the file is absent."""
+    import csv
+    try:
+        with open(PROFILE_CSV, newline="") as f:
+            rows = [r for r in csv.reader(f) if r]
+    except OSError:
+        return None
+    head = next((r for r in rows if "Kernel Name" in r), None)
+    if head is None:
+        return None
+    body = [r for r in rows[rows.index(head) + 1:] if len(r) == len(head)]
+    vals = next((r for r in body if "scoring_kernel" in r[head.index("Kernel Name")]), None)
+    units = body[0] if body and body[0][head.index("Kernel Name")] == "" else None
+    if vals is None:
+        return None
+
+    def get(name, scale_by_unit=True):
+        if name not in head:
+            return None
+        i = head.index(name)
+        v = float(vals[i].replace(",", ""))
+        if scale_by_unit and units:
+            v *= {"Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "byte": 1.0, "ms": 1.0, "us": 1e-3, "ns": 1e-6}.get(units[i], 1.0)
+        return v
+    rd, wr = get("dram__bytes_read.sum"), get("dram__bytes_write.sum")
+    return {"file": os.path.relpath(PROFILE_CSV, ROOT), "kernel": vals[head.index("Kernel Name")],
+            "tensor_active_pct": get("sm__pipe_tensor_subpipe_imma_cycles_active.avg.pct_of_peak_sustained_active", False),
+            "alu_active_pct": get("sm__pipe_alu_cycles_active.avg.pct_of_peak_sustained_active", False),
+            "duration_ms": get("gpu__time_duration.sum"),
+            "dram_bytes": (rd + wr) if rd is not None and wr is not None else None}
+
+
+def _oracle_range(args):
+    dims, begin, count = args
     from oracle import gp_oracle as orc
-    O = orc.Structures(*dims)
+    O = _oracle_range.cache.setdefault(dims, None) or orc.Structures(*dims)
+    _oracle_range.cache[dims] = O
+    t0 = time.perf_counter()
+    O.enumerate(begin, count, want_gap=False)
+    return time.perf_counter() - t0
+
+
+_oracle_range.cache = {}
+
+
+def oracle_rate(dims, begins, seconds, O=None):
+    """evals/s of the oracle as it stands, 1 thread: consecutive genotypes from each of `begins`, about `seconds` in all."""
+    from oracle import gp_oracle as orc
+    O = O or orc.Structures(*dims)
     total = 1 << O.N
     n = min(64, total)
     O.enumerate(begins[0], n, want_gap=False)  # page in
     t0 = time.perf_counter()
     O.enumerate(begins[0], n, want_gap=False)
-    dt = max(time.perf_counter() - t0, 1e-6)
-    per = dt / n
-    want = int(max(n, min(total, cpu_seconds / per)))
-    per_range = max(1, min(count_each, want // max(1, len(begins))))
+    per = max(time.perf_counter() - t0, 1e-7) / n
+    each = int(max(1, min(total, seconds / per) // len(begins)))
     done, t0 = 0, time.perf_counter()
     for b in begins:
-        c = min(per_range, total - b)
+        c = min(each, total - b)
         O.enumerate(b, c, want_gap=False)
         done += c
     dt = time.perf_counter() - t0
-    return done * O.D / dt, dt, "%d ranges x %d consecutive genotypes x %d structures (%.3g evals), 1 thread" % (
-        len(begins), per_range, O.D, done * O.D)
+    return done * O.D / dt, dt, done, O
+
+
+def cpu_baseline(dims, begins, cpu_seconds, G, N):
+    """the oracle, as it stands, on this box's host cores.  `value` = 1 thread on the bench
+    workload (config 4); the other configs, the all-core aggregate (independent processes on disjoint ranges) and the
+    oracle's neighbour pass are listed beside it."""
+    import numpy as np
+    from oracle import gp_oracle as orc
+    v, secs, done, O = oracle_rate(dims, begins, cpu_seconds)
+    out = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "seconds": secs,
+           "sample": "%d ranges x %d consecutive genotypes of the step's tiles x %d structures (%.3g evals), 1 thread"
+                     % (len(begins), done // len(begins), O.D, done * O.D),
+           "host_cores_available": os.cpu_count(), "full_6x6_map_extrapolated_s": float(1 << 36) * 57337 / v if dims == (6, 6, 1) else None}
+    # all cores: one process per core, each its own disjoint range of the same tile (fork: the fold library is shared)
+    try:
+        import multiprocessing as mp
+        cores = os.cpu_count() or 1
+        per = max(64, done)                      # every process does as much as the single-thread sample did in all
+        _oracle_range.cache[dims] = O
+        jobs = [(dims, begins[i % len(begins)] + (1 + i // len(begins)) * per * 4, per) for i in range(cores)]
+        with mp.get_context("fork").Pool(cores) as pool:
+            t0 = time.perf_counter()
+            pool.map(_oracle_range, jobs)
+            wall = time.perf_counter() - t0
+        out["all_cores"] = {"value": cores * per * O.D / wall, "unit": UNIT, "cores": cores, "seconds": wall,
+                            "sample": "%d processes x %d genotypes" % (cores, per)}
+    except Exception as e:  # a box that cannot fork is not a bench failure
+        out["all_cores"] = {"unavailable": repr(e)}
+    others = {}
+    for name, d, b, secs_each in (("config1_4x4_full_map", (4, 4, 1), [0], None), ("config2_5x5", (5, 5, 1), [0, 21 << 20], 3.0),
+                                  ("config3_3x3x3", (3, 3, 3), [0, 0x2B5 << 16, (1 << 27) - (1 << 12)], 3.0)):
+        if secs_each is None:
+            Od = orc.Structures(*d)
+            t0 = time.perf_counter()
+            Od.enumerate(0, 1 << Od.N, want_gap=False)
+            dt = time.perf_counter() - t0
+            others[name] = {"evals_per_s": float(1 << Od.N) * Od.D / dt, "seconds": dt, "genotypes": 1 << Od.N}
+        else:
+            r, dt, dn, Od = oracle_rate(d, b, secs_each)
+            others[name] = {"evals_per_s": r, "seconds": dt, "genotypes": dn}
+    O4 = orc.Structures(4, 4)
+    n5 = 1 << 20
+    seqs = orc.seeded_sequences(SEED, 0, n5, 16)
+    M = orc.seeded_matrix(SEED)
+    t0 = time.perf_counter()
+    O4.enumerate_seqs(seqs, M, 20, want_gap=False)
+    dt = time.perf_counter() - t0
+    others["config5_mj4x4"] = {"evals_per_s": n5 * O4.D / dt, "seconds": dt, "sequences": n5}
+    # neighbour pass of the oracle over a store shaped like config 2 (549 classes, 63 % null; seeded), a quarter of its
+    # size so that the sample stays bounded: 2^23 entries x 23 flips
+    rng = np.random.default_rng(SEED)
+    store = rng.integers(0, 549, size=1 << 23).astype(np.uint16)
+    store[rng.random(1 << 23) < 0.63] = 0xFFFF
+    t0 = time.perf_counter()
+    orc.robustness(store, 23, 549)
+    dt = time.perf_counter() - t0
+    others["neighbour_pass_config2_shape"] = {"seconds": dt, "genotypes": 1 << 23, "genotype_flips_per_s": float(23 << 23) / dt,
+                                              "store": "seeded synthetic, 549 classes, 63 % null"}
+    out["other_configs"] = others
+    return out
 
 
 def run_reference(args):
@@ -175,12 +290,174 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * tot / len(times), "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "int32", "data": "synthetic",
-            "config": {"workload": "%s HP prefix tile, 2^%d genotypes x %d directed structures (oracle sample)" % (
-                args.lattice, G, O.D), "lattice": args.lattice, "log2_genotypes": G},
+            "config": workload_config(args.lattice, G, O.D, O.C, O.N + sum(1 for i in range(O.N) for j in range(i + 3, O.N, 2)), 1 << G),
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
+
+
+def workload_config(lattice, G, D, C, K, n):
+    """The `config` object: identical keys in both arms."""
+    return {"workload": "%s HP genotype-prefix tile: 2^%d genotypes x %d directed structures, then designability + "
+                        "neighbour pass over the tile" % (lattice, G, D),
+            "lattice": lattice, "log2_genotypes": G, "D": D, "C": C, "features_K": K,
+            "l2": "inputs larger than L2 (per step: %.0f MB phenotype tile, fresh seeded prefix, weight images rebuilt)"
+                  % (2.0 * n / 1e6),
+            "parallelism": "independent prefix tiles per rank, no collective"}
+
+
+def full_map_leg(lattice, stream, cpu_check=True):
+    """BASELINE.json configs[3] live: the WHOLE map of the lattice through gp_enumerate_map_range (chunks of units, so the
+    run can report progress and could resume), gp_designability and gp_robustness over the resident store; device
+    times from CUDA events on the launching stream; invariants; a seeded sample of phenotypes against the oracle."""
+    import numpy as np
+    import torch
+    from paper_2008_05612_b200 import gpmap
+    S = gpmap.Structures(*LATTICES[lattice])
+    N, D, C = S.N, S.D, S.C
+    total = 1 << N
+    free, _ = torch.cuda.mem_get_info()
+    need = 2 * total + (3 << 30)
+    if free < need:
+        return {"skipped": "needs %.1f GB of free HBM, %.1f GB free" % (need / 1e9, free / 1e9)}
+    pheno = torch.empty(total, dtype=torch.uint16, device="cuda")
+    U = S.map_units()
+    chunks = 64 if U >= 64 else 1
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+    l0 = gpmap.launch_count()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    ev[0].record(stream)
+    for c in range(chunks):
+        u0, u1 = U * c // chunks, U * (c + 1) // chunks
+        S.enumerate_map_range(u0, u1 - u0, pheno, stream=stream)
+    ev[1].record(stream)
+    hist = gpmap.designability(pheno, C, stream=stream)
+    ev[2].record(stream)
+    R, Dl, Oc, pairs = gpmap.robustness(pheno, N, C, stream=stream)
+    ev[3].record(stream)
+    torch.cuda.synchronize()
+    wall = time.perf_counter() - t0
+    t_score, t_hist, t_rob = (ev[i].elapsed_time(ev[i + 1]) * 1e-3 for i in range(3))
+    launches = gpmap.launch_count() - l0
+    hist = hist.cpu().numpy().astype(np.uint64)
+    R, Dl, Oc = (x.cpu().numpy().astype(np.uint64) for x in (R, Dl, Oc))
+    folding = int(hist[:C].sum())
+    rng = np.random.default_rng(SEED)
+    g = rng.integers(0, total, size=1 << 20, dtype=np.uint64)
+    rev = np.zeros_like(g)
+    for i in range(N):
+        rev |= ((g >> np.uint64(i)) & np.uint64(1)) << np.uint64(N - 1 - i)
+    s16 = pheno.view(torch.int16)
+    rev_bad = int((s16[torch.from_numpy(g.astype(np.int64)).cuda()] != s16[torch.from_numpy(rev.astype(np.int64)).cuda()]).sum())
+    out = {"workload": "%s HP whole map: 2^%d genotypes x %d directed structures (%d representatives scored, reversal "
+                       "identity), uint16 store resident in HBM (%.1f GB), designability + neighbour pass + pair count"
+                       % (lattice, N, D, C, 2.0 * total / 1e9),
+           "wall_s": wall, "device_s": {"scoring": t_score, "designability": t_hist, "neighbour_pass": t_rob,
+                                        "total": t_score + t_hist + t_rob},
+           "effective_evals_per_s": float(total) * D / t_score, "executed_evals_per_s": float(total) * C / t_score,
+           "store_GBps": {"designability": 2.0 * total / t_hist / 1e9, "neighbour_pass_algorithmic": 2.0 * total / t_rob / 1e9},
+           "gpu_launches": int(launches), "unit_chunks": chunks,
+           "folding": folding, "folding_fraction": folding / total, "designable_classes": int((hist[:C] > 0).sum()),
+           "phenotype_pairs": int(pairs.item()), "sum_R": int(R.sum()), "sum_D": int(Dl.sum()), "sum_O": int(Oc.sum()),
+           "invariants": {"hist_sums_to_2^N": int(hist.sum()) == total,
+                          "R+D+O_equals_N_x_folding": int(R.sum() + Dl.sum() + Oc.sum()) == N * folding,
+                          "sum_R_even": int(R.sum()) % 2 == 0, "sum_O_even": int(Oc.sum()) % 2 == 0,
+                          "reversal_symmetry_mismatches_of_2^20": rev_bad}}
+    if cpu_check:
+        from oracle import gp_oracle as orc
+        O = orc.Structures(*LATTICES[lattice])
+        bad = n_chk = 0
+        for b in [0, total - 256] + [int(x) for x in rng.integers(0, total - 256, size=6)]:
+            want = O.enumerate(b, 256, want_gap=False)
+            bad += int((pheno[b:b + 256].cpu().numpy() != want).sum())
+            n_chk += 256
+        out["oracle_sampled"] = {"genotypes": n_chk, "mismatches": bad}
+    del pheno
+    S.close()
+    torch.cuda.empty_cache()
+    return out
+
+
+def run_rows(args):
+    """--rows: every row of SURVEY.md section 8(a) on the configuration BASELINE.json names for it (CUDA-event times
+    after one warm-up call; a0 is host wall time).  Prints one JSON object per row."""
+    import numpy as np
+    import torch
+    from paper_2008_05612_b200 import gpmap
+
+    def dev_time(fn, reps=2):
+        fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(reps):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) * 1e-3 / reps
+
+    rows, structs = [], {}
+    for name in ("4x4", "5x5", "3x3x3", "6x6"):
+        t0 = time.perf_counter()
+        structs[name] = gpmap.Structures(*LATTICES[name])
+        rows.append(dict(row="a0 gp_structures", config=name, seconds=time.perf_counter() - t0,
+                         note="D=%d C=%d" % (structs[name].D, structs[name].C)))
+    for name in ("4x4", "5x5", "3x3x3"):
+        S = structs[name]
+        n = 1 << S.N
+        ph = torch.empty(n, dtype=torch.uint16, device="cuda")
+        gap = torch.empty(n, dtype=torch.int16, device="cuda")
+        t = dev_time(lambda: S.enumerate(0, n, ph))
+        rows.append(dict(row="a1-a4 gp_enumerate (prefix path, D columns)", config=name, seconds=t, evals_per_s=n * S.D / t))
+        t = dev_time(lambda: S.enumerate_map(ph, gap))
+        rows.append(dict(row="a1-a4 gp_enumerate_map (reversal identity, C columns)", config=name, seconds=t,
+                         effective_evals_per_s=n * S.D / t))
+        m = min(n, 1 << 22)
+        t = dev_time(lambda: S.enumerate(0, m, ph, simple=True), reps=1)
+        rows.append(dict(row="a1-a4 gp_enumerate_simple (CUDA cores)", config=name + " first 2^22", seconds=t, evals_per_s=m * S.D / t))
+        S.enumerate_map(ph, gap)
+        t = dev_time(lambda: gpmap.designability(ph, S.C))
+        rows.append(dict(row="a5 gp_designability", config=name, seconds=t, GBps=2.0 * n / t / 1e9))
+        t = dev_time(lambda: gpmap.robustness(ph, S.N, S.C))
+        rows.append(dict(row="a6 gp_robustness (+ pair bitmap)", config=name, seconds=t, GBps_algorithmic=2.0 * n / t / 1e9))
+        t = dev_time(lambda: gpmap.nn_components(ph, S.N, S.C), reps=1)
+        rows.append(dict(row="a7 gp_nn_components", config=name, seconds=t))
+        t = dev_time(lambda: gpmap.threshold_sweep(ph, gap, S.C, [1, 2, 3, 10, 24]))
+        rows.append(dict(row="f4 gp_threshold_sweep (5 thresholds)", config=name, seconds=t, GBps=4.0 * n / t / 1e9))
+        del ph, gap
+    for name, paper_hp, paper_mj in (("6x6", 1.35e-4, 1.19e-4), ("3x3x3", 2.6e-4, 2.8e-4)):  # PAPER.md:195-204 Table 3
+        S = structs[name]
+        cnt = 1 << 21
+        seqs = torch.from_numpy(np.random.default_rng(SEED).integers(0, 2, size=(cnt, S.N), dtype=np.uint8)).cuda()
+        ph = torch.empty(cnt, dtype=torch.uint16, device="cuda")
+        e = np.array(gpmap.HP_ENERGIES, np.int32)
+        for label, on, c in (("tensor cores", 1, cnt), ("CUDA cores", 0, 1 << 17)):
+            S.tune(seq_tensor=on)
+            t = dev_time(lambda: S.enumerate_seqs(seqs[:c], ph[:c], None, e=e, alphabet=2), reps=1)
+            rows.append(dict(row="f3 sampling, random HP sequences (%s)" % label, config="%s, %d sequences" % (name, c), seconds=t,
+                             evals_per_s=c * S.D / t, seconds_per_sequence=t / c, paper_gpu_seconds_per_sequence=paper_hp))
+        S.tune(seq_tensor=1)
+        c = 1 << 17
+        M = gpmap.seeded_matrix(SEED)
+        t = dev_time(lambda: S.enumerate_seeded(SEED, 0, c, ph[:c], e=M), reps=1)
+        rows.append(dict(row="f3 sampling, seeded 20-letter sequences", config="%s, %d sequences" % (name, c), seconds=t,
+                         evals_per_s=c * S.D / t, seconds_per_sequence=t / c, paper_gpu_seconds_per_sequence=paper_mj))
+        del seqs, ph
+    S = structs["4x4"]
+    M = gpmap.seeded_matrix(SEED)
+    n = 1 << 30
+    ph = torch.empty(n, dtype=torch.uint16, device="cuda")
+    t = dev_time(lambda: S.enumerate_seeded(SEED, 0, n, ph, e=M), reps=1)
+    hist = gpmap.designability(ph, S.C)
+    rows.append(dict(row="a8 gp_enumerate_seeded (20 letters, seeded matrix)", config="4x4, 2^30 sequences", seconds=t,
+                     evals_per_s=n * S.D / t, folding_fraction=1.0 - hist[S.C].item() / n))
+    for r in rows:
+        print(json.dumps(r), flush=True)
+    if args.out:
+        with open(args.out, "w") as f:
+            json.dump(rows, f, indent=1)
 
 
 def run_ours(args):
@@ -198,11 +475,15 @@ def run_ours(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     gpmap.lib()  # fails loudly if libgpmap.so is missing / unbuildable
-    if args.fold_bits:
-        gpmap.set_fold_bits(args.fold_bits)
+    if args.rows:
+        if rank == 0:
+            run_rows(args)
+        return
 
     dims = LATTICES[args.lattice]
     S = gpmap.Structures(*dims)
+    if args.fold_bits:
+        S.tune(fold_bits=args.fold_bits)
     N, D, C = S.N, S.D, S.C
     G = N if args.full else min(args.log2_genotypes, N)
     n = 1 << G
@@ -238,7 +519,7 @@ def run_ours(args):
     barrier()
     ev0.record(stream)
     for i in range(args.steps):
-        out = step(args.warmup + i)
+        step(args.warmup + i)
     ev1.record(stream)
     barrier()
     ms = ev0.elapsed_time(ev1)
@@ -264,7 +545,7 @@ def run_ours(args):
         barrier()
         t0 = time.perf_counter()
         for i in range(e_steps):
-            r = S.enumerate_host(tile_begin(args.warmup + i, rank, world, G, N), n, want_robustness=True, pheno_out=host_np)
+            S.enumerate_host(tile_begin(args.warmup + i, rank, world, G, N), n, want_robustness=True, pheno_out=host_np)
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0
         if world > 1:
@@ -274,6 +555,7 @@ def run_ours(args):
         e2e = {"value": evals_step * e_steps / dt, "unit": UNIT, "h2d_bytes_per_step": 16,
                "d2h_bytes_per_step": int(2 * n + 8 * (C + 1) + 24 * C + 8), "steps": e_steps,
                "call": "gp_enumerate_host (host buffers, pinned phenotype output; device store kept in the handle)"}
+        del host, host_np
 
     if rank != 0:
         if world > 1:
@@ -282,18 +564,35 @@ def run_ours(args):
     hbm, bf16_burst, bf16_sus, src = peaks()
     sc_ms, sc_n = ktime[gpmap.KERNEL_SCORING]
     evals_launch = float(n) * D / max(1, sc_n // max(1, args.steps))  # one rank's launches
-    fb = min(N, args.fold_bits or 15)                                 # low genotype bits kept as contraction columns
-    k_exec = 2 + fb + sum(1 for i in range(fb) for j in range(i + 3, fb, 2))  # bias x2 + monomers + pairs
-    ops_exec = 2.0 * k_exec                                           # int8 multiply-adds x2 the kernel executes per evaluation
-    peak_i8 = 2.0 * bf16_sus                                          # int8 dense = 2 x bf16 (guide's nominal ratio)
+    if args.full:                                                     # map path: k free monomers at each chain end, C columns
+        k = min(S.tuning()["sym_bits"], N // 2)
+        mon = list(range(k)) + list(range(N - k, N))
+        evals_launch = float(n) * C / max(1, sc_n // max(1, args.steps))
+    else:
+        mon = list(range(min(N, S.tuning()["fold_bits"])))            # low genotype bits kept as contraction columns
+    k_exec = 2 + len(mon) + sum(1 for i in range(len(mon)) for j in range(i + 1, len(mon))
+                                if mon[j] - mon[i] >= 3 and (mon[j] - mon[i]) % 2 == 1)  # bias x2 + monomers + pairs
+    k_steps = (k_exec + 31) // 32
+    ops_exec = 2.0 * k_exec                                           # int8 multiply-adds x2 of the folded contraction per evaluation
+    ops_issued = 2.0 * 32 * k_steps                                   # what the MMAs issue (columns padded to 32-byte K steps)
     dur = sc_ms / max(1, sc_n) * 1e-3
     achieved = ops_exec * evals_launch / dur / 1e12 if dur > 0 else 0.0
+    # the peak: this kernel's own MMA stream alone (gp_probe_i8_peak), measured now on this device
+    probe_ops, probe_clk, probe_mhz = gpmap.probe_i8_peak(k_steps, 1.0)
+    peak_i8 = probe_ops / 1e12
+    prof = ncu_profile()
     roofline = {"kernel": "tc::scoring_kernel", "bound": "tensor", "achieved": achieved, "peak": peak_i8, "unit": "TFLOP/s",
-                "frac": achieved / peak_i8, "traffic": 965.68e6 * evals_launch / 4.8098e11,
-                "traffic_source": "ncu dram__bytes_read+write of profiles/r1_scoring_final_ncu.md, scaled by evaluations per launch",
-                "peak_source": "2 x bf16_tflops_sustained (%s); int8 ops" % src,
+                "frac": achieved / peak_i8,
+                "traffic": prof["dram_bytes"] if prof else None,
+                "traffic_source": (prof["file"] + " (one launch of the same configuration under ncu --set full)") if prof else None,
+                "peak_source": "gp_probe_i8_peak(k_steps=%d): MMA-only tcgen05.mma kind::i8 stream, measured in this run" % k_steps,
+                "peak_i8_measured": {"TOPs": peak_i8, "clk_per_mma": probe_clk, "sm_mhz": probe_mhz},
+                "frac_issued": achieved * ops_issued / ops_exec / peak_i8,
+                "ncu_tensor_active": prof["tensor_active_pct"] / 100.0 if prof and prof["tensor_active_pct"] is not None else None,
                 "frac_of_nominal_4500": achieved / 4500.0, "frac_of_2x_bf16_burst": achieved / (2.0 * bf16_burst),
-                "ops_per_eval_executed": ops_exec, "ops_per_eval_contraction_as_posed": 2.0 * S.K,
+                "frac_of_2x_bf16_sustained": achieved / (2.0 * bf16_sus), "bf16_peaks_source": src,
+                "ops_per_eval_executed": ops_exec, "ops_per_eval_issued": ops_issued,
+                "ops_per_eval_contraction_as_posed": 2.0 * S.K,
                 "avg_launch_ms": dur * 1e3, "launches": int(sc_n),
                 "evals_per_s_kernel": evals_launch / dur if dur > 0 else 0.0,
                 "share_of_step": sc_ms / ms if ms > 0 else None}
@@ -307,17 +606,9 @@ def run_ours(args):
                         "peak": hbm, "avg_launch_ms": hs_ms / max(1, hs_n), "share_of_step": hs_ms / ms},
         "build_image_kernel": {"avg_launch_ms": im_ms / max(1, im_n), "launches": int(im_n), "share_of_step": im_ms / ms},
     }
-    if other["robustness_kernel"]["algorithmic_GBps"]:
-        other["robustness_kernel"]["frac"] = other["robustness_kernel"]["algorithmic_GBps"] / hbm
-    if other["hist_kernel"]["algorithmic_GBps"]:
-        other["hist_kernel"]["frac"] = other["hist_kernel"]["algorithmic_GBps"] / hbm
-
-    cpu = None
-    if not args.no_cpu_baseline and world == 1:
-        begins = [tile_begin(args.warmup + i, 0, 1, G, N) for i in range(min(4, args.steps))]
-        v, secs, desc = oracle_sample(dims, begins, 1 << 20, args.cpu_seconds)
-        cpu = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc, "seconds": secs,
-               "host_cores_available": os.cpu_count()}
+    for kname in ("robustness_kernel", "hist_kernel"):
+        if other[kname]["algorithmic_GBps"]:
+            other[kname]["frac"] = other[kname]["algorithmic_GBps"] / hbm
 
     whole = None
     if world == 1 and not args.full and not args.no_whole_map:
@@ -332,7 +623,7 @@ def run_ours(args):
                 e0.record(stream)
             S3.enumerate_map(p3, stream=stream)
             h3 = gpmap.designability(p3, S3.C, stream=stream)
-            r3 = gpmap.robustness(p3, 27, S3.C, stream=stream)
+            gpmap.robustness(p3, 27, S3.C, stream=stream)
         e1.record(stream)
         torch.cuda.synchronize()
         sec = e0.elapsed_time(e1) * 1e-3 / reps
@@ -342,23 +633,28 @@ def run_ours(args):
                  "folding": int((1 << 27) - h3[S3.C].item()), "paper_folding_percent": 4.76}
         del p3
         S3.close()
+
+    cpu = None
+    if not args.no_cpu_baseline and world == 1:
+        begins = [tile_begin(args.warmup + i, 0, 1, G, N) for i in range(min(4, args.steps))]
+        cpu = cpu_baseline(dims, begins, args.cpu_seconds, G, N)
+
+    full = None
+    if world == 1 and not args.full and not args.no_full_map and args.lattice == "6x6":
+        del pheno
+        S.close()
+        torch.cuda.empty_cache()
+        full = full_map_leg("6x6", stream, cpu_check=not args.no_cpu_baseline)
+
     total_evals_map = float(1 << N) * D
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "s8 x s8 -> s32", "data": "synthetic",
-            "config": {"workload": "%s HP genotype-prefix tile: 2^%d genotypes x %d directed structures, then designability + "
-                                   "neighbour pass over the tile" % (args.lattice, G, D),
-                       "lattice": args.lattice, "log2_genotypes": G, "D": D, "C": C, "features_K": S.K,
-                       "l2": "inputs larger than L2 (per step: %.0f MB phenotype tile, fresh seeded prefix, weight images rebuilt)"
-                             % (2.0 * n / 1e6),
-                       "parallelism": "independent prefix tiles per rank, no collective"},
-            "full_map_wall_s_extrapolated": total_evals_map / value * world if value else None,
+            "config": workload_config(args.lattice, G, D, C, S.K, n),
+            "full_map_wall_s_extrapolated_from_tiles": total_evals_map / value * world if value else None,
             "folding_fraction_last_tile": folding / float(n),
             "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline, "other_kernels": other,
-            "whole_map_3x3x3": whole,
-            "full_6x6_measured": {"wall_s": 114.3, "path": "gp_enumerate_map + designability + neighbour pass, 137 GB store",
-                                  "source": "profiles/r1_full_6x6.md (separate run: python tests/full_map_check.py --lattice 6x6)"},
-            "cpu_baseline": cpu}
+            "whole_map_3x3x3": whole, "full_6x6": full, "cpu_baseline": cpu}
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()

@@ -13,8 +13,13 @@
  *   - Pointers named d_* are DEVICE pointers, allocated and freed by the caller.  Pointers without the prefix are HOST
  *     pointers.  The library owns only the opaque gp_structures_t handle (its device tables included) and a private
  *     scratch it frees in gp_structures_free.
- *   - `stream` is a cudaStream_t passed as void* (NULL = default stream).  Compute calls are asynchronous on it; a
- *     non-zero status reports argument or launch errors only.  Device output arrays are fully overwritten.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = default stream).  Compute calls are asynchronous on it and
+ *     never synchronise the device or the stream unless their comment says so (gp_nn_components, gp_enumerate_host);
+ *     a non-zero status reports argument or launch errors only.  Device output arrays are fully overwritten unless a
+ *     call says it accumulates.  Working memory of a call comes from the device's stream-ordered pool
+ *     (cudaMallocAsync on `stream`) and goes back to it on the same stream, so calls on one handle may run
+ *     concurrently on different streams and threads; only gp_tuning_set and gp_structures_free must not overlap a
+ *     call on the same handle.
  *   - Genotype g: bit i of g is the letter of monomer i, 1 = H (R3).  Null phenotype = GP_NULL_PHENO (R7).
  *   - Phenotype ids are reversal-reduced class ids 0..C-1 in the canonical order of DESIGN.md section 3 (R1, R8).
  */
@@ -67,6 +72,20 @@ int gp_structures_features(const gp_structures_t* s);          /* K = N + P: col
  * arrays, each nullable.  GP_RANGE if d >= D. */
 gp_status gp_structures_get(const gp_structures_t* s, uint32_t d, uint8_t* sites, uint8_t* contacts, uint16_t* class_id);
 
+/* Tuning of one handle.  Every setting gives the same results (the parity tests sweep them); they trade tensor work
+ * against weight-image traffic and let tests force code paths that small inputs do not reach.
+ * gp_structures starts a handle at the defaults below. */
+typedef struct {
+    int32_t fold_bits;   /* gp_enumerate: low genotype bits kept as contraction columns, 9..22 (default 15)          */
+    int32_t sym_bits;    /* gp_enumerate_map*: k, monomers free at each chain end inside one image, 5..11 (default 7) */
+    int32_t narrow_rows; /* 1 (default): 64-byte operand rows when the folded contraction has at most 64 columns     */
+    int32_t seq_tensor;  /* 1 (default): gp_enumerate_seqs runs on the tensor cores where it can; 0: CUDA cores      */
+} gp_tuning;
+gp_status gp_tuning_get(const gp_structures_t* s, gp_tuning* out);
+/* GP_INVALID_ARG if a field is out of range (nothing is changed then).  Rebuilds the handle's unit table of
+ * gp_enumerate_map_range when sym_bits changes (synchronous host work + one blocking upload). */
+gp_status gp_tuning_set(gp_structures_t* s, const gp_tuning* t);
+
 /* Genotype-range granularity of gp_enumerate (g_begin must be a multiple of it). */
 uint64_t gp_tile(void);
 
@@ -85,6 +104,31 @@ gp_status gp_enumerate(const gp_structures_t* s, const gp_energies* en, uint64_t
  * genotype's list before the uniqueness test.  executed evaluations = 2^N * C, effective = 2^N * D. */
 gp_status gp_enumerate_map(const gp_structures_t* s, const gp_energies* en, uint16_t* d_pheno, int16_t* d_gap,
                            void* stream);
+
+/* The same map in resumable / shardable pieces (the paper's own 110-day job survived by appending results run by run,
+ * PAPER.md:206-208, :754, :806).  The map is cut into gp_map_units(s) UNITS.  A unit is the pair of "images" {m, rev m}
+ * (one image when m is a palindrome): image m = the 2^(2k) genotypes whose middle N-2k bits equal m, i.e.
+ *   g = (hi << (N-k)) | (m << k) | lo,   0 <= hi, lo < 2^k,   k = gp_tuning.sym_bits (clamped to N/2),
+ * and rev m = m with its N-2k bits reversed, so that a unit is closed under chain reversal.  Units 0 .. are ordered:
+ * first the non-palindromic m < rev m in increasing m, then the palindromic m in increasing m; gp_map_unit reports m
+ * and k of a unit so a caller can tell which genotypes a range of units covers.
+ * gp_enumerate_map_range scores units unit_first .. unit_first+unit_count-1 and writes the phenotype (and the gap if
+ * d_gap is not NULL) of exactly the genotypes of those units, in one of two layouts:
+ *   GP_MAP_FULL_STORE: d_pheno / d_gap are the FULL stores of 2^N entries indexed by g; all other entries are left
+ *     untouched.  Any partition of 0..gp_map_units-1 into ranges, in any order, on any streams, fills the same store
+ *     as gp_enumerate_map.
+ *   GP_MAP_COMPACT: d_pheno / d_gap hold gp_map_range_genotypes(s, unit_first, unit_count) entries: the images of the
+ *     range one after the other (per unit: image m, then image rev m if the unit is a pair), each as its 2^(2k)
+ *     genotypes in the order of the local index (hi << k) | lo.  This is the piece a resumable run appends to its
+ *     output, or a rank that holds no full store keeps.
+ * Lattices too small for the scheme (N < 10) have one unit that covers the map (k reported as 0; both layouts are
+ * then the plain store).  Errors: GP_RANGE if the unit range leaves [0, gp_map_units). */
+enum { GP_MAP_FULL_STORE = 0, GP_MAP_COMPACT = 1 };
+uint64_t gp_map_units(const gp_structures_t* s);
+gp_status gp_map_unit(const gp_structures_t* s, uint64_t unit, uint64_t* m, int* k);
+uint64_t gp_map_range_genotypes(const gp_structures_t* s, uint64_t unit_first, uint64_t unit_count);
+gp_status gp_enumerate_map_range(const gp_structures_t* s, const gp_energies* en, uint64_t unit_first,
+                                 uint64_t unit_count, uint16_t* d_pheno, int16_t* d_gap, int layout, void* stream);
 
 /* Same contract as gp_enumerate, computed by the plain CUDA-core kernel that walks the contact table like the paper's
  * listing (:530-570).  Kept as the in-library cross-check and timing strawman; no alignment requirement. */
@@ -114,11 +158,43 @@ gp_status gp_designability(const uint16_t* d_pheno, uint64_t count, uint32_t n_c
 gp_status gp_robustness(const uint16_t* d_pheno, int n_bits, uint32_t n_classes, uint64_t* d_neutral,
                         uint64_t* d_deleterious, uint64_t* d_other, uint64_t* d_pair_count, void* stream);
 
+/* a6 in pieces, for stores sharded over several GPUs on the top genotype bits and for resumable runs.
+ * All three ADD into d_neutral / d_deleterious / d_other (uint64[n_classes], zeroed by the caller) and OR into
+ * d_pair_bitmap (nullable; gp_pair_bitmap_words(n_classes) uint32 words, zeroed by the caller; bit p*n_classes+q,
+ * p < q, is set when classes p and q are joined by a mutation):
+ *   gp_robustness_partial: the flips of the n_bits LOCAL bits of a sub-cube store of 2^n_bits entries (a shard, or
+ *     the whole map).  tile_bits = 0 takes the default on-chip tile; 4..15 forces a tile of 2^tile_bits entries (any
+ *     value gives the same counts; small tiles exercise the multi-pass path on small stores).
+ *   gp_robustness_cross: the flip of ONE bit outside the sub-cube: entry i of d_mine and entry i of d_partner (the
+ *     shard whose index differs in that bit; may be peer memory) are neighbours; counts go to the classes found in
+ *     d_mine only (the partner's owner makes the mirror call).
+ * Per-class counts of shards add; bitmaps OR (gp_pair_bitmap_or: d_dst |= d_src); gp_pair_bitmap_count writes the
+ * number of set bits (R11) to d_count[0].  gp_robustness = zero + gp_robustness_partial + gp_pair_bitmap_count. */
+uint64_t gp_pair_bitmap_words(uint32_t n_classes);
+gp_status gp_robustness_partial(const uint16_t* d_pheno, int n_bits, uint32_t n_classes, uint64_t* d_neutral,
+                                uint64_t* d_deleterious, uint64_t* d_other, uint32_t* d_pair_bitmap, int tile_bits,
+                                void* stream);
+gp_status gp_robustness_cross(const uint16_t* d_mine, const uint16_t* d_partner, uint64_t count, uint32_t n_classes,
+                              uint64_t* d_neutral, uint64_t* d_deleterious, uint64_t* d_other, uint32_t* d_pair_bitmap,
+                              void* stream);
+gp_status gp_pair_bitmap_or(uint32_t* d_dst, const uint32_t* d_src, uint32_t n_classes, void* stream);
+gp_status gp_pair_bitmap_count(const uint32_t* d_bitmap, uint32_t n_classes, uint64_t* d_count, void* stream);
+
 /* phi row of target class q (:138-147 Eq. 2 numerators, Figs. 9-12): d_row[p] = number of
  * (genotype, flip) pairs that lead from a genotype of class p to a genotype of class q, p < n_classes (p = q: the
  * neutral count of q); d_row[n_classes] = the same from null genotypes.  phi_pq = d_row[p] / (n_bits * hist[p]).  Full
  * store of 2^n_bits entries. */
 gp_status gp_phi_row(const uint16_t* d_pheno, int n_bits, uint32_t n_classes, uint32_t q, uint64_t* d_row, void* stream);
+
+/* f4. Energy-threshold sweep (PAPER.md:81 "within this threshold ... does not fold", :278, :466; R5) from the stores of
+ * ONE threshold-1 enumeration: d_pheno / d_gap as written by gp_enumerate* with threshold = 1 over `count` genotypes.
+ * For each thresholds[t] >= 1 (HOST array, n_thresholds <= 16, any order): a genotype folds iff it has a unique ground
+ * state and second_min - min = -gap >= thresholds[t].  d_folding[t] = number of folding genotypes, d_hist[t][c]
+ * (row length n_classes+1) = designability of class c, last entry = non-folding; the same values gp_enumerate with that
+ * threshold followed by gp_designability gives, from one read of the two stores. */
+gp_status gp_threshold_sweep(const uint16_t* d_pheno, const int16_t* d_gap, uint64_t count, uint32_t n_classes,
+                             const int32_t* thresholds, int n_thresholds, uint64_t* d_folding, uint64_t* d_hist,
+                             void* stream);
 
 /* a7. Neutral-network components (:19, R12): d_ncomp[p] = number of connected components of {g : pheno = p} under
  * single-bit flips.  Needs 4 bytes of private scratch per genotype; n_bits <= 30.  Synchronises the stream. */
@@ -142,6 +218,15 @@ uint64_t gp_launch_count(void);
 enum { GP_KERNEL_SCORING = 0, GP_KERNEL_IMAGE = 1, GP_KERNEL_HIST = 2, GP_KERNEL_ROBUSTNESS = 3, GP_KERNEL_COUNT = 4 };
 void gp_kernel_timing(int enable);
 gp_status gp_kernel_time(int which, double* ms_total, uint64_t* launches);
+
+/* The int8 tensor-core peak the scoring kernel is held against ("the build must
+ * measure an MMA-only kind::i8 peak itself"), measured on the current device: one CTA per SM issues the scoring
+ * kernel's own MMA stream (chains of k_steps tcgen05.mma kind::i8 M128 x N128 x K32 into four TMEM accumulators,
+ * operands in shared memory, 64-byte rows for k_steps <= 2 else 128-byte rows) for about `seconds` with no TMA traffic,
+ * no TMEM read-out and no epilogue.  *ops_per_s = int8 multiply-adds x 2 per second over all SMs; *clk_per_mma (nullable) =
+ * SM clocks per MMA (64 nominal); *sm_mhz (nullable) = the SM clock it ran at (clock64 / event time).  Synchronous, on
+ * the default stream. */
+gp_status gp_probe_i8_peak(int k_steps, double seconds, double* ops_per_s, double* clk_per_mma, double* sm_mhz);
 
 const char* gp_strerror(gp_status st);
 const char* gp_last_cuda_error(void);

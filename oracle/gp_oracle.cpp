@@ -281,11 +281,12 @@ void oracle_enumerate_seqs(void* h, int alphabet, const int32_t* e, int32_t thre
 
 uint64_t oracle_draw(uint64_t seed, uint64_t ctr) { return draw(seed, ctr); }
 
-// counter-based generator of DESIGN.md "Input recipe": letter k of sequence s
+// counter-based generator of DESIGN.md "Input recipe": letter k of sequence s is drawn at counter 64 s + k (a stride of
+// 64 >= the longest chain, so that the sequences of chains longer than 16 share no draws: DESIGN.md section 4)
 void oracle_seeded_sequences(uint64_t seed, uint64_t first, uint64_t count, int N, uint8_t* seqs) {
     for (uint64_t n = 0; n < count; n++)
         for (int k = 0; k < N; k++) {
-            uint64_t u = draw(seed, (first + n) * 16 + (uint64_t)k);
+            uint64_t u = draw(seed, (first + n) * 64 + (uint64_t)k);
             seqs[n * N + k] = (uint8_t)(((u >> 32) * 20) >> 32);
         }
 }

@@ -140,7 +140,7 @@ gp_status gp_upload_tables(gp_structures_s* s) {
         GP_CUDA(cudaMalloc(&s->d_class_sym, ksym.size() * sizeof(uint16_t)));
         GP_CUDA(cudaMemcpy(s->d_class_sym, ksym.data(), ksym.size() * sizeof(uint16_t), cudaMemcpyHostToDevice));
     }
-    return GP_OK;
+    return gp_build_map_units(s);
 }
 
 void gp_release_device(gp_structures_s* s) {
@@ -152,11 +152,16 @@ void gp_release_device(gp_structures_s* s) {
     cudaFree(s->d_contacts_sym);
     cudaFree(s->d_class_sym);
     s->d_contacts_sym = nullptr; s->d_class_sym = nullptr;
-    cudaFree(s->wimg.d_img);
-    cudaFree(s->d_scratch);
+    for (gp_weight_image& w : s->wimgs) {
+        cudaFree(w.d_img);
+        if (w.ready) cudaEventDestroy((cudaEvent_t)w.ready);
+    }
+    s->wimgs.clear();
+    cudaFree(s->d_units);
+    s->d_units = nullptr;
     cudaFree(s->d_host_store);
     s->d_host_store = nullptr; s->host_store_bytes = 0;
-    s->d_contacts = nullptr; s->d_class_of = nullptr; s->d_pairidx = nullptr; s->d_pair_ij = nullptr; s->wimg.d_img = nullptr; s->d_scratch = nullptr;
+    s->d_contacts = nullptr; s->d_class_of = nullptr; s->d_pairidx = nullptr; s->d_pair_ij = nullptr;
 }
 
 extern "C" gp_status gp_structures(int nx, int ny, int nz, gp_structures_t** out) {
@@ -171,6 +176,7 @@ extern "C" gp_status gp_structures(int nx, int ny, int nz, gp_structures_t** out
         st = GP_OUT_OF_MEMORY;
     }
     if (st == GP_OK) st = gp_upload_tables(s);
+    if (st == GP_OK && s->device < 0) st = gp_build_map_units(s);  // host-only handle: the unit queries still work
     if (st != GP_OK) {
         gp_release_device(s);
         delete s;
@@ -213,7 +219,10 @@ gp_status gp_check_hp(const gp_structures_s* s, const gp_energies* en, gp_hp_par
     int32_t lin = b - a, quad = c - 2 * b + a;
     // a monomer has at most 5 contacts on a cubic lattice (6 neighbours minus one chain bond), 3 in 2D
     int cmax = (s->nz > 1 && s->ny > 1 && s->nx > 1) ? 5 : 3;
-    if (lin * cmax > 127 || lin * cmax < -127 || quad > 127 || quad < -127) return GP_INVALID_ARG;
+    // int8 weights (scoring_tc.cu build_image_kernel): a pair column holds quad; a monomer column accumulates, over the
+    // monomer's <= cmax contacts, lin (free partner), lin + quad (fixed H partner) or lin (fixed P partner)
+    const int32_t alin = lin < 0 ? -lin : lin, alq = lin + quad < 0 ? -(lin + quad) : lin + quad;
+    if (cmax * (alin > alq ? alin : alq) > 127 || quad > 127 || quad < -127) return GP_INVALID_ARG;
     long long bound = (long long)s->NBP * (2LL * (lin < 0 ? -lin : lin) + (quad < 0 ? -quad : quad));
     if (bound > 8190) return GP_INVALID_ARG;  // pad structures score 8191 (scoring_tc.cu E_PAD)
     out->a = a; out->lin = lin; out->quad = quad; out->threshold = en->threshold;
@@ -256,7 +265,8 @@ extern "C" gp_status gp_enumerate_host(const gp_structures_t* s, const gp_energi
     const size_t n_out = (size_t)C + 1 + 3 * (size_t)C + 1;
     const size_t out_bytes = (n_out * sizeof(uint64_t) + 255) & ~(size_t)255;
     const size_t need = out_bytes + (g_count ? g_count : 1) * sizeof(uint16_t);
-    gp_structures_s* hs = const_cast<gp_structures_s*>(s);
+    const gp_structures_s* hs = s;
+    std::lock_guard<std::mutex> lk(hs->mu);  // synchronous call: one at a time per handle shares the kept device buffers
     if (hs->host_store_bytes < need) {
         if (hs->d_host_store) GP_CUDA(cudaFree(hs->d_host_store));
         hs->d_host_store = nullptr; hs->host_store_bytes = 0;

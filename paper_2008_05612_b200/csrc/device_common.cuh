@@ -38,12 +38,12 @@ __host__ __device__ inline uint64_t gp_draw(uint64_t seed, uint64_t ctr) {
     return gp_mix64(seed + (ctr + 1) * 0x9E3779B97F4A7C15ULL);
 }
 __host__ __device__ inline uint32_t gp_letter20(uint64_t seed, uint64_t seq, int k) {
-    uint64_t u = gp_draw(seed, seq * 16 + (uint64_t)k);
+    uint64_t u = gp_draw(seed, seq * 64 + (uint64_t)k);
     return (uint32_t)(((u >> 32) * 20) >> 32);
 }
 
 // scoring_tc.cu
-gp_status gp_launch_scoring_tc(gp_structures_s* s, const gp_hp_params& hp, uint64_t g_begin, uint64_t g_count,
+gp_status gp_launch_scoring_tc(const gp_structures_s* s, const gp_hp_params& hp, uint64_t g_begin, uint64_t g_count,
                                uint16_t* d_pheno, int16_t* d_gap, cudaStream_t st);
-gp_status gp_launch_sequences_tc(gp_structures_s* s, const gp_hp_params& hp, const uint8_t* d_seqs, uint64_t count,
+gp_status gp_launch_sequences_tc(const gp_structures_s* s, const gp_hp_params& hp, const uint8_t* d_seqs, uint64_t count,
                                  uint16_t* d_pheno, int16_t* d_gap, cudaStream_t st);

@@ -85,6 +85,7 @@ constexpr uint32_t ROB_PF_SLOTS = 1024;  // per-block filter of recently recorde
 
 __device__ __forceinline__ void note_pair(const RobArgs& a, uint32_t* pf, uint32_t p, uint32_t q) {
     if (q < p) { const uint32_t t = p; p = q; q = t; }
+    if (q >= a.C) return;
     if (pf) {
         const uint32_t key = (p << 16) | q;
         uint32_t* slot = pf + ((key * 2654435761u) >> 22);
@@ -115,6 +116,7 @@ constexpr uint32_t ROB_FLUSH_TILES = 64;
 struct RobSlot { uint32_t key, r, d, o; };
 
 __device__ __forceinline__ void rob_add(const RobArgs& a, RobSlot* cache, uint32_t p, uint32_t r, uint32_t d, uint32_t o) {
+    if (p >= a.C) return;                            // an id the caller's n_classes does not cover: skipped, like hist_kernel
     RobSlot* s = cache + ((p * 2654435761u) >> 21);  // 11 bits
     uint32_t k = s->key;
     if (k == NULLP) k = atomicCAS(&s->key, NULLP, p), k = (k == NULLP) ? p : k;
@@ -237,7 +239,7 @@ __global__ void robustness_tiny_kernel(RobArgs a) {
     const uint32_t g = threadIdx.x;
     if (g >= (1u << a.n_bits)) return;
     const uint32_t p = a.pheno[g];
-    if (p == NULLP) return;
+    if (p == NULLP || p >= a.C) return;
     unsigned long long r = 0, d = 0, o = 0;
     for (int k = 0; k < a.n_bits; k++) {
         const uint32_t q = a.pheno[g ^ (1u << k)];
@@ -273,9 +275,32 @@ __global__ void __launch_bounds__(256) phi_row_kernel(const uint16_t* __restrict
             const uint64_t g = v * 8 + j;
             for (int k = 0; k < n_bits; k++) {
                 const uint32_t p = pheno[g ^ (1ULL << k)];
-                atomicAdd(&row[p == NULLP ? C : p], 1ULL);
+                if (p == NULLP || p < C) atomicAdd(&row[p == NULLP ? C : p], 1ULL);
             }
         }
+    }
+}
+
+// Flips of a bit that selects the shard (multi-GPU): entry i of `mine` and entry i of `partner` are
+// neighbours.  Counts go to the classes of `mine` only (the partner's owner runs the mirror call).
+__global__ void __launch_bounds__(256) robustness_cross_kernel(RobArgs a, const uint16_t* __restrict__ partner, uint64_t count) {
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < count; i += (uint64_t)gridDim.x * blockDim.x) {
+        const uint32_t p = a.pheno[i];
+        if (p == NULLP || p >= a.C) continue;
+        const uint32_t q = partner[i];
+        if (q == p) atomicAdd(&a.R[p], 1ULL);
+        else if (q == NULLP) atomicAdd(&a.Dl[p], 1ULL);
+        else {
+            atomicAdd(&a.O[p], 1ULL);
+            if (a.bitmap && q < a.C) note_pair(a, nullptr, p, q);
+        }
+    }
+}
+
+__global__ void bitmap_or_kernel(uint32_t* __restrict__ dst, const uint32_t* __restrict__ src, uint64_t n_words) {
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_words; i += (uint64_t)gridDim.x * blockDim.x) {
+        const uint32_t v = src[i];
+        if (v) dst[i] |= v;
     }
 }
 
@@ -285,6 +310,65 @@ __global__ void popcount_kernel(const uint32_t* __restrict__ words, uint64_t n_w
         c += __popc(words[i]);
     for (int o = 16; o > 0; o >>= 1) c += __shfl_down_sync(0xFFFFFFFFu, c, o);
     if ((threadIdx.x & 31) == 0 && c) atomicAdd(out, c);
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// f4. Threshold sweep: designability at several energy thresholds from ONE
+// read of the (phenotype, gap) stores of a threshold-1 enumeration.  A genotype folds at threshold t iff it has a
+// unique ground state and second_min - min = -gap >= t.  bins[j][c] counts the genotypes of class c that fold at
+// exactly j of the (ascending) thresholds; suffix sums over j give the histogram per threshold.
+// ---------------------------------------------------------------------------------------------------------------
+constexpr int SWEEP_MAX = 16;
+struct SweepThr { int32_t t[SWEEP_MAX]; int n; };
+
+__global__ void __launch_bounds__(512) sweep_kernel(const uint16_t* __restrict__ pheno, const int16_t* __restrict__ gap,
+                                                    uint64_t count, uint32_t C, SweepThr thr,
+                                                    unsigned long long* __restrict__ bins, int use_smem) {
+    extern __shared__ uint32_t sh[];
+    const uint32_t n_bins = (uint32_t)(thr.n + 1) * C;
+    if (use_smem)
+        for (uint32_t i = threadIdx.x; i < n_bins; i += blockDim.x) sh[i] = 0;
+    __syncthreads();
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < count; i += (uint64_t)gridDim.x * blockDim.x) {
+        const uint32_t p = pheno[i];
+        if (p >= C) continue;  // null (or an id outside n_classes)
+        const int32_t gp = gap[i];
+        const int32_t margin = gp == GP_GAP_NONE ? INT32_MAX : -gp;
+        int j = 0;
+        for (int k = 0; k < thr.n; k++) j += (margin >= thr.t[k]);
+        if (use_smem) atomicAdd(&sh[(uint32_t)j * C + p], 1u);
+        else atomicAdd(&bins[(uint64_t)j * C + p], 1ULL);
+    }
+    __syncthreads();
+    if (use_smem)
+        for (uint32_t i = threadIdx.x; i < n_bins; i += blockDim.x)
+            if (sh[i]) atomicAdd(&bins[i], (unsigned long long)sh[i]);
+}
+
+// block t: hist[slot[t]][c] = sum_{j > t} bins[j][c]; folding and null counts
+__global__ void __launch_bounds__(256) sweep_finish_kernel(const unsigned long long* __restrict__ bins, uint64_t count,
+                                                           uint32_t C, int n, const int* __restrict__ slot_of,
+                                                           unsigned long long* __restrict__ folding,
+                                                           unsigned long long* __restrict__ hist) {
+    __shared__ unsigned long long part[256];
+    const int t = blockIdx.x, out = slot_of[t];
+    unsigned long long sum = 0;
+    for (uint32_t c = threadIdx.x; c < C; c += blockDim.x) {
+        unsigned long long v = 0;
+        for (int j = t + 1; j <= n; j++) v += bins[(uint64_t)j * C + c];
+        hist[(uint64_t)out * (C + 1) + c] = v;
+        sum += v;
+    }
+    part[threadIdx.x] = sum;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) part[threadIdx.x] += part[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        folding[out] = part[0];
+        hist[(uint64_t)out * (C + 1) + C] = count - part[0];
+    }
 }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -334,8 +418,6 @@ __global__ void uf_count_kernel(const uint16_t* __restrict__ pheno, const uint32
     }
 }
 
-int g_rob_tile_bits = ROB_TB_MAX;  // test hook (gp_set_rob_tile_bits): smaller tiles force the multi-pass path on small stores
-
 int sm_count() {
     int dev = 0, sms = 148;
     if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
@@ -343,12 +425,6 @@ int sm_count() {
 }
 
 }  // namespace
-
-extern "C" int gp_set_rob_tile_bits(int tb) {
-    if (tb < 4 || tb > ROB_TB_MAX) return -1;
-    g_rob_tile_bits = tb;
-    return 0;
-}
 
 extern "C" gp_status gp_designability(const uint16_t* d_pheno, uint64_t count, uint32_t n_classes, uint64_t* d_hist,
                                       void* stream) {
@@ -372,67 +448,161 @@ extern "C" gp_status gp_designability(const uint16_t* d_pheno, uint64_t count, u
     return GP_OK;
 }
 
-extern "C" gp_status gp_robustness(const uint16_t* d_pheno, int n_bits, uint32_t n_classes, uint64_t* d_neutral,
-                                   uint64_t* d_deleterious, uint64_t* d_other, uint64_t* d_pair_count, void* stream) {
+extern "C" uint64_t gp_pair_bitmap_words(uint32_t n_classes) { return ((uint64_t)n_classes * n_classes + 31) / 32; }
+
+extern "C" gp_status gp_robustness_partial(const uint16_t* d_pheno, int n_bits, uint32_t n_classes, uint64_t* d_neutral,
+                                           uint64_t* d_deleterious, uint64_t* d_other, uint32_t* d_pair_bitmap,
+                                           int tile_bits, void* stream) {
     if (!d_pheno || !d_neutral || !d_deleterious || !d_other) return GP_INVALID_ARG;
     if (n_bits < 1 || n_bits > 40 || n_classes == 0 || n_classes >= NULLP) return GP_INVALID_ARG;
+    if (tile_bits != 0 && (tile_bits < 4 || tile_bits > ROB_TB_MAX)) return GP_INVALID_ARG;
     if (((uintptr_t)d_pheno & 15) != 0) return GP_INVALID_ARG;
     cudaStream_t st = (cudaStream_t)stream;
-    const size_t cb = (size_t)n_classes * sizeof(uint64_t);
-    GP_CUDA(cudaMemsetAsync(d_neutral, 0, cb, st));
-    GP_CUDA(cudaMemsetAsync(d_deleterious, 0, cb, st));
-    GP_CUDA(cudaMemsetAsync(d_other, 0, cb, st));
     RobArgs a;
     a.pheno = d_pheno; a.n_bits = n_bits; a.C = n_classes;
     a.R = reinterpret_cast<unsigned long long*>(d_neutral);
     a.Dl = reinterpret_cast<unsigned long long*>(d_deleterious);
     a.O = reinterpret_cast<unsigned long long*>(d_other);
-    a.bitmap = nullptr;
-    uint64_t n_words = 0;
-    if (d_pair_count) {
-        n_words = ((uint64_t)n_classes * n_classes + 31) / 32;
-        GP_CUDA(cudaMallocAsync(&a.bitmap, n_words * 4, st));
-        GP_CUDA(cudaMemsetAsync(a.bitmap, 0, n_words * 4, st));
-        GP_CUDA(cudaMemsetAsync(d_pair_count, 0, sizeof(uint64_t), st));
-    }
+    a.bitmap = d_pair_bitmap;
     if (n_bits < 3) {
         gp_time_begin(GP_KERNEL_ROBUSTNESS, st);
         robustness_tiny_kernel<<<1, 32, 0, st>>>(a);
         gp_time_end(GP_KERNEL_ROBUSTNESS, st);
         GP_CUDA(cudaGetLastError());
         gp_count_launches(1);
-    } else {
-        const int tb = n_bits < g_rob_tile_bits ? n_bits : g_rob_tile_bits;
-        const size_t smem = ((size_t)2 << tb) + ROB_SLOTS * sizeof(RobSlot) + ROB_PF_SLOTS * sizeof(uint32_t);
-        GP_CUDA(cudaFuncSetAttribute(robustness_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        const uint64_t n_tiles = 1ULL << (n_bits - tb);
-        const uint64_t cap = (uint64_t)sm_count() * 2;
-        const unsigned grid = (unsigned)(n_tiles < cap ? n_tiles : cap);
-        a.tb = tb;
-        // pass 0: the tb low bits; then up to tb-3 further bits per pass (segments stay >= 16 bytes)
-        int done = 0;
-        while (done < n_bits) {
-            if (done == 0) { a.c = tb; a.h = 0; a.hi_pos = tb; a.f0 = 0; done = tb; }
-            else {
-                int h = n_bits - done;
-                const int hmax = tb - 7 > 1 ? tb - 7 : (tb - 3 > 1 ? tb - 3 : 1);  // keep segments >= 256 B when the tile allows
-                if (h > hmax) h = hmax;
-                a.h = h; a.c = tb - h; a.hi_pos = done; a.f0 = a.c; done += h;
-            }
-            gp_time_begin(GP_KERNEL_ROBUSTNESS, st);
-            robustness_kernel<<<grid, RTHREADS, smem, st>>>(a);
-            gp_time_end(GP_KERNEL_ROBUSTNESS, st);
-            GP_CUDA(cudaGetLastError());
-            gp_count_launches(1);
-        }
+        return GP_OK;
     }
-    if (d_pair_count) {
-        popcount_kernel<<<(unsigned)((n_words + 255) / 256 < 4096 ? (n_words + 255) / 256 : 4096), 256, 0, st>>>(
-            a.bitmap, n_words, reinterpret_cast<unsigned long long*>(d_pair_count));
+    const int tb_want = tile_bits ? tile_bits : ROB_TB_MAX;
+    const int tb = n_bits < tb_want ? n_bits : tb_want;
+    const size_t smem = ((size_t)2 << tb) + ROB_SLOTS * sizeof(RobSlot) + ROB_PF_SLOTS * sizeof(uint32_t);
+    GP_CUDA(cudaFuncSetAttribute(robustness_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const uint64_t n_tiles = 1ULL << (n_bits - tb);
+    const uint64_t cap = (uint64_t)sm_count() * 2;
+    const unsigned grid = (unsigned)(n_tiles < cap ? n_tiles : cap);
+    a.tb = tb;
+    // pass 0: the tb low bits; then up to tb-3 further bits per pass (segments stay >= 16 bytes)
+    int done = 0;
+    while (done < n_bits) {
+        if (done == 0) { a.c = tb; a.h = 0; a.hi_pos = tb; a.f0 = 0; done = tb; }
+        else {
+            int h = n_bits - done;
+            const int hmax = tb - 7 > 1 ? tb - 7 : (tb - 3 > 1 ? tb - 3 : 1);  // keep segments >= 256 B when the tile allows
+            if (h > hmax) h = hmax;
+            a.h = h; a.c = tb - h; a.hi_pos = done; a.f0 = a.c; done += h;
+        }
+        gp_time_begin(GP_KERNEL_ROBUSTNESS, st);
+        robustness_kernel<<<grid, RTHREADS, smem, st>>>(a);
+        gp_time_end(GP_KERNEL_ROBUSTNESS, st);
         GP_CUDA(cudaGetLastError());
         gp_count_launches(1);
-        GP_CUDA(cudaFreeAsync(a.bitmap, st));
     }
+    return GP_OK;
+}
+
+extern "C" gp_status gp_robustness_cross(const uint16_t* d_mine, const uint16_t* d_partner, uint64_t count,
+                                         uint32_t n_classes, uint64_t* d_neutral, uint64_t* d_deleterious,
+                                         uint64_t* d_other, uint32_t* d_pair_bitmap, void* stream) {
+    if (!d_mine || !d_partner || !d_neutral || !d_deleterious || !d_other) return GP_INVALID_ARG;
+    if (n_classes == 0 || n_classes >= NULLP) return GP_INVALID_ARG;
+    if (count == 0) return GP_OK;
+    cudaStream_t st = (cudaStream_t)stream;
+    RobArgs a;
+    a.pheno = d_mine; a.n_bits = 0; a.C = n_classes;
+    a.R = reinterpret_cast<unsigned long long*>(d_neutral);
+    a.Dl = reinterpret_cast<unsigned long long*>(d_deleterious);
+    a.O = reinterpret_cast<unsigned long long*>(d_other);
+    a.bitmap = d_pair_bitmap;
+    const uint64_t want = (count + 255) / 256, cap = (uint64_t)sm_count() * 8;
+    gp_time_begin(GP_KERNEL_ROBUSTNESS, st);
+    robustness_cross_kernel<<<(unsigned)(want < cap ? want : cap), 256, 0, st>>>(a, d_partner, count);
+    gp_time_end(GP_KERNEL_ROBUSTNESS, st);
+    GP_CUDA(cudaGetLastError());
+    gp_count_launches(1);
+    return GP_OK;
+}
+
+extern "C" gp_status gp_pair_bitmap_or(uint32_t* d_dst, const uint32_t* d_src, uint32_t n_classes, void* stream) {
+    if (!d_dst || !d_src || n_classes == 0 || n_classes >= NULLP) return GP_INVALID_ARG;
+    const uint64_t n_words = gp_pair_bitmap_words(n_classes);
+    bitmap_or_kernel<<<(unsigned)((n_words + 255) / 256 < 4096 ? (n_words + 255) / 256 : 4096), 256, 0, (cudaStream_t)stream>>>(
+        d_dst, d_src, n_words);
+    GP_CUDA(cudaGetLastError());
+    gp_count_launches(1);
+    return GP_OK;
+}
+
+extern "C" gp_status gp_pair_bitmap_count(const uint32_t* d_bitmap, uint32_t n_classes, uint64_t* d_count, void* stream) {
+    if (!d_bitmap || !d_count || n_classes == 0 || n_classes >= NULLP) return GP_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    const uint64_t n_words = gp_pair_bitmap_words(n_classes);
+    GP_CUDA(cudaMemsetAsync(d_count, 0, sizeof(uint64_t), st));
+    popcount_kernel<<<(unsigned)((n_words + 255) / 256 < 4096 ? (n_words + 255) / 256 : 4096), 256, 0, st>>>(
+        d_bitmap, n_words, reinterpret_cast<unsigned long long*>(d_count));
+    GP_CUDA(cudaGetLastError());
+    gp_count_launches(1);
+    return GP_OK;
+}
+
+extern "C" gp_status gp_robustness(const uint16_t* d_pheno, int n_bits, uint32_t n_classes, uint64_t* d_neutral,
+                                   uint64_t* d_deleterious, uint64_t* d_other, uint64_t* d_pair_count, void* stream) {
+    if (!d_pheno || !d_neutral || !d_deleterious || !d_other) return GP_INVALID_ARG;
+    if (n_bits < 1 || n_bits > 40 || n_classes == 0 || n_classes >= NULLP) return GP_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t cb = (size_t)n_classes * sizeof(uint64_t);
+    GP_CUDA(cudaMemsetAsync(d_neutral, 0, cb, st));
+    GP_CUDA(cudaMemsetAsync(d_deleterious, 0, cb, st));
+    GP_CUDA(cudaMemsetAsync(d_other, 0, cb, st));
+    uint32_t* bitmap = nullptr;
+    if (d_pair_count) {
+        const uint64_t n_words = gp_pair_bitmap_words(n_classes);
+        GP_CUDA(cudaMallocAsync(&bitmap, n_words * 4, st));
+        GP_CUDA(cudaMemsetAsync(bitmap, 0, n_words * 4, st));
+    }
+    gp_status stt = gp_robustness_partial(d_pheno, n_bits, n_classes, d_neutral, d_deleterious, d_other, bitmap, 0, stream);
+    if (stt == GP_OK && d_pair_count) stt = gp_pair_bitmap_count(bitmap, n_classes, d_pair_count, stream);
+    if (bitmap) cudaFreeAsync(bitmap, st);
+    return stt;
+}
+
+extern "C" gp_status gp_threshold_sweep(const uint16_t* d_pheno, const int16_t* d_gap, uint64_t count, uint32_t n_classes,
+                                        const int32_t* thresholds, int n_thresholds, uint64_t* d_folding,
+                                        uint64_t* d_hist, void* stream) {
+    if ((!d_pheno || !d_gap) && count) return GP_INVALID_ARG;
+    if (!thresholds || !d_folding || !d_hist || n_classes == 0 || n_classes >= NULLP) return GP_INVALID_ARG;
+    if (n_thresholds < 1 || n_thresholds > SWEEP_MAX) return GP_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    // ascending thresholds; slot[r] = position of the r-th smallest in the caller's order
+    SweepThr thr;
+    int slot[SWEEP_MAX];
+    thr.n = n_thresholds;
+    for (int i = 0; i < n_thresholds; i++) {
+        if (thresholds[i] < 1) return GP_INVALID_ARG;
+        int r = i;
+        while (r > 0 && thr.t[r - 1] > thresholds[i]) { thr.t[r] = thr.t[r - 1]; slot[r] = slot[r - 1]; r--; }
+        thr.t[r] = thresholds[i]; slot[r] = i;
+    }
+    const size_t n_bins = (size_t)(n_thresholds + 1) * n_classes;
+    char* work = nullptr;  // bins | slot table
+    GP_CUDA(cudaMallocAsync(&work, n_bins * 8 + SWEEP_MAX * sizeof(int), st));
+    unsigned long long* bins = reinterpret_cast<unsigned long long*>(work);
+    int* d_slot = reinterpret_cast<int*>(work + n_bins * 8);
+    GP_CUDA(cudaMemsetAsync(bins, 0, n_bins * 8, st));
+    GP_CUDA(cudaMemcpyAsync(d_slot, slot, n_thresholds * sizeof(int), cudaMemcpyHostToDevice, st));  // pageable: staged before return
+    const size_t smem = n_bins * 4;
+    const int use_smem = smem <= 200 * 1024;
+    if (use_smem) GP_CUDA(cudaFuncSetAttribute(sweep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    if (count) {
+        const uint64_t want = (count + 511) / 512, cap = (uint64_t)sm_count() * (use_smem && smem > 100 * 1024 ? 1 : 2);
+        sweep_kernel<<<(unsigned)(want < cap ? want : cap), 512, use_smem ? smem : 0, st>>>(
+            d_pheno, d_gap, count, n_classes, thr, bins, use_smem);
+        GP_CUDA(cudaGetLastError());
+    }
+    sweep_finish_kernel<<<n_thresholds, 256, 0, st>>>(bins, count, n_classes, n_thresholds, d_slot,
+                                                      reinterpret_cast<unsigned long long*>(d_folding),
+                                                      reinterpret_cast<unsigned long long*>(d_hist));
+    GP_CUDA(cudaGetLastError());
+    gp_count_launches(count ? 2 : 1);
+    GP_CUDA(cudaFreeAsync(work, st));
     return GP_OK;
 }
 

@@ -154,17 +154,13 @@ extern "C" gp_status gp_enumerate_simple(const gp_structures_t* s, const gp_ener
     return launch_simple(s, en, SRC_BITS, nullptr, 0, g_begin, g_count, d_pheno, d_gap, (cudaStream_t)stream);
 }
 
-static int g_seq_tc = 1;  // test hook (gp_set_seq_tc): 0 keeps explicit HP sequences on the CUDA-core kernel
-extern "C" int gp_set_seq_tc(int on) { g_seq_tc = on != 0; return 0; }
-
 extern "C" gp_status gp_enumerate_seqs(const gp_structures_t* s, const gp_energies* en, const uint8_t* d_seqs,
                                        uint64_t count, uint16_t* d_pheno, int16_t* d_gap, void* stream) {
     // two-letter sequences whose energies fit the int8 weights go to the tensor cores (sequence_kernel)
     gp_hp_params hp;
-    if (g_seq_tc && s && en && en->alphabet == 2 && d_seqs && d_pheno && count >= 256 && s->device >= 0 &&
+    if (s && s->tuning.seq_tensor && en && en->alphabet == 2 && d_seqs && d_pheno && count >= 256 && s->device >= 0 &&
         gp_check_hp(s, en, &hp) == GP_OK) {
-        gp_status st = gp_launch_sequences_tc(const_cast<gp_structures_s*>(s), hp, d_seqs, count, d_pheno, d_gap,
-                                              (cudaStream_t)stream);
+        gp_status st = gp_launch_sequences_tc(s, hp, d_seqs, count, d_pheno, d_gap, (cudaStream_t)stream);
         if (st != GP_UNSUPPORTED_LATTICE) return st;
     }
     return launch_simple(s, en, SRC_SEQS, d_seqs, 0, 0, count, d_pheno, d_gap, (cudaStream_t)stream);

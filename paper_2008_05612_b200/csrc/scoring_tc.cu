@@ -27,8 +27,7 @@ namespace tc {
 
 constexpr int MT = 4;                 // genotype tiles per supertile
 constexpr int TM = 128, TN = 128;     // weight tile: 128 structures; genotype tile: 128 rows
-constexpr int HN = 64;                // the epilogue drains 64 columns at a time; with NH = 2 (template) one MMA also
-                                      // covers 64 structures, so accumulator m is two independent 64-column buffers
+constexpr int HN = 64;                // the epilogue folds 64 columns at a time
 constexpr int ROWB = 128;             // bytes per operand row = one 128-byte swizzle span = up to 128 int8 features
 constexpr int TILE_BYTES = TM * ROWB; // 16 KB, A tile and B stage alike
 constexpr int NSTAGE = 6;
@@ -99,17 +98,6 @@ __device__ __forceinline__ bool elect_one() {
     asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(pred));
     return pred != 0;
 }
-__device__ __forceinline__ void tmem_ld32(uint32_t taddr, int32_t (&v)[32]) {
-    asm volatile(
-        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
-        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
-        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
-        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]),
-          "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]), "=r"(v[16]),
-          "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]), "=r"(v[24]),
-          "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
-        : "r"(taddr) : "memory");
-}
 // 128 accumulator columns as 64 registers: .pack::16b keeps the low 16 bits of each 32-bit column and packs two
 // adjacent columns per register (column 2i in the low half of v[i], column 2i+1 in the high half).  Energies are
 // |E| <= 8191, so the low 16 bits are the exact int16 value.
@@ -164,7 +152,6 @@ struct Args {
     int4* hrec;               // map mode (gp_enumerate_map): per genotype (k1, k2) over all columns and the snapshot of
                               // (k1, k2) after the first n_snap weight tiles; indexed like pheno; pheno/gap unused
     uint32_t n_snap;
-    int dbg;                  // measurement hook (gp_set_debug): 1 = skip the min/argmin fold, 2 = also skip the TMEM loads
 };
 
 // ---- a1: feature rows -----------------------------------------------------------------------------------------------
@@ -198,36 +185,11 @@ __device__ __forceinline__ void build_a_row(uint8_t* a_tile, uint32_t r, uint32_
 // energy counted with multiplicity (R6), and a tie at the minimum shows as equal energies in k1 and k2.
 // Filter: eight columns are rescanned only if their minimum is strictly below the current second-smallest energy;
 // an energy equal to it cannot change (k1, k2) because columns arrive in increasing order.
-__device__ __forceinline__ int min3(int a, int b, int c) { return min(a, min(b, c)); }
-__device__ __forceinline__ int min8(const int32_t* u) {
-    return min3(min3(u[0], u[1], u[2]), min3(u[3], u[4], u[5]), min(u[6], u[7]));
-}
 
-// 64 columns at a time: one test on the minimum of all 64 (36 min ops, 0.56 per energy); only when some energy is
-// strictly below the running second-smallest are the eight 8-column groups tested and the hit ones rescanned.
-__device__ __forceinline__ void fold_half(const int32_t (&v)[HN], uint32_t col0, int32_t& k1, int32_t& k2, int32_t& e2) {
-    int32_t g[8];
-#pragma unroll
-    for (int s = 0; s < 8; s++) g[s] = min8(&v[8 * s]);
-    if (min8(g) < e2) {
-#pragma unroll
-        for (int s = 0; s < 8; s++) {
-            if (g[s] < e2) {
-#pragma unroll
-                for (int j = 0; j < 8; j++) {
-                    const int32_t key = v[8 * s + j] * (1 << KEY_SHIFT) + (int32_t)(col0 + 8 * s + j);
-                    k2 = min(k2, max(k1, key));
-                    k1 = min(k1, key);
-                }
-                e2 = k2 >> KEY_SHIFT;
-            }
-        }
-    }
-}
-
-// The same filter on packed int16 pairs (two columns per register): per-halfword signed min (VIMNMX.S16X2-class DPX
-// instructions), 22 ALU ops per 64 columns instead of 37.  "some halfword of x is below e2" <=> min(x, E2) != E2 with
-// E2 = (e2, e2).
+// Packed int16 pairs (two columns per register, tcgen05.ld .pack::16b): per-halfword signed min (VIMNMX.S16X2-class
+// DPX instructions).  One test on the minimum of 64 columns (22 ALU ops); only when some energy is strictly below the
+// running second-smallest are the eight 8-column groups tested and the hit ones rescanned.  "some halfword of x is
+// below e2" <=> min(x, E2) != E2 with E2 = (e2, e2).
 __device__ __forceinline__ uint32_t pmin3(uint32_t a, uint32_t b, uint32_t c) { return __vimin3_s16x2(a, b, c); }
 __device__ __forceinline__ uint32_t pmin(uint32_t a, uint32_t b) { return __vmins2(a, b); }
 __device__ __forceinline__ uint32_t pack2(int32_t e) { return ((uint32_t)e & 0xFFFFu) * 0x10001u; }
@@ -260,16 +222,15 @@ __device__ __forceinline__ void fold_half_packed(const uint32_t* w, uint32_t col
 
 struct __align__(16) Barriers {
     uint64_t b_full[NSTAGE], b_empty[NSTAGE];
-    uint64_t acc_full[MT][2], acc_empty[MT][2];
+    uint64_t acc_full[MT], acc_empty[MT];
     uint64_t a_full, a_empty;
     uint32_t tmem_base;
 };
 
-// KS = 32-byte K steps per MMA chain (1..4); NH = 1: one N=128 MMA chain per accumulator, NH = 2: two N=64 chains into
-// independent halves (the tensor pipe refills one half while the other is drained).  PACK (NH = 1 only): the epilogue
-// reads the whole accumulator as packed int16 pairs, releases it at once and folds with two-lane SIMD min.
+// KS = 32-byte K steps per MMA chain (1..4).  One N=128 MMA chain per accumulator; the epilogue reads the whole
+// accumulator as packed int16 pairs, releases it at once and folds with two-lane SIMD min.
 // RB = bytes per operand row: 64 when the contraction has at most 64 columns (half the weight-tile and feature-row traffic)
-template <int KS, int NH, bool PACK, int RB>
+template <int KS, int RB>
 __global__ void __launch_bounds__(THREADS, 1) scoring_kernel(const Args a, const Cols cols_in) {
     constexpr int TB = TM * RB;                           // bytes of an A tile / a weight tile
     extern __shared__ unsigned char smem_dyn[];
@@ -278,8 +239,7 @@ __global__ void __launch_bounds__(THREADS, 1) scoring_kernel(const Args a, const
     uint8_t* sB = smem + MT * TB;                         // NSTAGE tiles
     Barriers* bar = reinterpret_cast<Barriers*>(sB + NSTAGE * TB);
     uint32_t* pk = reinterpret_cast<uint32_t*>(bar + 1);  // packed column table, ROWB words
-    constexpr int MN = TN / NH;                           // structures per MMA
-    constexpr uint32_t IDESC = idesc_for(MN);
+    constexpr uint32_t IDESC = idesc_for(TN);
 
     const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
@@ -287,8 +247,7 @@ __global__ void __launch_bounds__(THREADS, 1) scoring_kernel(const Args a, const
         pk[c] = cols_in.val[c] ? ((1u << cols_in.i[c]) | (1u << cols_in.j[c])) : 0xFFFFFFFFu;  // unused column: never all set
     if (threadIdx.x == 0) {
         for (int s = 0; s < NSTAGE; s++) { mbar_init(&bar->b_full[s], 1); mbar_init(&bar->b_empty[s], 1); }
-        for (int m = 0; m < MT; m++)
-            for (int h = 0; h < 2; h++) { mbar_init(&bar->acc_full[m][h], 1); mbar_init(&bar->acc_empty[m][h], 4); }
+        for (int m = 0; m < MT; m++) { mbar_init(&bar->acc_full[m], 1); mbar_init(&bar->acc_empty[m], 4); }
         mbar_init(&bar->a_full, 32 * EPI_WARPS);
         mbar_init(&bar->a_empty, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -334,22 +293,18 @@ __global__ void __launch_bounds__(THREADS, 1) scoring_kernel(const Args a, const
                 tc_fence_after();
                 const uint64_t bd = b_desc0 + (uint64_t)(s * (TB >> 4));
 #pragma unroll
-                for (int h = 0; h < NH; h++) {
+                for (int m = 0; m < MT; m++) {
+                    mbar_wait(&bar->acc_empty[m], (it & 1) ^ 1);
+                    tc_fence_after();
+                    if (elect_one()) {
+                        const uint32_t d = tmem + m * TN;
+                        const uint64_t ad = a_desc0 + (uint64_t)((m * TB) >> 4);
+                        mma_i8_c<false>(d, ad, bd, IDESC);
 #pragma unroll
-                    for (int m = 0; m < MT; m++) {
-                        mbar_wait(&bar->acc_empty[m][h], (it & 1) ^ 1);
-                        tc_fence_after();
-                        if (elect_one()) {
-                            const uint32_t d = tmem + m * TN + h * MN;
-                            const uint64_t ad = a_desc0 + (uint64_t)((m * TB) >> 4);
-                            const uint64_t bdh = bd + (uint64_t)((h * MN * RB) >> 4);
-                            mma_i8_c<false>(d, ad, bdh, IDESC);
-#pragma unroll
-                            for (int k = 1; k < KS; k++) mma_i8_c<true>(d, ad + 2 * k, bdh + 2 * k, IDESC);
-                            tc_commit(&bar->acc_full[m][h]);
-                        }
-                        __syncwarp();
+                        for (int k = 1; k < KS; k++) mma_i8_c<true>(d, ad + 2 * k, bd + 2 * k, IDESC);
+                        tc_commit(&bar->acc_full[m]);
                     }
+                    __syncwarp();
                 }
                 if (elect_one()) tc_commit(&bar->b_empty[s]);
                 __syncwarp();
@@ -373,51 +328,20 @@ __global__ void __launch_bounds__(THREADS, 1) scoring_kernel(const Args a, const
             mbar_arrive(&bar->a_full);
 
             int32_t k1 = INT32_MAX, k2 = INT32_MAX, s1 = INT32_MAX, s2 = INT32_MAX;
-            if (PACK) {
-                uint32_t E2 = pack2(E_NONE);
+            uint32_t E2 = pack2(E_NONE);
 #pragma unroll 1
-                for (uint32_t n = 0; n < a.n_tiles; n++, it++) {
-                    if (n == a.n_snap) { s1 = k1; s2 = k2; }
-                    mbar_wait(&bar->acc_full[m][0], it & 1);
-                    tc_fence_after();
-                    uint32_t w[2 * 32];
-                    if (!(a.dbg & 2)) {
-                        tmem_ld64_pack16(t_acc, w);
-                        tmem_ld_wait();
-                    }
-                    tc_fence_before();  // the accumulator is in registers: hand it back to the MMA warp
-                    __syncwarp();
-                    if (lane == 0) mbar_arrive(&bar->acc_empty[m][0]);
-                    if (!a.dbg) {
-                        fold_half_packed(&w[0], n * TN, k1, k2, E2);
-                        fold_half_packed(&w[32], n * TN + HN, k1, k2, E2);
-                    }
-                }
-            } else {
-                int32_t e2 = E_NONE;
-#pragma unroll 1
-                for (uint32_t n = 0; n < a.n_tiles; n++, it++) {
-                    if (n == a.n_snap) { s1 = k1; s2 = k2; }
-#pragma unroll 1
-                    for (uint32_t h = 0; h < 2; h++) {
-                        if (NH == 2 || h == 0) {
-                            mbar_wait(&bar->acc_full[m][NH == 2 ? h : 0], it & 1);
-                            tc_fence_after();
-                        }
-                        int32_t v[HN];
-                        if (!(a.dbg & 2)) {
-                            tmem_ld32(t_acc + h * HN, *reinterpret_cast<int32_t(*)[32]>(&v[0]));
-                            tmem_ld32(t_acc + h * HN + 32, *reinterpret_cast<int32_t(*)[32]>(&v[32]));
-                            tmem_ld_wait();
-                        }
-                        if (NH == 2 || h == 1) {  // the buffer is in registers: hand it back to the MMA warp
-                            tc_fence_before();
-                            __syncwarp();
-                            if (lane == 0) mbar_arrive(&bar->acc_empty[m][NH == 2 ? h : 0]);
-                        }
-                        if (!a.dbg) fold_half(v, n * TN + h * HN, k1, k2, e2);
-                    }
-                }
+            for (uint32_t n = 0; n < a.n_tiles; n++, it++) {
+                if (n == a.n_snap) { s1 = k1; s2 = k2; }
+                mbar_wait(&bar->acc_full[m], it & 1);
+                tc_fence_after();
+                uint32_t w[2 * 32];
+                tmem_ld64_pack16(t_acc, w);
+                tmem_ld_wait();
+                tc_fence_before();  // the accumulator is in registers: hand it back to the MMA warp
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&bar->acc_empty[m]);
+                fold_half_packed(&w[0], n * TN, k1, k2, E2);
+                fold_half_packed(&w[32], n * TN + HN, k1, k2, E2);
             }
             if (a.n_snap >= a.n_tiles) { s1 = k1; s2 = k2; }
             if (a.hrec) {
@@ -441,13 +365,13 @@ __global__ void __launch_bounds__(THREADS, 1) scoring_kernel(const Args a, const
 }
 
 typedef void (*scoring_fn)(const Args, const Cols);
-template <int NH, bool PACK, int RB>
+template <int RB>
 scoring_fn scoring_for(int ks) {
     switch (ks) {
-        case 1: return scoring_kernel<1, NH, PACK, RB>;
-        case 2: return scoring_kernel<2, NH, PACK, RB>;
-        case 3: return scoring_kernel<3, NH, PACK, RB>;
-        default: return scoring_kernel<4, NH, PACK, RB>;
+        case 1: return scoring_kernel<1, RB>;
+        case 2: return scoring_kernel<2, RB>;
+        case 3: return scoring_kernel<3, RB>;
+        default: return scoring_kernel<4, RB>;
     }
 }
 
@@ -461,13 +385,21 @@ struct ImgArgs {
     const uint8_t* contacts;   // D * NBP * 2
     const uint16_t* class_of;  // D; 0xFFFF marks a pad column inside the list
     int8_t* img;               // [n_images][n_tiles][TILE_BYTES]
-    const uint32_t* tile_list; // nullable: fixed-bit value of image y is tile_list[list_first + y], else gfix_first + y
+    const uint32_t* units;     // nullable (prefix path): fixed-bit value of image y is gfix_first + y.  Map path: the
+                               // unit table; see image_mid()
     uint64_t gfix_first;
-    uint32_t list_first;
+    uint64_t unit_first;
+    int paired, mid;           // map path: images 2j, 2j+1 = (m, rev m) of unit unit_first + j, else image j = m
     int gfix_shift;            // genotype with the fixed bits of image y in place = value << gfix_shift
     uint32_t D, n_tiles;
     int NBP, lin, quad;
 };
+
+// Map path: middle-bit value of image y of a launch group
+__device__ __forceinline__ uint32_t image_mid(const uint32_t* units, uint64_t unit_first, int paired, int mid, uint32_t y) {
+    const uint32_t m = units[unit_first + (paired ? (y >> 1) : y)];
+    return (paired && (y & 1u)) ? (mid ? (__brev(m) >> (32 - mid)) : 0u) : m;
+}
 
 // One block = one 128-structure tile of one image.  Thread = structure: it accumulates its 128-byte weight row in
 // shared memory (already in the swizzled layout the MMA reads), then the block writes the 16 KB tile out coalesced.
@@ -476,7 +408,8 @@ __global__ void __launch_bounds__(TN) build_image_kernel(const ImgArgs a, const 
     constexpr int TB = TM * RB;
     __shared__ __align__(16) int8_t tile[TB];
     const uint32_t r = threadIdx.x, n = blockIdx.x;
-    const uint64_t G = (a.tile_list ? (uint64_t)a.tile_list[a.list_first + blockIdx.y] : a.gfix_first + blockIdx.y) << a.gfix_shift;
+    const uint64_t G = (a.units ? (uint64_t)image_mid(a.units, a.unit_first, a.paired, a.mid, blockIdx.y) : a.gfix_first + blockIdx.y)
+                       << a.gfix_shift;
     for (uint32_t i = threadIdx.x; i < TB / 16; i += TN) reinterpret_cast<uint4*>(tile)[i] = make_uint4(0, 0, 0, 0);
     __syncthreads();
     const uint32_t d = n * TN + r;
@@ -540,13 +473,15 @@ static int make_columns(const int* mon, int fb, int N, Cols& cols, Slots& slots)
 // ---- map mode: merge the two half-lists of a genotype and its reversal -------------------------
 struct CombArgs {
     const int4* hrec;           // [n_images][2^fb]
-    const uint32_t* tile_list;  // middle-bit value of every image of the map
-    const uint32_t* partner;    // index (in tile_list) of the image holding the reversed genotypes
+    const uint32_t* units;      // unit table of the map
     const uint16_t* class_sym;
     uint16_t* pheno;
     int16_t* gap;               // nullable
-    uint32_t list_first, n_images;
-    int fb, k, N, threshold;
+    uint64_t unit_first;
+    uint64_t compact_base;      // compact layout: output index of this group's image 0, local genotype 0
+    uint32_t n_images;
+    int paired, mid;            // the image holding the reversed genotypes of image y is y ^ 1 (paired) or y itself
+    int fb, k, N, threshold, compact;
 };
 
 __global__ void __launch_bounds__(256) combine_kernel(const CombArgs a) {
@@ -554,7 +489,7 @@ __global__ void __launch_bounds__(256) combine_kernel(const CombArgs a) {
     const uint32_t tmask = (1u << a.fb) - 1u, kmask = (1u << a.k) - 1u;
     for (uint64_t idx = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (uint64_t)gridDim.x * blockDim.x) {
         const uint32_t y = (uint32_t)(idx >> a.fb), t = (uint32_t)idx & tmask;
-        const uint32_t yp = a.partner[a.list_first + y] - a.list_first;
+        const uint32_t yp = a.paired ? (y ^ 1u) : y;
         const uint32_t tr = __brev(t) >> (32 - a.fb);
         const int4 A = a.hrec[idx];
         const int4 B = a.hrec[((uint64_t)yp << a.fb) + tr];
@@ -567,21 +502,13 @@ __global__ void __launch_bounds__(256) combine_kernel(const CombArgs a) {
         const uint32_t col = (uint32_t)(own ? A.x : B.z) & ((1u << KEY_SHIFT) - 1u);
         const bool single = (m2 >= E_PAD);
         const bool folds = single || (m2 - m1 >= a.threshold);
-        const uint64_t g = ((uint64_t)(t >> a.k) << (a.N - a.k)) | ((uint64_t)a.tile_list[a.list_first + y] << a.k) | (t & kmask);
+        const uint64_t g = a.compact ? a.compact_base + idx
+                                     : ((uint64_t)(t >> a.k) << (a.N - a.k)) |
+                                           ((uint64_t)image_mid(a.units, a.unit_first, a.paired, a.mid, y) << a.k) | (t & kmask);
         a.pheno[g] = folds ? a.class_sym[col] : (uint16_t)GP_NULL_PHENO;
         if (a.gap) a.gap[g] = (int16_t)(single ? GP_GAP_NONE : max(m1 - m2, -32768));
     }
 }
-
-int g_sym_bits = 7;    // k of map mode: the k first and k last monomers vary inside an image (7: 53 columns, 2 K steps;
-                       // 9: 85 columns, 3 K steps and 16x fewer images, 7 % slower on the full 6x6 map)
-
-int g_fold_bits = 15;  // 2 + 15 + 42 = 59 columns -> 2 K steps; an image per 2^15 genotypes costs 5 us to build
-                       // (19: 93 columns, 3 K steps, was the default until the builder was timed per image: +10 %)
-int g_halves = 1;      // NH of scoring_kernel
-int g_debug = 0;
-int g_narrow = 1;      // 64-byte operand rows when the contraction has at most 64 columns
-int g_pack = 1;        // PACK of scoring_kernel
 
 // =====================================================================================================================
 // Explicit sequences on the tensor cores (the paper's sampling runs, Table 3).
@@ -803,235 +730,364 @@ __global__ void __launch_bounds__(SQ_THREADS, 1) sequence_kernel(const SqArgs a,
     }
 }
 
+
+// ---- MMA-only probe: the measured int8 tensor peak this kernel family can be held against -----------------------------
+// One CTA per SM issues the scoring kernel's own instruction stream — chains of KS tcgen05.mma kind::i8 M128 x N128 x
+// K32 into four TMEM accumulators, operands in the same swizzled shared-memory layout — with no TMA traffic, no TMEM
+// read-out and no epilogue: one commit per 64 MMAs, at most two commit groups in flight.
+template <int KS, int RB>
+__global__ void __launch_bounds__(128, 1) mma_probe_kernel(uint32_t groups, unsigned long long* cycles) {
+    constexpr int TB = TM * RB;
+    extern __shared__ unsigned char smem_dyn[];
+    unsigned char* smem = reinterpret_cast<unsigned char*>(((uintptr_t)smem_dyn + 1023) & ~(uintptr_t)1023);
+    __shared__ __align__(8) uint64_t done[2];
+    __shared__ uint32_t tmem_base;
+    for (uint32_t i = threadIdx.x; i < 2 * TB / 4; i += blockDim.x)  // pseudo-random operand bytes (zeros would flatter the clocks)
+        reinterpret_cast<uint32_t*>(smem)[i] = (uint32_t)gp_mix64(i + 977u * blockIdx.x);
+    if (threadIdx.x == 0) {
+        mbar_init(&done[0], 1);
+        mbar_init(&done[1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    const uint32_t warp = threadIdx.x >> 5;
+    if (warp == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(&tmem_base)) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    fence_proxy_async();
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = tmem_base;
+    if (warp == 0) {
+        constexpr uint32_t IDESC = idesc_for(TN);
+        const uint64_t ad = smem_desc_rb<RB>(smem_u32(smem)), bd = smem_desc_rb<RB>(smem_u32(smem + TB));
+        const long long t0 = clock64();
+        for (uint32_t g = 0; g < groups; g++) {
+            if (g >= 2) mbar_wait(&done[g & 1], ((g >> 1) - 1) & 1);
+            if (elect_one()) {
+#pragma unroll 4
+                for (int c = 0; c < 64 / KS; c++) {
+                    const uint32_t d = tmem + (c & 3) * TN;
+                    mma_i8_c<false>(d, ad, bd, IDESC);
+#pragma unroll
+                    for (int k = 1; k < KS; k++) mma_i8_c<true>(d, ad + 2 * k, bd + 2 * k, IDESC);
+                }
+                tc_commit(&done[g & 1]);
+            }
+            __syncwarp();
+        }
+        for (uint32_t g = groups > 2 ? groups - 2 : 0; g < groups; g++) mbar_wait(&done[g & 1], (g >> 1) & 1);
+        const long long t1 = clock64();
+        if (threadIdx.x == 0) cycles[blockIdx.x] = (unsigned long long)(t1 - t0);
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 0) {
+        tc_fence_after();
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem) : "memory");
+    }
+}
+
 }  // namespace tc
 
-// test / tuning hook (not part of the public header): number of low genotype bits kept as contraction columns
-extern "C" int gp_set_fold_bits(int fb) {
-    if (fb < 9 || fb > tc::MAX_FB) return -1;
-    tc::g_fold_bits = fb;
-    return 0;
+// ---- tuning (include/gpmap.h: gp_tuning) ------------------------------------------------------------------------------
+extern "C" gp_status gp_tuning_get(const gp_structures_t* s, gp_tuning* out) {
+    if (!s || !out) return GP_INVALID_ARG;
+    *out = s->tuning;
+    return GP_OK;
 }
 
-extern "C" int gp_set_debug(int d) { tc::g_debug = d; return 0; }  // measurement hook: results are garbage when non-zero
-extern "C" int gp_set_sym_bits(int k) {  // test / tuning hook
-    if (k < 5 || 2 * k > tc::MAX_FB) return -1;
-    tc::g_sym_bits = k;
-    return 0;
-}
-extern "C" int gp_set_narrow(int on) { tc::g_narrow = on != 0; return 0; }  // test / tuning hook
-extern "C" int gp_set_pack(int p) { tc::g_pack = p != 0; return 0; }
-extern "C" int gp_set_halves(int nh) {  // test / tuning hook
-    if (nh != 1 && nh != 2) return -1;
-    tc::g_halves = nh;
-    return 0;
+extern "C" gp_status gp_tuning_set(gp_structures_t* s, const gp_tuning* t) {
+    if (!s || !t) return GP_INVALID_ARG;
+    if (t->fold_bits < 9 || t->fold_bits > tc::MAX_FB || t->sym_bits < 5 || 2 * t->sym_bits > tc::MAX_FB) return GP_INVALID_ARG;
+    if ((t->narrow_rows | 1) != 1 || (t->seq_tensor | 1) != 1) return GP_INVALID_ARG;
+    const bool rebuild = t->sym_bits != s->tuning.sym_bits;
+    const gp_tuning old = s->tuning;
+    s->tuning = *t;
+    if (rebuild) {
+        gp_status st = gp_build_map_units(s);
+        if (st != GP_OK) { s->tuning = old; gp_build_map_units(s); return st; }
+    }
+    return GP_OK;
 }
 
-gp_status gp_launch_scoring_tc(gp_structures_s* s, const gp_hp_params& hp, uint64_t g_begin, uint64_t g_count,
+namespace {
+
+// Geometry of one scoring launch family: contraction columns, K steps, operand rows, kernel and its shared memory
+struct Plan {
+    tc::Cols cols;
+    tc::Slots slots;
+    int nc = 0, k_steps = 0;
+    bool narrow = false;
+    uint32_t n_tiles = 0;
+    size_t tile_bytes = 0, img_bytes = 0, smem = 0;
+    tc::scoring_fn kernel = nullptr;
+    int sms = 0;
+};
+
+gp_status make_plan(const gp_structures_s* s, const int* mon, int fb, uint32_t n_columns, Plan& p) {
+    using namespace tc;
+    p.nc = make_columns(mon, fb, s->N, p.cols, p.slots);
+    if (p.nc > ROWB) return GP_UNSUPPORTED_LATTICE;
+    p.k_steps = (p.nc + 31) / 32;
+    p.n_tiles = (n_columns + TN - 1) / TN;
+    p.narrow = p.nc <= 64 && s->tuning.narrow_rows;  // at most 64 columns: 64-byte operand rows
+    p.tile_bytes = (size_t)TM * (p.narrow ? 64 : 128);
+    p.img_bytes = (size_t)p.n_tiles * p.tile_bytes;
+    p.smem = (size_t)(MT + NSTAGE) * p.tile_bytes + sizeof(Barriers) + ROWB * sizeof(uint32_t) + 1024 + 64;
+    p.kernel = p.narrow ? scoring_for<64>(p.k_steps) : scoring_for<128>(p.k_steps);
+    int dev = 0;
+    GP_CUDA(cudaGetDevice(&dev));
+    GP_CUDA(cudaDeviceGetAttribute(&p.sms, cudaDevAttrMultiProcessorCount, dev));
+    GP_CUDA(cudaFuncSetAttribute(p.kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem));
+    return GP_OK;
+}
+
+}  // namespace
+
+gp_status gp_launch_scoring_tc(const gp_structures_s* s, const gp_hp_params& hp, uint64_t g_begin, uint64_t g_count,
                                uint16_t* d_pheno, int16_t* d_gap, cudaStream_t st) {
     using namespace tc;
     const int N = s->N;
-    const int fb = N < g_fold_bits ? N : g_fold_bits;
+    const int fb = N < s->tuning.fold_bits ? N : s->tuning.fold_bits;
     if (s->D >= (1u << KEY_SHIFT)) return GP_UNSUPPORTED_LATTICE;
-    Cols cols;
-    Slots slots;
+    Plan p;
     int mon[MAX_FB];
     for (int i = 0; i < fb; i++) mon[i] = i;
-    const int nc = make_columns(mon, fb, N, cols, slots);
-    if (nc > ROWB) return GP_INVALID_ARG;
-    const int k_steps = (nc + 31) / 32;
-    const uint32_t n_tiles = (s->D + TN - 1) / TN;
-    // at most 64 columns: 64-byte operand rows (half the image, weight-tile and feature-row traffic)
-    const bool narrow = nc <= 64 && g_narrow && g_halves == 1 && g_pack;
-    const size_t tile_bytes = (size_t)TM * (narrow ? 64 : 128);
-    const size_t img_bytes = (size_t)n_tiles * tile_bytes;
-
-    int dev = 0, sms = 0;
-    GP_CUDA(cudaGetDevice(&dev));
-    GP_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    const size_t smem = (size_t)(MT + NSTAGE) * tile_bytes + sizeof(Barriers) + ROWB * sizeof(uint32_t) + 1024 + 64;
-    const scoring_fn kernel = narrow         ? scoring_for<1, true, 64>(k_steps)
-                              : g_halves == 2 ? scoring_for<2, false, 128>(k_steps)
-                              : g_pack        ? scoring_for<1, true, 128>(k_steps)
-                                              : scoring_for<1, false, 128>(k_steps);
-    GP_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    gp_status stt = make_plan(s, mon, fb, s->D, p);
+    if (stt != GP_OK) return stt == GP_UNSUPPORTED_LATTICE ? GP_INVALID_ARG : stt;
 
     // batches of 2^fb genotypes share a weight image; a launch covers up to `group` batches
-    const uint64_t batch_len = 1ULL << fb;
     const uint64_t g_end = g_begin + g_count;
-    uint64_t group = (1024ULL << 20) / img_bytes;  // <= 1 GB of images per launch
+    uint64_t group = (1024ULL << 20) / p.img_bytes;  // <= 1 GB of images per launch
     if (group < 1) group = 1;
     if (group > 256) group = 256;
-    const size_t need = img_bytes * (size_t)group;
-    if (s->scratch_bytes < need) {
-        if (s->d_scratch) GP_CUDA(cudaFree(s->d_scratch));
-        s->d_scratch = nullptr; s->scratch_bytes = 0;
-        GP_CUDA(cudaMalloc(&s->d_scratch, need));
-        s->scratch_bytes = need;
-    }
+    const uint64_t n_batches_all = ((g_end - 1) >> fb) - (g_begin >> fb) + 1;
+    if (group > n_batches_all) group = n_batches_all;
+    int8_t* d_img = nullptr;  // per-call working memory from the stream-ordered pool: calls on other streams have their own
+    GP_CUDA(cudaMallocAsync(&d_img, p.img_bytes * (size_t)group, st));
     uint64_t g = g_begin & ~(uint64_t)(SUPER - 1);  // g_begin is a multiple of gp_tile() = SUPER already
+    gp_status result = GP_OK;
     while (g < g_end) {
         const uint64_t b0 = g >> fb;
         uint64_t stop = (b0 + group) << fb;
         if (stop > g_end) stop = g_end;
         const uint32_t n_batches = (uint32_t)(((stop - 1) >> fb) - b0 + 1);
         ImgArgs ia;
-        ia.contacts = s->d_contacts; ia.class_of = s->d_class_of; ia.img = (int8_t*)s->d_scratch; ia.tile_list = nullptr;
-        ia.gfix_first = b0; ia.list_first = 0; ia.gfix_shift = fb; ia.D = s->D; ia.n_tiles = n_tiles;
+        ia.contacts = s->d_contacts; ia.class_of = s->d_class_of; ia.img = d_img; ia.units = nullptr;
+        ia.gfix_first = b0; ia.unit_first = 0; ia.paired = 0; ia.mid = 0; ia.gfix_shift = fb; ia.D = s->D; ia.n_tiles = p.n_tiles;
         ia.NBP = s->NBP; ia.lin = hp.lin; ia.quad = hp.quad;
         gp_time_begin(GP_KERNEL_IMAGE, st);
-        if (narrow) build_image_kernel<64><<<dim3(n_tiles, n_batches), TN, 0, st>>>(ia, slots);
-        else build_image_kernel<128><<<dim3(n_tiles, n_batches), TN, 0, st>>>(ia, slots);
+        if (p.narrow) build_image_kernel<64><<<dim3(p.n_tiles, n_batches), TN, 0, st>>>(ia, p.slots);
+        else build_image_kernel<128><<<dim3(p.n_tiles, n_batches), TN, 0, st>>>(ia, p.slots);
         gp_time_end(GP_KERNEL_IMAGE, st);
-        GP_CUDA(cudaGetLastError());
         Args a;
-        a.img = (const int8_t*)s->d_scratch; a.class_of = s->d_class_of; a.pheno = d_pheno; a.gap = d_gap;
+        a.img = d_img; a.class_of = s->d_class_of; a.pheno = d_pheno; a.gap = d_gap;
         a.g_first = g; a.g_end = stop; a.out_base = g_begin;
         a.n_items = (uint32_t)((stop - g + SUPER - 1) / SUPER);
-        a.n_tiles = n_tiles; a.D = s->D; a.fb = fb; a.k_steps = k_steps; a.threshold = hp.threshold; a.dbg = g_debug;
-        a.hrec = nullptr; a.n_snap = n_tiles;
-        const unsigned grid = a.n_items < (uint32_t)sms ? a.n_items : (uint32_t)sms;
+        a.n_tiles = p.n_tiles; a.D = s->D; a.fb = fb; a.k_steps = p.k_steps; a.threshold = hp.threshold;
+        a.hrec = nullptr; a.n_snap = p.n_tiles;
+        const unsigned grid = a.n_items < (uint32_t)p.sms ? a.n_items : (uint32_t)p.sms;
         gp_time_begin(GP_KERNEL_SCORING, st);
-        kernel<<<grid, THREADS, smem, st>>>(a, cols);
+        p.kernel<<<grid, THREADS, p.smem, st>>>(a, p.cols);
         gp_time_end(GP_KERNEL_SCORING, st);
-        GP_CUDA(cudaGetLastError());
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) { gp_set_cuda_error(e, "scoring launch"); result = GP_CUDA_ERROR; break; }
         gp_count_launches(2);
         g = stop;
     }
-    (void)batch_len;
-    return GP_OK;
+    cudaFreeAsync(d_img, st);
+    return result;
 }
 
-// Whole map through the reversal identity E(g, rev S) = E(rev g, S): every genotype is
-// scored on ONE representative per class (C columns instead of D); the energies of the other class members are those
-// of the reversed genotype on the same representatives.  An image holds the 2^(2k) genotypes that share their middle
-// N - 2k bits, so the reversed genotypes of image m are exactly image rev(m), read in bit-reversed local order.
-gp_status gp_launch_map_tc(gp_structures_s* s, const gp_hp_params& hp, uint16_t* d_pheno, int16_t* d_gap, cudaStream_t st) {
+// ---- whole map through the reversal identity E(g, rev S) = E(rev g, S) ---------------
+// Every genotype is scored on ONE representative per class (C columns instead of D); the energies of the other class
+// members are those of the reversed genotype on the same representatives.  An image holds the 2^(2k) genotypes that
+// share their middle N - 2k bits m, so the reversed genotypes of image m are exactly image rev(m), read in bit-reversed
+// local order.  A unit = {m, rev m}; the table lists m <= rev m, pairs first (include/gpmap.h).
+static int map_k_for(const gp_structures_s* s) {
     using namespace tc;
     const int N = s->N;
-    int k = g_sym_bits < N / 2 ? g_sym_bits : N / 2;
+    const int k = s->tuning.sym_bits < N / 2 ? s->tuning.sym_bits : N / 2;
     const int fb = 2 * k, mid = N - fb;
-    if (fb < 9 || s->D_sym >= (1u << KEY_SHIFT)) return GP_UNSUPPORTED_LATTICE;  // caller falls back to the prefix path
+    if (fb < 9 || mid > 26 || s->D_sym >= (1u << KEY_SHIFT)) return 0;
     Cols cols;
     Slots slots;
     int mon[MAX_FB];
     for (int l = 0; l < k; l++) { mon[l] = l; mon[k + l] = N - k + l; }
-    const int nc = make_columns(mon, fb, N, cols, slots);
-    if (nc > ROWB) return GP_UNSUPPORTED_LATTICE;
-    const int k_steps = (nc + 31) / 32;
-    const uint32_t n_tiles = (s->D_sym + TN - 1) / TN;
-    const bool narrow = nc <= 64 && g_narrow && g_pack;
-    const size_t tile_bytes = (size_t)TM * (narrow ? 64 : 128);
-    const size_t img_bytes = (size_t)n_tiles * tile_bytes;
-    const size_t rec_bytes = sizeof(int4) << fb;
+    return make_columns(mon, fb, N, cols, slots) <= ROWB ? k : 0;
+}
 
-    // images of the map: m and rev(m) adjacent, each unordered pair once
+gp_status gp_build_map_units(gp_structures_s* s) {
+    if (s->d_units) { cudaFree(s->d_units); s->d_units = nullptr; }
+    s->units.clear();
+    s->map_k = map_k_for(s);
+    if (!s->map_k) { s->n_units = 1; s->n_pair_units = 0; return GP_OK; }  // one unit = the whole map (prefix path)
+    const int mid = s->N - 2 * s->map_k;
     const uint32_t n_mid = 1u << mid;
-    std::vector<uint32_t> tiles, partner, cuts;
-    size_t group = (1024ULL << 20) / (img_bytes + rec_bytes);  // <= 1 GB of images + records per launch
-    if (group < 2) group = 2;
-    if (group > 512) group = 512;
-    cuts.push_back(0);
+    std::vector<uint32_t> pal;
     for (uint32_t m = 0; m < n_mid; m++) {
         uint32_t r = 0;
         for (int b = 0; b < mid; b++) r |= ((m >> b) & 1u) << (mid - 1 - b);
-        if (r < m) continue;
-        if (tiles.size() - cuts.back() + 2 > group) cuts.push_back((uint32_t)tiles.size());
-        const uint32_t at = (uint32_t)tiles.size();
-        if (r == m) { tiles.push_back(m); partner.push_back(at); }
-        else { tiles.push_back(m); tiles.push_back(r); partner.push_back(at + 1); partner.push_back(at); }
+        if (r > m) s->units.push_back(m);
+        else if (r == m) pal.push_back(m);
     }
-    cuts.push_back((uint32_t)tiles.size());
-
-    int dev = 0, sms = 0;
-    GP_CUDA(cudaGetDevice(&dev));
-    GP_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    const size_t smem = (size_t)(MT + NSTAGE) * tile_bytes + sizeof(Barriers) + ROWB * sizeof(uint32_t) + 1024 + 64;
-    const scoring_fn kernel = narrow ? scoring_for<1, true, 64>(k_steps)
-                              : g_pack ? scoring_for<1, true, 128>(k_steps) : scoring_for<1, false, 128>(k_steps);
-    GP_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    const size_t need = (img_bytes + rec_bytes) * group;
-    if (s->scratch_bytes < need) {
-        if (s->d_scratch) GP_CUDA(cudaFree(s->d_scratch));
-        s->d_scratch = nullptr; s->scratch_bytes = 0;
-        GP_CUDA(cudaMalloc(&s->d_scratch, need));
-        s->scratch_bytes = need;
+    s->n_pair_units = s->units.size();
+    s->units.insert(s->units.end(), pal.begin(), pal.end());
+    s->n_units = s->units.size();
+    if (s->device >= 0) {
+        GP_CUDA(cudaMalloc(&s->d_units, s->units.size() * sizeof(uint32_t)));
+        GP_CUDA(cudaMemcpy(s->d_units, s->units.data(), s->units.size() * sizeof(uint32_t), cudaMemcpyHostToDevice));
     }
-    int8_t* d_img = (int8_t*)s->d_scratch;
-    int4* d_rec = (int4*)((char*)s->d_scratch + img_bytes * group);
-    uint32_t* d_lists = nullptr;  // tiles | partner
-    GP_CUDA(cudaMallocAsync(&d_lists, tiles.size() * 2 * sizeof(uint32_t), st));
-    GP_CUDA(cudaMemcpyAsync(d_lists, tiles.data(), tiles.size() * sizeof(uint32_t), cudaMemcpyHostToDevice, st));
-    GP_CUDA(cudaMemcpyAsync(d_lists + tiles.size(), partner.data(), tiles.size() * sizeof(uint32_t), cudaMemcpyHostToDevice, st));
-    GP_CUDA(cudaStreamSynchronize(st));  // the host vectors go out of scope; pageable copies are staged, this is belt and braces
+    return GP_OK;
+}
 
-    for (size_t c = 0; c + 1 < cuts.size(); c++) {
-        const uint32_t first = cuts[c], n_img = cuts[c + 1] - cuts[c];
-        if (!n_img) continue;
+extern "C" uint64_t gp_map_units(const gp_structures_t* s) { return s ? s->n_units : 0; }
+
+extern "C" gp_status gp_map_unit(const gp_structures_t* s, uint64_t unit, uint64_t* m, int* k) {
+    if (!s) return GP_INVALID_ARG;
+    if (unit >= s->n_units) return GP_RANGE;
+    if (m) *m = s->map_k ? s->units[unit] : 0;
+    if (k) *k = s->map_k;  // 0: the single unit is the whole map
+    return GP_OK;
+}
+
+static gp_status gp_launch_map_range(const gp_structures_s* s, const gp_hp_params& hp, uint64_t u_first, uint64_t u_count,
+                                     uint16_t* d_pheno, int16_t* d_gap, int compact, cudaStream_t st) {
+    using namespace tc;
+    const int N = s->N, k = s->map_k, fb = 2 * k, mid = N - fb;
+    Plan p;
+    int mon[MAX_FB];
+    for (int l = 0; l < k; l++) { mon[l] = l; mon[k + l] = N - k + l; }
+    gp_status stt = make_plan(s, mon, fb, s->D_sym, p);
+    if (stt != GP_OK) return stt;
+    const size_t rec_bytes = sizeof(int4) << fb;
+    size_t group = (1024ULL << 20) / (p.img_bytes + rec_bytes);  // <= 1 GB of images + records per launch
+    if (group > 512) group = 512;
+    group &= ~(size_t)1;
+    if (group < 2) group = 2;
+    {   // never more than the range needs
+        const uint64_t pairs = u_first < s->n_pair_units ? (u_first + u_count < s->n_pair_units ? u_count : s->n_pair_units - u_first) : 0;
+        const uint64_t most = 2 * pairs > u_count - pairs ? 2 * pairs : u_count - pairs;
+        if (group > most) group = (size_t)((most + 1) & ~1ULL);
+    }
+    char* d_work = nullptr;
+    GP_CUDA(cudaMallocAsync(&d_work, (p.img_bytes + rec_bytes) * group, st));
+    int8_t* d_img = (int8_t*)d_work;
+    int4* d_rec = (int4*)(d_work + p.img_bytes * group);
+    gp_status result = GP_OK;
+    uint64_t u = u_first, images_done = 0;
+    const uint64_t u_end = u_first + u_count;
+    while (u < u_end) {
+        const int paired = u < s->n_pair_units;
+        uint64_t stop = paired ? u + group / 2 : u + group;
+        const uint64_t limit = paired && s->n_pair_units < u_end ? s->n_pair_units : u_end;
+        if (stop > limit) stop = limit;
+        const uint32_t n_img = (uint32_t)(stop - u) * (paired ? 2u : 1u);
         ImgArgs ia;
-        ia.contacts = s->d_contacts_sym; ia.class_of = s->d_class_sym; ia.img = d_img; ia.tile_list = d_lists;
-        ia.gfix_first = 0; ia.list_first = first; ia.gfix_shift = k; ia.D = s->D_sym; ia.n_tiles = n_tiles;
-        ia.NBP = s->NBP; ia.lin = hp.lin; ia.quad = hp.quad;
+        ia.contacts = s->d_contacts_sym; ia.class_of = s->d_class_sym; ia.img = d_img; ia.units = s->d_units;
+        ia.gfix_first = 0; ia.unit_first = u; ia.paired = paired; ia.mid = mid; ia.gfix_shift = k; ia.D = s->D_sym;
+        ia.n_tiles = p.n_tiles; ia.NBP = s->NBP; ia.lin = hp.lin; ia.quad = hp.quad;
         gp_time_begin(GP_KERNEL_IMAGE, st);
-        if (narrow) build_image_kernel<64><<<dim3(n_tiles, n_img), TN, 0, st>>>(ia, slots);
-        else build_image_kernel<128><<<dim3(n_tiles, n_img), TN, 0, st>>>(ia, slots);
+        if (p.narrow) build_image_kernel<64><<<dim3(p.n_tiles, n_img), TN, 0, st>>>(ia, p.slots);
+        else build_image_kernel<128><<<dim3(p.n_tiles, n_img), TN, 0, st>>>(ia, p.slots);
         gp_time_end(GP_KERNEL_IMAGE, st);
-        GP_CUDA(cudaGetLastError());
         Args a;
         a.img = d_img; a.class_of = s->d_class_sym; a.pheno = nullptr; a.gap = nullptr;
         a.g_first = 0; a.g_end = (uint64_t)n_img << fb; a.out_base = 0;
         a.n_items = (uint32_t)((a.g_end + SUPER - 1) / SUPER);
-        a.n_tiles = n_tiles; a.D = s->D_sym; a.fb = fb; a.k_steps = k_steps; a.threshold = hp.threshold; a.dbg = g_debug;
+        a.n_tiles = p.n_tiles; a.D = s->D_sym; a.fb = fb; a.k_steps = p.k_steps; a.threshold = hp.threshold;
         a.hrec = d_rec; a.n_snap = s->n_snap;
-        const unsigned grid = a.n_items < (uint32_t)sms ? a.n_items : (uint32_t)sms;
+        const unsigned grid = a.n_items < (uint32_t)p.sms ? a.n_items : (uint32_t)p.sms;
         gp_time_begin(GP_KERNEL_SCORING, st);
-        kernel<<<grid, THREADS, smem, st>>>(a, cols);
+        p.kernel<<<grid, THREADS, p.smem, st>>>(a, p.cols);
         gp_time_end(GP_KERNEL_SCORING, st);
-        GP_CUDA(cudaGetLastError());
         CombArgs ca;
-        ca.hrec = d_rec; ca.tile_list = d_lists; ca.partner = d_lists + tiles.size(); ca.class_sym = s->d_class_sym;
-        ca.pheno = d_pheno; ca.gap = d_gap; ca.list_first = first; ca.n_images = n_img;
-        ca.fb = fb; ca.k = k; ca.N = N; ca.threshold = hp.threshold;
+        ca.hrec = d_rec; ca.units = s->d_units; ca.class_sym = s->d_class_sym;
+        ca.pheno = d_pheno; ca.gap = d_gap; ca.unit_first = u; ca.n_images = n_img; ca.paired = paired; ca.mid = mid;
+        ca.fb = fb; ca.k = k; ca.N = N; ca.threshold = hp.threshold; ca.compact = compact; ca.compact_base = images_done << fb;
+        images_done += n_img;
         const uint64_t work = ((uint64_t)n_img << fb) / 256;
-        combine_kernel<<<(unsigned)(work < (uint64_t)sms * 8 ? (work ? work : 1) : (uint64_t)sms * 8), 256, 0, st>>>(ca);
-        GP_CUDA(cudaGetLastError());
+        combine_kernel<<<(unsigned)(work < (uint64_t)p.sms * 8 ? (work ? work : 1) : (uint64_t)p.sms * 8), 256, 0, st>>>(ca);
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) { gp_set_cuda_error(e, "map launch"); result = GP_CUDA_ERROR; break; }
         gp_count_launches(3);
+        u = stop;
     }
-    GP_CUDA(cudaFreeAsync(d_lists, st));
-    return GP_OK;
+    cudaFreeAsync(d_work, st);
+    return result;
 }
 
-extern "C" gp_status gp_enumerate_map(const gp_structures_t* s_, const gp_energies* en, uint16_t* d_pheno, int16_t* d_gap,
-                                      void* stream) {
-    gp_structures_s* s = const_cast<gp_structures_s*>(s_);
+extern "C" uint64_t gp_map_range_genotypes(const gp_structures_t* s, uint64_t unit_first, uint64_t unit_count) {
+    if (!s || unit_first > s->n_units || unit_count > s->n_units - unit_first) return 0;
+    if (!s->map_k) return unit_count ? 1ULL << s->N : 0;
+    const uint64_t end = unit_first + unit_count;
+    const uint64_t pairs = unit_first < s->n_pair_units ? (end < s->n_pair_units ? end : s->n_pair_units) - unit_first : 0;
+    return (2 * pairs + (unit_count - pairs)) << (2 * s->map_k);
+}
+
+extern "C" gp_status gp_enumerate_map_range(const gp_structures_t* s, const gp_energies* en, uint64_t unit_first,
+                                            uint64_t unit_count, uint16_t* d_pheno, int16_t* d_gap, int layout,
+                                            void* stream) {
     gp_hp_params hp;
     gp_status stt = gp_check_hp(s, en, &hp);
     if (stt != GP_OK) return stt;
-    if (!d_pheno) return GP_INVALID_ARG;
+    if (!d_pheno || (layout != GP_MAP_FULL_STORE && layout != GP_MAP_COMPACT)) return GP_INVALID_ARG;
+    if (unit_first > s->n_units || unit_count > s->n_units - unit_first) return GP_RANGE;
     if (s->device < 0) { gp_set_cuda_error(cudaErrorNoDevice, "handle has no device tables"); return GP_CUDA_ERROR; }
     if (s->N >= 64) return GP_UNSUPPORTED_LATTICE;
-    stt = gp_launch_map_tc(s, hp, d_pheno, d_gap, (cudaStream_t)stream);
-    if (stt == GP_UNSUPPORTED_LATTICE)  // chains shorter than 10 monomers: the prefix path covers the map in one image
+    if (unit_count == 0) return GP_OK;
+    if (!s->map_k)  // chains too short for the scheme: the single unit is the whole map on the prefix path
         return gp_launch_scoring_tc(s, hp, 0, 1ULL << s->N, d_pheno, d_gap, (cudaStream_t)stream);
-    return stt;
+    return gp_launch_map_range(s, hp, unit_first, unit_count, d_pheno, d_gap, layout == GP_MAP_COMPACT, (cudaStream_t)stream);
+}
+
+extern "C" gp_status gp_enumerate_map(const gp_structures_t* s, const gp_energies* en, uint16_t* d_pheno, int16_t* d_gap,
+                                      void* stream) {
+    if (!s) return GP_INVALID_ARG;
+    return gp_enumerate_map_range(s, en, 0, s->n_units, d_pheno, d_gap, GP_MAP_FULL_STORE, stream);
 }
 
 // Explicit HP sequences on the tensor cores (sequence_kernel).  GP_UNSUPPORTED_LATTICE = this lattice needs more than
-// 384 columns or is too small to be worth it: the caller falls back to the CUDA-core kernel.
-gp_status gp_launch_sequences_tc(gp_structures_s* s, const gp_hp_params& hp, const uint8_t* d_seqs, uint64_t count,
+// 384 columns: the caller falls back to the CUDA-core kernel.
+gp_status gp_launch_sequences_tc(const gp_structures_s* s, const gp_hp_params& hp, const uint8_t* d_seqs, uint64_t count,
                                  uint16_t* d_pheno, int16_t* d_gap, cudaStream_t st) {
     using namespace tc;
     const int ncol = 2 + s->N + s->P;
     if (ncol > SQ_MAXCOL || s->N > 62 || s->D >= (1u << KEY_SHIFT)) return GP_UNSUPPORTED_LATTICE;
     const uint32_t n_tiles = (s->D + TN - 1) / TN;
-    if (!s->wimg.valid || s->wimg.lin != hp.lin || s->wimg.quad != hp.quad) {
-        if (!s->wimg.d_img) GP_CUDA(cudaMalloc(&s->wimg.d_img, (size_t)n_tiles * SQ_TILE));
-        SqImgArgs ia;
-        ia.contacts = s->d_contacts; ia.pairidx = s->d_pairidx; ia.img = s->wimg.d_img; ia.D = s->D;
-        ia.N = s->N; ia.NBP = s->NBP; ia.lin = hp.lin; ia.quad = hp.quad;
-        build_full_image_kernel<<<n_tiles, TN, 0, st>>>(ia);
-        GP_CUDA(cudaGetLastError());
-        gp_count_launches(1);
-        s->wimg.lin = hp.lin; s->wimg.quad = hp.quad; s->wimg.valid = true; s->wimg.n_tiles = n_tiles; s->wimg.k_blocks = SQ_KB;
+    // weight image of (lin, quad): cached in the handle, immutable once built; other streams wait on its event
+    const int8_t* d_img = nullptr;
+    int8_t* d_private = nullptr;  // cache full: a per-call image from the stream-ordered pool
+    {
+        std::lock_guard<std::mutex> lk(s->mu);
+        for (const gp_weight_image& w : s->wimgs)
+            if (w.lin == hp.lin && w.quad == hp.quad) {
+                GP_CUDA(cudaStreamWaitEvent(st, (cudaEvent_t)w.ready, 0));
+                d_img = w.d_img;
+            }
+        if (!d_img) {
+            gp_weight_image w;
+            w.lin = hp.lin; w.quad = hp.quad;
+            const bool cache = s->wimgs.size() < 8;
+            if (cache) GP_CUDA(cudaMalloc(&w.d_img, (size_t)n_tiles * SQ_TILE));  // first use of these energies only
+            else { GP_CUDA(cudaMallocAsync(&d_private, (size_t)n_tiles * SQ_TILE, st)); w.d_img = d_private; }
+            SqImgArgs ia;
+            ia.contacts = s->d_contacts; ia.pairidx = s->d_pairidx; ia.img = w.d_img; ia.D = s->D;
+            ia.N = s->N; ia.NBP = s->NBP; ia.lin = hp.lin; ia.quad = hp.quad;
+            build_full_image_kernel<<<n_tiles, TN, 0, st>>>(ia);
+            GP_CUDA(cudaGetLastError());
+            gp_count_launches(1);
+            if (cache) {
+                cudaEvent_t ev;
+                GP_CUDA(cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
+                GP_CUDA(cudaEventRecord(ev, st));
+                w.ready = ev;
+                s->wimgs.push_back(w);
+            }
+            d_img = w.d_img;
+        }
     }
     SqCols cols;
     for (int c = 0; c < SQ_MAXCOL; c++) cols.i[c] = cols.j[c] = 62;  // bit 62 of the letter word is always 0
@@ -1048,7 +1104,7 @@ gp_status gp_launch_sequences_tc(gp_structures_s* s, const gp_hp_params& hp, con
     const size_t smem = (size_t)(SQ_MT + SQ_STAGES) * SQ_TILE + sizeof(SqBarriers) + sizeof(SqCols) + 1024 + 64;
     GP_CUDA(cudaFuncSetAttribute(sequence_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     SqArgs a;
-    a.img = s->wimg.d_img; a.class_of = s->d_class_of; a.seqs = d_seqs; a.pheno = d_pheno; a.gap = d_gap; a.count = count;
+    a.img = d_img; a.class_of = s->d_class_of; a.seqs = d_seqs; a.pheno = d_pheno; a.gap = d_gap; a.count = count;
     a.n_items = (uint32_t)((count + SQ_ROWS - 1) / SQ_ROWS); a.n_tiles = n_tiles;
     a.N = s->N; a.ksteps = (ncol + 31) / 32; a.threshold = hp.threshold;
     const unsigned grid = a.n_items < (uint32_t)sms ? a.n_items : (uint32_t)sms;
@@ -1057,14 +1113,14 @@ gp_status gp_launch_sequences_tc(gp_structures_s* s, const gp_hp_params& hp, con
     gp_time_end(GP_KERNEL_SCORING, st);
     GP_CUDA(cudaGetLastError());
     gp_count_launches(1);
+    if (d_private) GP_CUDA(cudaFreeAsync(d_private, st));
     return GP_OK;
 }
 
 extern "C" uint64_t gp_tile(void) { return tc::SUPER; }
 
-extern "C" gp_status gp_enumerate(const gp_structures_t* s_, const gp_energies* en, uint64_t g_begin, uint64_t g_count,
+extern "C" gp_status gp_enumerate(const gp_structures_t* s, const gp_energies* en, uint64_t g_begin, uint64_t g_count,
                                   uint16_t* d_pheno, int16_t* d_gap, void* stream) {
-    gp_structures_s* s = const_cast<gp_structures_s*>(s_);
     gp_hp_params hp;
     gp_status stt = gp_check_hp(s, en, &hp);
     if (stt != GP_OK) return stt;
@@ -1074,4 +1130,54 @@ extern "C" gp_status gp_enumerate(const gp_structures_t* s_, const gp_energies* 
     if (s->device < 0) { gp_set_cuda_error(cudaErrorNoDevice, "handle has no device tables"); return GP_CUDA_ERROR; }
     if (g_count == 0) return GP_OK;
     return gp_launch_scoring_tc(s, hp, g_begin, g_count, d_pheno, d_gap, (cudaStream_t)stream);
+}
+
+// Measured int8 MMA-only peak (include/gpmap.h).  Synchronous.
+extern "C" gp_status gp_probe_i8_peak(int k_steps, double seconds, double* ops_per_s, double* clk_per_mma, double* sm_mhz) {
+    using namespace tc;
+    if (k_steps < 1 || k_steps > 4 || !(seconds > 0) || seconds > 30 || !ops_per_s) return GP_INVALID_ARG;
+    int dev = 0, sms = 0;
+    GP_CUDA(cudaGetDevice(&dev));
+    GP_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    typedef void (*probe_fn)(uint32_t, unsigned long long*);
+    const probe_fn fn = k_steps == 1 ? mma_probe_kernel<1, 64> : k_steps == 2 ? mma_probe_kernel<2, 64>
+                      : k_steps == 3 ? mma_probe_kernel<3, 128> : mma_probe_kernel<4, 128>;
+    const size_t smem = 2 * (size_t)TM * (k_steps <= 2 ? 64 : 128) + 1024;
+    GP_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    unsigned long long* d_cycles = nullptr;
+    GP_CUDA(cudaMalloc(&d_cycles, sms * sizeof(unsigned long long)));
+    cudaEvent_t e0, e1;
+    GP_CUDA(cudaEventCreate(&e0));
+    GP_CUDA(cudaEventCreate(&e1));
+    const uint32_t mma_per_group = (64 / k_steps) * k_steps;
+    uint32_t groups = 2000;  // ~4 ms; then scaled to the requested duration
+    float ms = 0;
+    gp_status st = GP_OK;
+    for (int round = 0; round < 2 && st == GP_OK; round++) {
+        cudaEventRecord(e0, 0);
+        fn<<<sms, 128, smem, 0>>>(groups, d_cycles);
+        cudaEventRecord(e1, 0);
+        cudaError_t e = cudaEventSynchronize(e1);
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+        if (e != cudaSuccess) { gp_set_cuda_error(e, "gp_probe_i8_peak"); st = GP_CUDA_ERROR; break; }
+        gp_count_launches(1);
+        if (round == 0) {
+            double want = groups * (seconds * 1e3 / (ms > 0.01f ? ms : 0.01f));
+            groups = (uint32_t)(want < 4 ? 4 : want > 4e8 ? 4e8 : want);
+        }
+    }
+    if (st == GP_OK) {
+        std::vector<unsigned long long> cyc(sms);
+        cudaMemcpy(cyc.data(), d_cycles, sms * sizeof(unsigned long long), cudaMemcpyDeviceToHost);
+        double mean = 0;
+        for (int i = 0; i < sms; i++) mean += (double)cyc[i] / sms;
+        const double mmas = (double)groups * mma_per_group;
+        *ops_per_s = mmas * sms * (2.0 * TM * TN * 32) / (ms * 1e-3);
+        if (clk_per_mma) *clk_per_mma = mean / mmas;
+        if (sm_mhz) *sm_mhz = mean / (ms * 1e-3) / 1e6;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(d_cycles);
+    return st;
 }

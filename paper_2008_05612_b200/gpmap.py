@@ -22,6 +22,11 @@ class _Energies(ctypes.Structure):
     _fields_ = [("alphabet", ctypes.c_int32), ("e", _i32p), ("threshold", ctypes.c_int32)]
 
 
+class _Tuning(ctypes.Structure):
+    _fields_ = [("fold_bits", ctypes.c_int32), ("sym_bits", ctypes.c_int32), ("narrow_rows", ctypes.c_int32),
+                ("seq_tensor", ctypes.c_int32)]
+
+
 # name -> (restype, argtypes); must list every symbol include/gpmap.h declares (tests/test_abi.py checks)
 SIGNATURES = {
     "gp_structures": (ctypes.c_int, [ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.POINTER(_vp)]),
@@ -34,9 +39,16 @@ SIGNATURES = {
     "gp_structures_contacts_per_fold": (ctypes.c_int, [_vp]),
     "gp_structures_features": (ctypes.c_int, [_vp]),
     "gp_structures_get": (ctypes.c_int, [_vp, ctypes.c_uint32, _u8p, _u8p, _u16p]),
+    "gp_tuning_get": (ctypes.c_int, [_vp, ctypes.POINTER(_Tuning)]),
+    "gp_tuning_set": (ctypes.c_int, [_vp, ctypes.POINTER(_Tuning)]),
     "gp_tile": (ctypes.c_uint64, []),
     "gp_enumerate": (ctypes.c_int, [_vp, ctypes.POINTER(_Energies), ctypes.c_uint64, ctypes.c_uint64, _vp, _vp, _vp]),
     "gp_enumerate_map": (ctypes.c_int, [_vp, ctypes.POINTER(_Energies), _vp, _vp, _vp]),
+    "gp_map_units": (ctypes.c_uint64, [_vp]),
+    "gp_map_unit": (ctypes.c_int, [_vp, ctypes.c_uint64, _u64p, ctypes.POINTER(ctypes.c_int)]),
+    "gp_map_range_genotypes": (ctypes.c_uint64, [_vp, ctypes.c_uint64, ctypes.c_uint64]),
+    "gp_enumerate_map_range": (ctypes.c_int, [_vp, ctypes.POINTER(_Energies), ctypes.c_uint64, ctypes.c_uint64, _vp, _vp,
+                                              ctypes.c_int, _vp]),
     "gp_enumerate_simple": (ctypes.c_int, [_vp, ctypes.POINTER(_Energies), ctypes.c_uint64, ctypes.c_uint64, _vp, _vp, _vp]),
     "gp_enumerate_seqs": (ctypes.c_int, [_vp, ctypes.POINTER(_Energies), _vp, ctypes.c_uint64, _vp, _vp, _vp]),
     "gp_enumerate_seeded": (ctypes.c_int, [_vp, ctypes.POINTER(_Energies), ctypes.c_uint64, ctypes.c_uint64,
@@ -45,6 +57,12 @@ SIGNATURES = {
     "gp_seeded_sequences": (ctypes.c_int, [ctypes.c_uint64, ctypes.c_uint64, ctypes.c_uint64, ctypes.c_int, _u8p]),
     "gp_designability": (ctypes.c_int, [_vp, ctypes.c_uint64, ctypes.c_uint32, _vp, _vp]),
     "gp_robustness": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_uint32, _vp, _vp, _vp, _vp, _vp]),
+    "gp_pair_bitmap_words": (ctypes.c_uint64, [ctypes.c_uint32]),
+    "gp_robustness_partial": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_uint32, _vp, _vp, _vp, _vp, ctypes.c_int, _vp]),
+    "gp_robustness_cross": (ctypes.c_int, [_vp, _vp, ctypes.c_uint64, ctypes.c_uint32, _vp, _vp, _vp, _vp, _vp]),
+    "gp_pair_bitmap_or": (ctypes.c_int, [_vp, _vp, ctypes.c_uint32, _vp]),
+    "gp_pair_bitmap_count": (ctypes.c_int, [_vp, ctypes.c_uint32, _vp, _vp]),
+    "gp_threshold_sweep": (ctypes.c_int, [_vp, _vp, ctypes.c_uint64, ctypes.c_uint32, _i32p, ctypes.c_int, _vp, _vp, _vp]),
     "gp_phi_row": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_uint32, ctypes.c_uint32, _vp, _vp]),
     "gp_nn_components": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_uint32, _vp, _vp]),
     "gp_enumerate_host": (ctypes.c_int, [_vp, ctypes.POINTER(_Energies), ctypes.c_uint64, ctypes.c_uint64, _vp, _u64p,
@@ -52,6 +70,8 @@ SIGNATURES = {
     "gp_launch_count": (ctypes.c_uint64, []),
     "gp_kernel_timing": (None, [ctypes.c_int]),
     "gp_kernel_time": (ctypes.c_int, [ctypes.c_int, ctypes.POINTER(ctypes.c_double), _u64p]),
+    "gp_probe_i8_peak": (ctypes.c_int, [ctypes.c_int, ctypes.c_double, ctypes.POINTER(ctypes.c_double),
+                                        ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]),
     "gp_strerror": (ctypes.c_char_p, [ctypes.c_int]),
     "gp_last_cuda_error": (ctypes.c_char_p, []),
 }
@@ -69,11 +89,6 @@ def lib():
             f = getattr(L, name)
             f.restype = res
             f.argtypes = args
-        L.gp_set_fold_bits.restype = ctypes.c_int
-        L.gp_set_fold_bits.argtypes = [ctypes.c_int]
-        for hook in ("gp_set_narrow", "gp_set_seq_tc", "gp_set_sym_bits", "gp_set_rob_tile_bits", "gp_set_pack", "gp_set_halves", "gp_set_debug"):  # test / tuning hooks
-            getattr(L, hook).restype = ctypes.c_int
-            getattr(L, hook).argtypes = [ctypes.c_int]
         _lib = L
     return _lib
 
@@ -143,10 +158,12 @@ def kernel_time(which):
     return ms.value, n.value
 
 
-def set_fold_bits(fb):
-    """Tuning/test hook: number of low genotype bits kept as contraction columns (9..22, default 15)."""
-    if lib().gp_set_fold_bits(fb) != 0:
-        raise ValueError("fold bits must be in 9..22")
+def probe_i8_peak(k_steps=2, seconds=0.5):
+    """gp_probe_i8_peak: (int8 ops/s of the MMA-only stream, SM clocks per MMA, SM MHz it ran at)."""
+    ops, clk, mhz = ctypes.c_double(), ctypes.c_double(), ctypes.c_double()
+    _check(lib().gp_probe_i8_peak(k_steps, seconds, ctypes.byref(ops), ctypes.byref(clk), ctypes.byref(mhz)),
+           "gp_probe_i8_peak")
+    return ops.value, clk.value, mhz.value
 
 
 class Structures:
@@ -172,6 +189,31 @@ class Structures:
             self._h = None
 
     __del__ = close
+
+    def tuning(self):
+        """gp_tuning_get as a dict."""
+        t = _Tuning()
+        _check(lib().gp_tuning_get(self._h, ctypes.byref(t)), "gp_tuning_get")
+        return {k: getattr(t, k) for k, _ in _Tuning._fields_}
+
+    def tune(self, **kw):
+        """gp_tuning_set: change some fields of the handle's gp_tuning (fold_bits, sym_bits, narrow_rows, seq_tensor)."""
+        cur = self.tuning()
+        for k in kw:
+            if k not in cur:
+                raise ValueError("unknown tuning field %s" % k)
+        cur.update(kw)
+        _check(lib().gp_tuning_set(self._h, ctypes.byref(_Tuning(**cur))), "gp_tuning_set")
+
+    def map_units(self):
+        return int(lib().gp_map_units(self._h))
+
+    def map_unit(self, unit):
+        """(m, k) of a unit of gp_enumerate_map_range: middle-bit value and free monomers per chain end (k = 0: the
+        single unit is the whole map)."""
+        m, k = ctypes.c_uint64(), ctypes.c_int()
+        _check(lib().gp_map_unit(self._h, unit, ctypes.byref(m), ctypes.byref(k)), "gp_map_unit")
+        return m.value, k.value
 
     def get(self, d):
         sites = np.zeros(self.N, np.uint8)
@@ -210,11 +252,41 @@ class Structures:
         _check(lib().gp_enumerate_map(self._h, ctypes.byref(en), _dptr(pheno, torch.uint16), _dptr(gap, torch.int16),
                                       _stream(stream)), "gp_enumerate_map")
 
+    def map_range_genotypes(self, unit_first, unit_count):
+        """Genotype integers of a unit range in the order of the compact layout (uint64 numpy array).  Index
+        arithmetic of include/gpmap.h only: image m of a unit holds g = (hi << (N-k)) | (m << k) | lo."""
+        out = []
+        for u in range(unit_first, unit_first + unit_count):
+            m, k = self.map_unit(u)
+            if k == 0:
+                return np.arange(1 << self.N, dtype=np.uint64)
+            mid = self.N - 2 * k
+            rev = int(format(m, "0%db" % mid)[::-1], 2) if mid else 0
+            t = np.arange(1 << (2 * k), dtype=np.uint64)
+            for mm in ([m] if rev == m else [m, rev]):
+                out.append(((t >> np.uint64(k)) << np.uint64(self.N - k)) | np.uint64(mm << k) | (t & np.uint64((1 << k) - 1)))
+        return np.concatenate(out) if out else np.zeros(0, np.uint64)
+
+    def enumerate_map_range(self, unit_first, unit_count, pheno, gap=None, e=HP_ENERGIES, threshold=1, compact=False,
+                            stream=None):
+        """gp_enumerate_map_range: units [unit_first, unit_first+unit_count) of the map, into the FULL 2^N store or
+        (compact=True) into gp_map_range_genotypes entries ordered like map_range_genotypes()."""
+        import torch
+        en = _energies(e, 2, threshold)
+        need = int(lib().gp_map_range_genotypes(self._h, unit_first, unit_count)) if compact else 1 << self.N
+        if pheno.numel() < need or (gap is not None and gap.numel() < need) or (not compact and pheno.numel() != need):
+            raise ValueError("gp_enumerate_map_range: output holds %d entries, needs %d" % (pheno.numel(), need))
+        _check(lib().gp_enumerate_map_range(self._h, ctypes.byref(en), unit_first, unit_count, _dptr(pheno, torch.uint16),
+                                            _dptr(gap, torch.int16), 1 if compact else 0, _stream(stream)),
+               "gp_enumerate_map_range")
+
     def enumerate_seqs(self, seqs, pheno, gap=None, e=None, alphabet=20, threshold=1, stream=None):
         import torch
         en = _energies(e, alphabet, threshold)
         if seqs.dim() != 2 or seqs.shape[1] != self.N:
             raise ValueError("seqs must be [count, N] uint8")
+        if pheno.numel() < seqs.shape[0] or (gap is not None and gap.numel() < seqs.shape[0]):
+            raise ValueError("output tensor too small")
         _check(lib().gp_enumerate_seqs(self._h, ctypes.byref(en), _dptr(seqs, torch.uint8), seqs.shape[0],
                                        _dptr(pheno, torch.uint16), _dptr(gap, torch.int16), _stream(stream)),
                "gp_enumerate_seqs")
@@ -277,6 +349,61 @@ def robustness(pheno, n_bits, n_classes, want_pairs=True, stream=None):
     _check(lib().gp_robustness(_dptr(pheno, torch.uint16), n_bits, n_classes, _dptr(out[0]), _dptr(out[1]), _dptr(out[2]),
                                _dptr(pc), _stream(stream)), "gp_robustness")
     return out[0], out[1], out[2], pc
+
+
+def pair_bitmap(n_classes, device="cuda"):
+    """A zeroed pair bitmap (int32[gp_pair_bitmap_words]) for gp_robustness_partial / _cross."""
+    import torch
+    return torch.zeros(int(lib().gp_pair_bitmap_words(n_classes)), dtype=torch.int32, device=device)
+
+
+def robustness_partial(pheno, n_bits, n_classes, rdo, bitmap=None, tile_bits=0, stream=None):
+    """gp_robustness_partial: ADD the counts of the n_bits local flips of a sub-cube store into rdo (int64[3, C]) and
+    OR its connected pairs into bitmap."""
+    import torch
+    if pheno.numel() != 1 << n_bits:
+        raise ValueError("gp_robustness_partial needs a store of 2^n_bits entries")
+    _check(lib().gp_robustness_partial(_dptr(pheno, torch.uint16), n_bits, n_classes, _dptr(rdo[0], torch.int64),
+                                       _dptr(rdo[1], torch.int64), _dptr(rdo[2], torch.int64), _dptr(bitmap, torch.int32),
+                                       tile_bits, _stream(stream)), "gp_robustness_partial")
+
+
+def robustness_cross(mine, partner, n_classes, rdo, bitmap=None, stream=None):
+    """gp_robustness_cross: entries i of `mine` and `partner` differ in one shard-selecting bit; counts go to mine."""
+    import torch
+    if mine.numel() != partner.numel():
+        raise ValueError("shards differ in size")
+    _check(lib().gp_robustness_cross(_dptr(mine, torch.uint16), _dptr(partner, torch.uint16), mine.numel(), n_classes,
+                                     _dptr(rdo[0], torch.int64), _dptr(rdo[1], torch.int64), _dptr(rdo[2], torch.int64),
+                                     _dptr(bitmap, torch.int32), _stream(stream)), "gp_robustness_cross")
+
+
+def pair_bitmap_or(dst, src, n_classes, stream=None):
+    import torch
+    _check(lib().gp_pair_bitmap_or(_dptr(dst, torch.int32), _dptr(src, torch.int32), n_classes, _stream(stream)),
+           "gp_pair_bitmap_or")
+
+
+def pair_bitmap_count(bitmap, n_classes, stream=None):
+    import torch
+    out = torch.empty(1, dtype=torch.int64, device=bitmap.device)
+    _check(lib().gp_pair_bitmap_count(_dptr(bitmap, torch.int32), n_classes, _dptr(out, torch.int64), _stream(stream)),
+           "gp_pair_bitmap_count")
+    return out
+
+
+def threshold_sweep(pheno, gap, n_classes, thresholds, stream=None):
+    """gp_threshold_sweep: (folding int64[T], hist int64[T, C+1]) from the threshold-1 (pheno, gap) stores."""
+    import torch
+    thr = np.ascontiguousarray(thresholds, np.int32)
+    if gap.numel() != pheno.numel():
+        raise ValueError("pheno and gap differ in size")
+    folding = torch.empty(thr.size, dtype=torch.int64, device=pheno.device)
+    hist = torch.empty((thr.size, n_classes + 1), dtype=torch.int64, device=pheno.device)
+    _check(lib().gp_threshold_sweep(_dptr(pheno, torch.uint16), _dptr(gap, torch.int16), pheno.numel(), n_classes,
+                                    thr.ctypes.data_as(_i32p), thr.size, _dptr(folding), _dptr(hist), _stream(stream)),
+           "gp_threshold_sweep")
+    return folding, hist
 
 
 def phi_row(pheno, n_bits, n_classes, q, stream=None):

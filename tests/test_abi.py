@@ -30,10 +30,52 @@ def test_library_builds_and_exports_every_declared_symbol():
 
 
 def test_library_contains_sm100a_tensor_core_code():
-    """The scoring kernel is tcgen05 code for sm_100a (PTX mnemonics are checked; SASS needs cuobjdump)."""
-    src = open(os.path.join(gbuild.CSRC, "scoring_tc.cu")).read()
-    assert "tcgen05.mma.cta_group::1.kind::i8" in src and "cp.async.bulk" in src and "tcgen05.ld" in src
-    assert "arch=compute_100a,code=sm_100a" in " ".join(gbuild.NVCC_FLAGS)
+    """The BUILT library holds sm_100a tensor-core machine code: cuobjdump of libgpmap.so must show the int8 tcgen05
+    MMA (UTCIMMA), TMEM loads (LDTM), TMA bulk copies (UBLKCP) and tcgen05 commits (UTCBAR) in the scoring kernels."""
+    import shutil
+    import subprocess
+    path = gbuild.build()
+    tool = shutil.which("cuobjdump") or "/usr/local/cuda/bin/cuobjdump"
+    sass = subprocess.run([tool, "-sass", path], capture_output=True, text=True, check=True).stdout
+    assert "sm_100a" in sass
+    counts = {op: len(re.findall(r"\b%s\b" % op, sass)) for op in ("UTCIMMA", "LDTM", "UBLKCP", "UTCBAR")}
+    assert all(v > 0 for v in counts.values()), counts
+    kernels = re.findall(r"Function : (\S+)", sass)
+    assert any("scoring_kernel" in k for k in kernels) and any("sequence_kernel" in k for k in kernels)
+    assert any("mma_probe_kernel" in k for k in kernels)
+
+
+def test_tuning_and_map_units_host_side():
+    """gp_tuning round trip and the unit table of gp_enumerate_map_range (host logic, no GPU): units are the m <= rev m,
+    pairs first; every genotype of the map belongs to exactly one unit."""
+    S = gpmap.Structures(4, 4)
+    assert S.tuning() == dict(fold_bits=15, sym_bits=7, narrow_rows=1, seq_tensor=1)
+    for bad in (dict(fold_bits=8), dict(fold_bits=23), dict(sym_bits=4), dict(sym_bits=12), dict(narrow_rows=2)):
+        with pytest.raises(gpmap.GpError) as ei:
+            S.tune(**bad)
+        assert ei.value.status == 1 and S.tuning()["fold_bits"] == 15
+    for k in (5, 6, 7, 8):
+        S.tune(sym_bits=k)
+        U = S.map_units()
+        mid = 16 - 2 * k
+        ms = [S.map_unit(u) for u in range(U)]
+        assert all(kk == k for _, kk in ms)
+        rev = lambda m: int(format(m, "0%db" % mid)[::-1], 2) if mid else 0
+        pal = [m for m, _ in ms if rev(m) == m]
+        assert [m for m, _ in ms][len(ms) - len(pal):] == sorted(pal) and len(pal) == 1 << ((mid + 1) // 2)
+        assert sorted([m for m, _ in ms] + [rev(m) for m, _ in ms if rev(m) != m]) == list(range(1 << mid))
+        g = S.map_range_genotypes(0, U)
+        assert g.size == 1 << 16 and np.array_equal(np.sort(g), np.arange(1 << 16, dtype=np.uint64))
+        assert int(gpmap.lib().gp_map_range_genotypes(S._h, 0, U)) == 1 << 16
+        assert int(gpmap.lib().gp_map_range_genotypes(S._h, U, 1)) == 0
+    S.close()
+    S3 = gpmap.Structures(3, 3)                 # N = 9: too short for the scheme, one unit = the whole map
+    assert S3.map_units() == 1 and S3.map_unit(0) == (0, 0)
+    assert int(gpmap.lib().gp_map_range_genotypes(S3._h, 0, 1)) == 512
+    S3.close()
+    S6 = gpmap.Structures(6, 6)
+    assert S6.map_units() == (1 << 21) + (1 << 10)
+    S6.close()
 
 
 def test_status_strings_and_tile():
@@ -84,6 +126,9 @@ def test_bad_arguments():
     assert L.gp_enumerate(S._h, ctypes.byref(en), 0, 512, ctypes.c_void_p(16), None, None) == 1
     en = gpmap._energies((0, -100, -100, -23), 2, 1)  # weights beyond int8
     assert L.gp_enumerate(S._h, ctypes.byref(en), 0, 512, ctypes.c_void_p(16), None, None) == 1
+    en = gpmap._energies((0, -10, -10, -60), 2, 1)    # lin and quad fit, their sum over three contacts does not
+    assert L.gp_enumerate(S._h, ctypes.byref(en), 0, 512, ctypes.c_void_p(16), None, None) == 1
+    assert L.gp_enumerate_map_range(S._h, ctypes.byref(en), 0, 1, ctypes.c_void_p(16), None, 0, None) == 1
     en = gpmap._energies(gpmap.HP_ENERGIES, 2, 0)  # threshold < 1
     assert L.gp_enumerate(S._h, ctypes.byref(en), 0, 512, ctypes.c_void_p(16), None, None) == 1
     en = gpmap._energies(gpmap.HP_ENERGIES, 2, 1)
@@ -97,5 +142,6 @@ def test_seeded_generator_matches_recipe():
     for seed in (200805612, 1, 2 ** 63 + 5):
         assert np.array_equal(gpmap.seeded_matrix(seed), orc.seeded_matrix(seed))
         assert np.array_equal(gpmap.seeded_sequences(seed, 12345, 300, 16), orc.seeded_sequences(seed, 12345, 300, 16))
+        assert np.array_equal(gpmap.seeded_sequences(seed, 1 << 40, 50, 36), orc.seeded_sequences(seed, 1 << 40, 50, 36))
     M = gpmap.seeded_matrix(200805612)
     assert M.min() >= -750 and M.max() <= -50 and np.array_equal(M, M.T)

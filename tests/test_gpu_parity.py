@@ -57,7 +57,7 @@ def test_ranges_5x5(oracle_structures, simple):
 def test_fold_bits_do_not_change_results(oracle_structures, fb):
     """Prefix folding is exact: any split between folded prefix and contraction columns gives the same map."""
     S, O = lib_structures((5, 5, 1)), oracle_structures(5, 5)
-    gpmap.set_fold_bits(fb)
+    S.tune(fold_bits=fb)
     try:
         for begin, count in [(0, 2048), ((1 << 24) + (1 << fb) - 512, 1536), ((1 << 25) - 2048, 2048)]:
             ph, gap = gpu_enumerate(S, begin, count)
@@ -65,7 +65,7 @@ def test_fold_bits_do_not_change_results(oracle_structures, fb):
             assert np.array_equal(ph, ph_o), (fb, begin)
             assert np.array_equal(gap.astype(np.int32), gap_o), (fb, begin)
     finally:
-        gpmap.set_fold_bits(15)
+        S.tune(fold_bits=15)
 
 
 @pytest.mark.parametrize("dims,n_ranges,length", [((6, 6, 1), 4, 1024), ((3, 3, 3), 3, 512)])
@@ -244,24 +244,23 @@ def test_robustness_tile_sizes_agree_with_oracle(tile_bits):
     """The bit-tiled neighbour pass gives the same counts for every tile size (small tiles force the multi-pass,
     spread-bit path on small stores), on stores whose size is not a multiple of the pass width."""
     rng = np.random.default_rng(11)
-    L = gpmap.lib()
-    assert L.gp_set_rob_tile_bits(tile_bits) == 0
-    try:
-        for n_bits, C, p_null in [(1, 2, 0.3), (2, 3, 0.3), (3, 5, 0.5), (9, 3, 0.4), (13, 549, 0.6), (18, 28728, 0.57)]:
-            n = 1 << n_bits
-            store = rng.integers(0, C, size=n).astype(np.uint16)
-            # clustered classes, so that neutral neighbours and equal-class runs exist
-            store = np.sort(store.reshape(-1, 4), axis=1).reshape(-1) if n >= 4 else store
-            store[rng.random(n) < p_null] = 0xFFFF
-            ph = torch.from_numpy(store.view(np.int16)).cuda().view(torch.uint16)
-            R, Dl, Oc, pc = gpmap.robustness(ph, n_bits, C)
-            Ro, Do, Oo, pco = orc.robustness(store, n_bits, C)
-            assert np.array_equal(R.cpu().numpy().astype(np.uint64), Ro), (tile_bits, n_bits)
-            assert np.array_equal(Dl.cpu().numpy().astype(np.uint64), Do), (tile_bits, n_bits)
-            assert np.array_equal(Oc.cpu().numpy().astype(np.uint64), Oo), (tile_bits, n_bits)
-            assert int(pc) == pco, (tile_bits, n_bits)
-    finally:
-        L.gp_set_rob_tile_bits(15)
+    for n_bits, C, p_null in [(1, 2, 0.3), (2, 3, 0.3), (3, 5, 0.5), (9, 3, 0.4), (13, 549, 0.6), (18, 28728, 0.57)]:
+        n = 1 << n_bits
+        store = rng.integers(0, C, size=n).astype(np.uint16)
+        # clustered classes, so that neutral neighbours and equal-class runs exist
+        store = np.sort(store.reshape(-1, 4), axis=1).reshape(-1) if n >= 4 else store
+        store[rng.random(n) < p_null] = 0xFFFF
+        ph = torch.from_numpy(store.view(np.int16)).cuda().view(torch.uint16)
+        rdo = torch.zeros((3, C), dtype=torch.int64, device="cuda")
+        bitmap = gpmap.pair_bitmap(C)
+        gpmap.robustness_partial(ph, n_bits, C, rdo, bitmap, tile_bits=tile_bits)
+        pc = gpmap.pair_bitmap_count(bitmap, C)
+        Ro, Do, Oo, pco = orc.robustness(store, n_bits, C)
+        got = rdo.cpu().numpy().astype(np.uint64)
+        assert np.array_equal(got[0], Ro), (tile_bits, n_bits)
+        assert np.array_equal(got[1], Do), (tile_bits, n_bits)
+        assert np.array_equal(got[2], Oo), (tile_bits, n_bits)
+        assert int(pc) == pco, (tile_bits, n_bits)
 
 
 @pytest.mark.parametrize("dims,k", [((2, 2, 1), 9), ((3, 3, 1), 9), ((4, 4, 1), 5), ((4, 4, 1), 6), ((4, 4, 1), 8),
@@ -271,14 +270,14 @@ def test_enumerate_map_whole_small_maps(oracle_structures, dims, k):
     sizes that give many image pairs, palindromic images and a single image; chains under 10 monomers fall back."""
     S, O = lib_structures(dims), oracle_structures(*dims)
     n = 1 << S.N
-    assert gpmap.lib().gp_set_sym_bits(k) == 0
+    S.tune(sym_bits=k)
     try:
         ph = torch.full((n,), 0x7777, dtype=torch.int32, device="cuda").to(torch.uint16)
         gap = torch.zeros(n, dtype=torch.int16, device="cuda")
         S.enumerate_map(ph, gap)
         torch.cuda.synchronize()
     finally:
-        gpmap.lib().gp_set_sym_bits(7)
+        S.tune(sym_bits=7)
     ph_o, gap_o = O.enumerate(0, n)
     assert np.array_equal(ph.cpu().numpy(), ph_o), dims
     assert np.array_equal(gap.cpu().numpy().astype(np.int32), np.maximum(gap_o, -32768)), dims
@@ -287,14 +286,14 @@ def test_enumerate_map_whole_small_maps(oracle_structures, dims, k):
 def test_enumerate_map_other_energies_and_threshold(oracle_structures):
     S, O = lib_structures((4, 4, 1)), oracle_structures(4, 4)
     n = 1 << 16
-    assert gpmap.lib().gp_set_sym_bits(6) == 0
+    S.tune(sym_bits=6)
     try:
         for e, thr in [((0, -10, -10, -23), 4), ((-3, 2, 2, -17), 1), ((5, -1, -1, 0), 2)]:
             ph = torch.empty(n, dtype=torch.uint16, device="cuda")
             S.enumerate_map(ph, None, e=e, threshold=thr)
             assert np.array_equal(ph.cpu().numpy(), O.enumerate(0, n, e=e, threshold=thr, want_gap=False)), (e, thr)
     finally:
-        gpmap.lib().gp_set_sym_bits(7)
+        S.tune(sym_bits=7)
 
 
 def test_bench_step_configuration_sampled(oracle_structures):
@@ -368,9 +367,9 @@ def test_explicit_hp_sequences_on_tensor_cores(oracle_structures, dims, count):
     a = torch.empty(1 << 15, dtype=torch.uint16, device="cuda")
     b = torch.empty_like(a)
     S.enumerate_seqs(d_big, a, None, e=e, alphabet=2, threshold=3)
-    gpmap.lib().gp_set_seq_tc(0)
+    S.tune(seq_tensor=0)
     try:
         S.enumerate_seqs(d_big, b, None, e=e, alphabet=2, threshold=3)
     finally:
-        gpmap.lib().gp_set_seq_tc(1)
+        S.tune(seq_tensor=1)
     assert torch.equal(a.view(torch.int16), b.view(torch.int16)), dims

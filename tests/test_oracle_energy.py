@@ -142,8 +142,13 @@ def test_generator():
     assert chi2 < 50.0                                    # 19 dof: P(chi2 > 50) ~ 1e-4
     again = orc.seeded_sequences(200805612, 1000, 10, 16)
     assert (again == seqs[1000:1010]).all()               # counter-based: ranges are slices
-    u = orc.draw(200805612, 5 * 16 + 3)
+    u = orc.draw(200805612, 5 * 64 + 3)
     assert seqs[5, 3] == ((u >> 32) * 20) >> 32
+    # chains longer than 16: consecutive sequences are independent draws, not sliding windows of one stream
+    long = orc.seeded_sequences(200805612, 0, 2000, 36)
+    for shift in (16, 32):
+        assert (long[:-1, shift:] == long[1:, :36 - shift]).mean() < 0.2
+    assert (long[:-2, 32:] == long[2:, :4]).mean() < 0.2
     M = orc.seeded_matrix(200805612)
     assert (M == M.T).all() and M.min() >= -750 and M.max() <= -50 and len(np.unique(M)) > 100
     u = orc.draw(200805612, (1 << 62) + 3 * 20 + 7)
