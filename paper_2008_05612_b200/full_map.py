@@ -1,10 +1,15 @@
-"""Whole GP map of one lattice on one GPU: phenotype store in HBM, designability, neighbour counts, pair count.
+"""Whole GP map of one lattice on one GPU, in resumable pieces: phenotype store in HBM, designability, neighbour counts,
+pair count.
 
-    python -m paper_2008_05612_b200.full_map --lattice 6x6 --out gpurun_out/map_6x6
+    python -m paper_2008_05612_b200.full_map --lattice 6x6 --out gpurun_out/map_6x6 [--chunks 64] [--resume]
 
-Scores all 2^N genotypes in chunks (progress lines go to <out>/progress.log), then runs gp_designability and
-gp_robustness over the resident store and checks the invariants that need no reference:
-sum(hist) = 2^N, sum(R+D+O) = N x folding, sum R and sum O even, pheno(rev g) = pheno(g) on a seeded sample.
+The map is scored as `chunks` ranges of units through gp_enumerate_map_range (include/gpmap.h; the paper's own 110-day
+job survived by appending results run by run).  After every chunk <out>/progress.json
+records the units done; with --checkpoint-store the store is also saved (<out>/store.u16, sensible up to 3x3x3), and
+--resume continues from the recorded unit instead of starting over.  Then gp_designability and gp_robustness run over
+the resident store and the invariants that need no reference are checked: sum(hist) = 2^N,
+sum(R+D+O) = N x folding, sum R and sum O even, pheno(rev g) = pheno(g) on a seeded sample
+(tests/test_gpu_map_range.py::test_full_map_run_survives_an_interruption compares such a run with the CPU oracle).
 Writes summary.json and counts.npz (hist, R, D, O).  6x6 needs 137.4 GB for the store (BASELINE.json configs[3])."""
 import argparse
 import json
@@ -23,41 +28,73 @@ def bit_reverse(g, n):
     return r
 
 
-def run(lattice, out, chunk_bits=30, sample=1 << 20, seed=200805612, keep_store=False, prefix_path=False):
+def run(lattice, out, chunks=64, sample=1 << 20, seed=200805612, keep_store=False, prefix_path=False, resume=False,
+        checkpoint_store=False, stop_after=None):
+    """stop_after = number of chunks after which the run stops as if interrupted (returns None); used by the tests."""
     import torch
     from . import gpmap
 
     os.makedirs(out, exist_ok=True)
-    log = open(os.path.join(out, "progress.log"), "w")
+    prog_path, store_path = os.path.join(out, "progress.json"), os.path.join(out, "store.u16")
+    S = gpmap.Structures(*LATTICES[lattice])
+    N, D, C = S.N, S.D, S.C
+    total = 1 << N
+    U = S.map_units()
+    chunks = max(1, min(chunks, U))
+    pheno = torch.empty(total, dtype=torch.uint16, device="cuda")
+    done_chunks, seconds_before = 0, 0.0
+    if resume and os.path.exists(prog_path):
+        with open(prog_path) as f:
+            prog = json.load(f)
+        same = (prog.get("lattice"), prog.get("chunks"), prog.get("units"), prog.get("prefix_path")) == (lattice, chunks, U, prefix_path)
+        if same and prog.get("store_saved") and os.path.exists(store_path):
+            pheno.copy_(torch.from_numpy(np.fromfile(store_path, dtype=np.int16)).view(torch.uint16))
+            done_chunks, seconds_before = prog["chunks_done"], prog.get("scoring_seconds", 0.0)
+    log = open(os.path.join(out, "progress.log"), "a" if done_chunks else "w")
 
     def say(msg):
         log.write("%.1f %s\n" % (time.time(), msg))
         log.flush()
 
-    S = gpmap.Structures(*LATTICES[lattice])
-    N, D, C = S.N, S.D, S.C
-    total = 1 << N
-    chunk = min(total, 1 << chunk_bits)
-    say("lattice %s N=%d D=%d C=%d store %.1f GB" % (lattice, N, D, C, 2.0 * total / 1e9))
-    pheno = torch.empty(total, dtype=torch.uint16, device="cuda")
-    ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
-    torch.cuda.synchronize()
+    say("lattice %s N=%d D=%d C=%d units=%d store %.1f GB, starting at chunk %d of %d" % (lattice, N, D, C, U, 2.0 * total / 1e9,
+                                                                                         done_chunks, chunks))
+    t_score = seconds_before
+    for c in range(done_chunks, chunks):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        if prefix_path:   # gp_enumerate on consecutive ranges: every genotype on all D directed structures
+            b0, b1 = total * c // chunks // 512 * 512, (total * (c + 1) // chunks // 512 * 512 if c + 1 < chunks else total)
+            S.enumerate(b0, b1 - b0, pheno[b0:b1])
+        else:             # reversal identity, one representative per class (C columns)
+            u0, u1 = U * c // chunks, U * (c + 1) // chunks
+            S.enumerate_map_range(u0, u1 - u0, pheno)
+        e1.record()
+        torch.cuda.synchronize()
+        t_score += e0.elapsed_time(e1) * 1e-3
+        prog = {"lattice": lattice, "chunks": chunks, "units": U, "prefix_path": prefix_path, "chunks_done": c + 1,
+                "scoring_seconds": t_score, "store_saved": False}
+        if checkpoint_store:
+            pheno.view(torch.int16).cpu().numpy().tofile(store_path + ".tmp")
+            os.replace(store_path + ".tmp", store_path)
+            prog["store_saved"] = True
+        with open(prog_path + ".tmp", "w") as f:
+            json.dump(prog, f)
+        os.replace(prog_path + ".tmp", prog_path)
+        if (c + 1) % 8 == 0 or c + 1 == chunks:
+            say("scored %d / %d chunks, %.1f s" % (c + 1, chunks, t_score))
+        if stop_after is not None and c + 1 - done_chunks >= stop_after and c + 1 < chunks:
+            say("stopped after %d chunks (as if interrupted)" % (c + 1))
+            log.close()
+            S.close()
+            return None
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
     ev[0].record()
-    if prefix_path:   # gp_enumerate on consecutive ranges: every genotype on all D directed structures
-        for b in range(0, total, chunk):
-            S.enumerate(b, chunk, pheno[b:b + chunk])
-            if (b // chunk) % 8 == 7:
-                torch.cuda.synchronize()
-                say("scored %d / %d chunks" % (b // chunk + 1, total // chunk))
-    else:             # gp_enumerate_map: reversal identity, one representative per class (C columns)
-        S.enumerate_map(pheno)
-    ev[1].record()
     hist = gpmap.designability(pheno, C)
-    ev[2].record()
+    ev[1].record()
     R, Dl, Oc, pairs = gpmap.robustness(pheno, N, C)
-    ev[3].record()
+    ev[2].record()
     torch.cuda.synchronize()
-    t_score, t_hist, t_rob = (ev[i].elapsed_time(ev[i + 1]) * 1e-3 for i in range(3))
+    t_hist, t_rob = (ev[i].elapsed_time(ev[i + 1]) * 1e-3 for i in range(2))
     say("scoring %.1f s, designability %.2f s, neighbour pass %.1f s" % (t_score, t_hist, t_rob))
 
     hist = hist.cpu().numpy().astype(np.uint64)
@@ -79,7 +116,8 @@ def run(lattice, out, chunk_bits=30, sample=1 << 20, seed=200805612, keep_store=
     order = np.argsort(hist[:C])[::-1]
     summary = {
         "lattice": lattice, "N": N, "D": D, "C": C, "genotypes": total, "evaluations": float(total) * D,
-        "path": "gp_enumerate (prefix tiles, D columns)" if prefix_path else "gp_enumerate_map (reversal identity, C columns)",
+        "path": "gp_enumerate (prefix tiles, D columns)" if prefix_path else "gp_enumerate_map_range (reversal identity, C columns)",
+        "chunks": chunks, "resumed_at_chunk": done_chunks,
         "evaluations_executed": float(total) * (D if prefix_path else C),
         "seconds": {"scoring": t_score, "designability": t_hist, "neighbour_pass": t_rob,
                     "total": t_score + t_hist + t_rob},
@@ -102,10 +140,14 @@ def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--lattice", default="6x6", choices=sorted(LATTICES))
     ap.add_argument("--out", default="gpurun_out/map")
-    ap.add_argument("--chunk-bits", type=int, default=30)
-    ap.add_argument("--prefix-path", action="store_true", help="score with gp_enumerate instead of gp_enumerate_map")
+    ap.add_argument("--chunks", type=int, default=64)
+    ap.add_argument("--resume", action="store_true", help="continue from <out>/progress.json (needs a saved store)")
+    ap.add_argument("--checkpoint-store", action="store_true", help="save the store after every chunk (up to 3x3x3)")
+    ap.add_argument("--prefix-path", action="store_true", help="score with gp_enumerate instead of gp_enumerate_map_range")
     a = ap.parse_args()
-    print(json.dumps(run(a.lattice, a.out, a.chunk_bits, prefix_path=a.prefix_path)))
+    summary = run(a.lattice, a.out, a.chunks, prefix_path=a.prefix_path, resume=a.resume, checkpoint_store=a.checkpoint_store)
+    print(json.dumps(summary))
+    raise SystemExit(0 if all(v is True or v == 0 for v in summary["checks"].values()) else 1)
 
 
 if __name__ == "__main__":

@@ -273,3 +273,29 @@ def test_small_explicit_hp_batches_take_the_cuda_core_branch(oracle_structures):
         S.enumerate_seqs(torch.from_numpy(seqs).cuda(), ph, gap, e=np.array(gpmap.HP_ENERGIES, np.int32), alphabet=2)
         ph_o, gap_o = O.enumerate_seqs(seqs, np.array(gpmap.HP_ENERGIES, np.int32), 2)
         assert np.array_equal(ph.cpu().numpy(), ph_o) and np.array_equal(gap.cpu().numpy().astype(np.int32), gap_o)
+
+
+@pytest.mark.parametrize("lattice,golden", [("5x5", "5x5")])
+def test_full_map_run_survives_an_interruption(oracle_structures, tmp_path, lattice, golden):
+    """full_map.run in 16 chunks of units, stopped after 5 chunks as if the job had died, resumed from progress.json and
+    the saved store (the paper's long run appended per run): the finished map equals the
+    oracle on seeded ranges, every count equals tests/golden/whole_maps.txt, and equals an uninterrupted run."""
+    from paper_2008_05612_b200 import full_map
+    from tests._golden import read_whole_maps
+    out = str(tmp_path / "map")
+    assert full_map.run(lattice, out, chunks=16, checkpoint_store=True, stop_after=5) is None
+    import json, os
+    prog = json.load(open(os.path.join(out, "progress.json")))
+    assert prog["chunks_done"] == 5 and prog["store_saved"]
+    summary, pheno, S = full_map.run(lattice, out, chunks=16, checkpoint_store=True, resume=True, keep_store=True)
+    assert summary["resumed_at_chunk"] == 5 and all(v is True or v == 0 for v in summary["checks"].values())
+    O = oracle_structures(*full_map.LATTICES[lattice])
+    for b, c in workloads.sample_ranges(S.N, 6, 2048, 512):
+        assert np.array_equal(pheno[b:b + c].cpu().numpy(), O.enumerate(b, c, want_gap=False)), b
+    gold = read_whole_maps()[golden]
+    assert (summary["folding"], summary["null"], summary["top5_designability"]) == (gold["folding"], gold["null"], gold["top5"])
+    assert (summary["sum_R"], summary["sum_D"], summary["sum_O"], summary["phenotype_pairs"]) == (
+        gold["sumR"], gold["sumD"], gold["sumO"], gold["pairs"])
+    once = full_map.run(lattice, str(tmp_path / "once"), chunks=3)
+    for key in ("folding", "sum_R", "sum_D", "sum_O", "phenotype_pairs", "top5_designability"):
+        assert once[key] == summary[key], key
