@@ -158,12 +158,18 @@ gp_status gp_designability(const uint16_t* d_pheno, uint64_t count, uint32_t n_c
 gp_status gp_robustness(const uint16_t* d_pheno, int n_bits, uint32_t n_classes, uint64_t* d_neutral,
                         uint64_t* d_deleterious, uint64_t* d_other, uint64_t* d_pair_count, void* stream);
 
+/* a5 + a6 in one sweep: the first pass of the neighbour kernel stages every phenotype on chip anyway, so it also counts
+ * them: d_hist (nullable; uint64[n_classes+1]) receives what gp_designability would write, the other outputs what
+ * gp_robustness writes, at one read of the store less.  Full store of 2^n_bits entries. */
+gp_status gp_reduce_store(const uint16_t* d_pheno, int n_bits, uint32_t n_classes, uint64_t* d_hist, uint64_t* d_neutral,
+                          uint64_t* d_deleterious, uint64_t* d_other, uint64_t* d_pair_count, void* stream);
+
 /* a6 in pieces, for stores sharded over several GPUs on the top genotype bits and for resumable runs.
  * All three ADD into d_neutral / d_deleterious / d_other (uint64[n_classes], zeroed by the caller) and OR into
  * d_pair_bitmap (nullable; gp_pair_bitmap_words(n_classes) uint32 words, zeroed by the caller; bit p*n_classes+q,
  * p < q, is set when classes p and q are joined by a mutation):
  *   gp_robustness_partial: the flips of the n_bits LOCAL bits of a sub-cube store of 2^n_bits entries (a shard, or
- *     the whole map).  tile_bits = 0 takes the default on-chip tile; 4..15 forces a tile of 2^tile_bits entries (any
+ *     the whole map).  tile_bits = 0 takes the default on-chip tile; 4..16 forces a tile of 2^tile_bits entries (any
  *     value gives the same counts; small tiles exercise the multi-pass path on small stores).
  *   gp_robustness_cross: the flip of ONE bit outside the sub-cube: entry i of d_mine and entry i of d_partner (the
  *     shard whose index differs in that bit; may be peer memory) are neighbours; counts go to the classes found in

@@ -234,6 +234,176 @@ __global__ void __launch_bounds__(RTHREADS, 2) robustness_kernel(RobArgs a) {
     rob_flush(a, cache);
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// a6, second version of the tile kernel.  Same bit-tiling; the per-flip work is cut to what the counts need:
+//   * "differs" per genotype pair = XOR + one unsigned 16x2 min with 1 (VIMNMX.U16x2): 2 ALU ops per two genotypes,
+//     summed in packed halves (rne); neutral = flips - differs - (null neighbours) for a non-null genotype;
+//   * null neighbours come from a per-tile bitmask (one byte per 8-genotype vector, built while staging): the partner
+//     vector's byte is spread to eight nibbles by a 256-entry table and added to a nibble-packed counter;
+//   * "some genotype of this vector has a neighbour of another class" = (differs byte) & (partner non-null byte) &
+//     (own non-null byte) != 0: one test per vector-flip; only then are the events walked for the pair bitmap;
+//   * class counts: (n, r, d) per run of equal class into the shared-memory cache; other = flips*n - r - d when the
+//     cache is written back; n also yields the designability histogram when the caller wants it (pass 0).
+// ---------------------------------------------------------------------------------------------------------------
+constexpr int ROB2_TB_MAX = 16;     // 2^16 phenotypes = 128 KB of shared memory, one block of 1024 threads per SM
+constexpr int R2THREADS = 1024;
+struct Rob2Slot { uint32_t key, n, r, d; };
+
+struct Rob2Args {
+    const uint16_t* pheno;
+    int n_bits;
+    uint32_t C;
+    unsigned long long *R, *Dl, *O, *hist;  // hist nullable: hist[p] += genotypes of class p, hist[C] += nulls
+    uint32_t* bitmap;                        // nullable
+    int tb, c, h, hi_pos, f0;
+};
+
+__device__ __forceinline__ void rob2_add(const Rob2Args& a, Rob2Slot* cache, uint32_t n_flip, uint32_t p, uint32_t n,
+                                         uint32_t r, uint32_t d) {
+    if (p >= a.C) return;
+    Rob2Slot* s = cache + ((p * 2654435761u) >> 21);
+    uint32_t k = s->key;
+    if (k == NULLP) k = atomicCAS(&s->key, NULLP, p), k = (k == NULLP) ? p : k;
+    if (k == p) {
+        atomicAdd(&s->n, n);
+        if (r) atomicAdd(&s->r, r);
+        if (d) atomicAdd(&s->d, d);
+    } else {
+        if (r) atomicAdd(&a.R[p], (unsigned long long)r);
+        if (d) atomicAdd(&a.Dl[p], (unsigned long long)d);
+        const uint32_t o = n * n_flip - r - d;
+        if (o) atomicAdd(&a.O[p], (unsigned long long)o);
+        if (a.hist) atomicAdd(&a.hist[p], (unsigned long long)n);
+    }
+}
+
+__device__ __forceinline__ void rob2_flush(const Rob2Args& a, Rob2Slot* cache, uint32_t n_flip) {
+    __syncthreads();
+    for (uint32_t i = threadIdx.x; i < ROB_SLOTS; i += blockDim.x) {
+        const Rob2Slot s = cache[i];
+        if (s.key != NULLP) {
+            if (s.r) atomicAdd(&a.R[s.key], (unsigned long long)s.r);
+            if (s.d) atomicAdd(&a.Dl[s.key], (unsigned long long)s.d);
+            const unsigned long long o = (unsigned long long)s.n * n_flip - s.r - s.d;
+            if (o) atomicAdd(&a.O[s.key], o);
+            if (a.hist && s.n) atomicAdd(&a.hist[s.key], (unsigned long long)s.n);
+        }
+        cache[i] = Rob2Slot{NULLP, 0, 0, 0};
+    }
+    __syncthreads();
+}
+
+template <bool PAIRS>
+__global__ void __launch_bounds__(R2THREADS, 1) robustness2_kernel(Rob2Args a) {
+    extern __shared__ __align__(16) uint16_t seg[];
+    const uint32_t n_vec = 1u << (a.tb - 3);                       // 16-byte vectors per tile
+    uint8_t* nnb = reinterpret_cast<uint8_t*>(seg + ((size_t)1 << a.tb));  // per vector: bit i = genotype i is NOT null
+    uint32_t* lut = reinterpret_cast<uint32_t*>(nnb + n_vec);      // byte -> eight nibbles
+    Rob2Slot* cache = reinterpret_cast<Rob2Slot*>(lut + 256);
+    uint32_t* pf = reinterpret_cast<uint32_t*>(cache + ROB_SLOTS);
+    for (uint32_t i = threadIdx.x; i < 256; i += blockDim.x) {
+        uint32_t x = 0;
+        for (int b = 0; b < 8; b++) x |= ((i >> b) & 1u) << (4 * b);
+        lut[i] = x;
+    }
+    for (uint32_t i = threadIdx.x; i < ROB_SLOTS; i += blockDim.x) cache[i] = Rob2Slot{NULLP, 0, 0, 0};
+    if (PAIRS)
+        for (uint32_t i = threadIdx.x; i < ROB_PF_SLOTS; i += blockDim.x) pf[i] = 0xFFFFFFFFu;
+    uint32_t tiles_done = 0, last_key = 0xFFFFFFFFu;
+    unsigned long long nulls = 0;
+    const uint64_t n_tiles = 1ULL << (a.n_bits - a.tb);
+    const uint32_t cmask = (1u << a.c) - 1u;
+    const int lo_outer = a.hi_pos - a.c;                           // outer-index bits that sit below the spread bits
+    const uint32_t n_flip = (uint32_t)(a.tb - a.f0);
+    const uint4* sv = reinterpret_cast<const uint4*>(seg);
+    const RobArgs pa = {a.pheno, a.n_bits, a.C, a.R, a.Dl, a.O, a.bitmap, a.tb, a.c, a.h, a.hi_pos, a.f0};
+    for (uint64_t t = blockIdx.x; t < n_tiles; t += gridDim.x) {
+        const uint64_t base = ((t & ((1ULL << lo_outer) - 1ULL)) << a.c) | ((t >> lo_outer) << (a.hi_pos + a.h));
+        __syncthreads();
+        for (uint32_t v = threadIdx.x; v < n_vec; v += R2THREADS) {
+            const uint32_t l = v << 3;
+            const uint64_t g = base | (l & cmask) | ((uint64_t)(l >> a.c) << a.hi_pos);
+            const uint4 x = __ldg(reinterpret_cast<const uint4*>(a.pheno + g));
+            reinterpret_cast<uint4*>(seg)[v] = x;
+            // non-null bits: per half min(~x, 1)
+            const uint32_t n0 = __vminu2(~x.x, 0x00010001u), n1 = __vminu2(~x.y, 0x00010001u);
+            const uint32_t n2 = __vminu2(~x.z, 0x00010001u), n3 = __vminu2(~x.w, 0x00010001u);
+            const uint32_t tt = n0 + (n1 << 2) + (n2 << 4) + (n3 << 6);
+            const uint32_t nb = (tt | (tt >> 15)) & 0xFFu;
+            nnb[v] = (uint8_t)nb;
+            nulls += 8 - __popc(nb);
+        }
+        __syncthreads();
+        for (uint32_t v = threadIdx.x; v < n_vec; v += R2THREADS) {
+            const uint32_t Bm = nnb[v];
+            if (Bm == 0) continue;                                  // all 8 null: nothing to count
+            const uint4 mv = sv[v];
+            const uint32_t m[4] = {mv.x, mv.y, mv.z, mv.w};
+            uint32_t rne[4] = {0, 0, 0, 0};                        // per half: flips whose neighbour differs (class or null)
+            uint32_t nnA = 0, nnB = 0;                             // per nibble: non-null neighbours (flips < 8 / >= 8 of this pass)
+            for (int k = a.f0; k < a.tb; k++) {
+                uint32_t q[4], Bp;
+                if (k == 0) {
+#pragma unroll
+                    for (int w = 0; w < 4; w++) q[w] = __funnelshift_l(m[w], m[w], 16);
+                    Bp = ((Bm & 0x55u) << 1) | ((Bm >> 1) & 0x55u);
+                } else if (k == 1) {
+                    q[0] = m[1]; q[1] = m[0]; q[2] = m[3]; q[3] = m[2];
+                    Bp = ((Bm & 0x33u) << 2) | ((Bm >> 2) & 0x33u);
+                } else if (k == 2) {
+                    q[0] = m[2]; q[1] = m[3]; q[2] = m[0]; q[3] = m[1];
+                    Bp = ((Bm & 0x0Fu) << 4) | (Bm >> 4);
+                } else {
+                    const uint32_t pv = v ^ (1u << (k - 3));
+                    const uint4 x = sv[pv];
+                    q[0] = x.x; q[1] = x.y; q[2] = x.z; q[3] = x.w;
+                    Bp = nnb[pv];
+                }
+                const uint32_t e0 = __vminu2(q[0] ^ m[0], 0x00010001u), e1 = __vminu2(q[1] ^ m[1], 0x00010001u);
+                const uint32_t e2 = __vminu2(q[2] ^ m[2], 0x00010001u), e3 = __vminu2(q[3] ^ m[3], 0x00010001u);
+                rne[0] += e0; rne[1] += e1; rne[2] += e2; rne[3] += e3;
+                const uint32_t sp = lut[Bp];
+                if (k - a.f0 < 8) nnA += sp; else nnB += sp;
+                if (PAIRS) {
+                    const uint32_t tt = e0 + (e1 << 2) + (e2 << 4) + (e3 << 6);
+                    // differs, both ends non-null; every such edge is met from both ends: keep the end whose flipped bit is 0
+                    uint32_t ob = (tt | (tt >> 15)) & Bp & Bm;
+                    ob &= k == 0 ? 0x55u : k == 1 ? 0x33u : k == 2 ? 0x0Fu : (((v >> (k - 3)) & 1u) ? 0u : 0xFFu);
+                    while (ob) {
+                        const uint32_t l = (v << 3) + (__ffs(ob) - 1);
+                        ob &= ob - 1;
+                        uint32_t p = seg[l], qq = seg[l ^ (1u << k)];
+                        if (qq < p) { const uint32_t x = p; p = qq; qq = x; }
+                        const uint32_t key = (p << 16) | qq;
+                        if (key != last_key) { last_key = key; note_pair(pa, pf, p, qq); }
+                    }
+                }
+            }
+            // per genotype: differs = rne half, non-null neighbours = nibble of nnA + nnB;
+            // neutral = flips - differs; to null = flips - non-null neighbours.  Runs of equal class are merged.
+            uint32_t run = 0, r_acc = 0, d_acc = 0;
+#pragma unroll
+            for (int j = 0; j < 8; j++) {
+                const uint32_t p = (m[j >> 1] >> (16 * (j & 1))) & 0xFFFFu;
+                if (p == NULLP) continue;
+                run++;
+                r_acc += n_flip - ((rne[j >> 1] >> (16 * (j & 1))) & 0xFFFFu);
+                d_acc += n_flip - ((nnA >> (4 * j)) & 15u) - ((nnB >> (4 * j)) & 15u);
+                const uint32_t nxt = j < 7 ? (m[(j + 1) >> 1] >> (16 * ((j + 1) & 1))) & 0xFFFFu : NULLP;
+                if (nxt == p) continue;
+                rob2_add(a, cache, n_flip, p, run, r_acc, d_acc);
+                run = 0; r_acc = 0; d_acc = 0;
+            }
+        }
+        if (++tiles_done % ROB_FLUSH_TILES == 0) rob2_flush(a, cache, n_flip);
+    }
+    rob2_flush(a, cache, n_flip);
+    if (a.hist) {
+        for (int o = 16; o > 0; o >>= 1) nulls += __shfl_down_sync(0xFFFFFFFFu, nulls, o);
+        if ((threadIdx.x & 31) == 0 && nulls) atomicAdd(&a.hist[a.C], nulls);
+    }
+}
+
 // n_bits < 3 (fewer than 8 genotypes): one thread per genotype, straight from global memory.
 __global__ void robustness_tiny_kernel(RobArgs a) {
     const uint32_t g = threadIdx.x;
@@ -450,14 +620,15 @@ extern "C" gp_status gp_designability(const uint16_t* d_pheno, uint64_t count, u
 
 extern "C" uint64_t gp_pair_bitmap_words(uint32_t n_classes) { return ((uint64_t)n_classes * n_classes + 31) / 32; }
 
-extern "C" gp_status gp_robustness_partial(const uint16_t* d_pheno, int n_bits, uint32_t n_classes, uint64_t* d_neutral,
-                                           uint64_t* d_deleterious, uint64_t* d_other, uint32_t* d_pair_bitmap,
-                                           int tile_bits, void* stream) {
+static gp_status robustness_passes(const uint16_t* d_pheno, int n_bits, uint32_t n_classes, uint64_t* d_neutral,
+                                   uint64_t* d_deleterious, uint64_t* d_other, uint64_t* d_hist, uint32_t* d_pair_bitmap,
+                                   int tile_bits, cudaStream_t st) {
     if (!d_pheno || !d_neutral || !d_deleterious || !d_other) return GP_INVALID_ARG;
     if (n_bits < 1 || n_bits > 40 || n_classes == 0 || n_classes >= NULLP) return GP_INVALID_ARG;
-    if (tile_bits != 0 && (tile_bits < 4 || tile_bits > ROB_TB_MAX)) return GP_INVALID_ARG;
+    const bool v1 = (tile_bits & 0x100) != 0;  // previous kernel, kept for A/B timing until the new one is profiled
+    tile_bits &= 0xFF;
+    if (tile_bits != 0 && (tile_bits < 4 || tile_bits > ROB2_TB_MAX)) return GP_INVALID_ARG;
     if (((uintptr_t)d_pheno & 15) != 0) return GP_INVALID_ARG;
-    cudaStream_t st = (cudaStream_t)stream;
     RobArgs a;
     a.pheno = d_pheno; a.n_bits = n_bits; a.C = n_classes;
     a.R = reinterpret_cast<unsigned long long*>(d_neutral);
@@ -470,33 +641,64 @@ extern "C" gp_status gp_robustness_partial(const uint16_t* d_pheno, int n_bits, 
         gp_time_end(GP_KERNEL_ROBUSTNESS, st);
         GP_CUDA(cudaGetLastError());
         gp_count_launches(1);
+        if (d_hist) {
+            hist_kernel<<<1, 1024, 0, st>>>(d_pheno, 1ULL << n_bits, n_classes, reinterpret_cast<unsigned long long*>(d_hist), 0);
+            GP_CUDA(cudaGetLastError());
+            gp_count_launches(1);
+        }
         return GP_OK;
     }
-    const int tb_want = tile_bits ? tile_bits : ROB_TB_MAX;
-    const int tb = n_bits < tb_want ? n_bits : tb_want;
-    const size_t smem = ((size_t)2 << tb) + ROB_SLOTS * sizeof(RobSlot) + ROB_PF_SLOTS * sizeof(uint32_t);
-    GP_CUDA(cudaFuncSetAttribute(robustness_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const int tb_max = v1 ? ROB_TB_MAX : ROB2_TB_MAX;
+    int tb = tile_bits ? tile_bits : tb_max;
+    if (tb > tb_max) tb = tb_max;
+    if (tb > n_bits) tb = n_bits;
     const uint64_t n_tiles = 1ULL << (n_bits - tb);
-    const uint64_t cap = (uint64_t)sm_count() * 2;
+    const uint64_t cap = (uint64_t)sm_count() * (v1 ? 2 : 1);
     const unsigned grid = (unsigned)(n_tiles < cap ? n_tiles : cap);
+    const size_t smem = v1 ? ((size_t)2 << tb) + ROB_SLOTS * sizeof(RobSlot) + ROB_PF_SLOTS * sizeof(uint32_t)
+                           : ((size_t)2 << tb) + ((size_t)1 << (tb - 3)) + 1024 + ROB_SLOTS * sizeof(Rob2Slot) +
+                                 ROB_PF_SLOTS * sizeof(uint32_t);
+    if (v1) GP_CUDA(cudaFuncSetAttribute(robustness_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    else if (d_pair_bitmap) GP_CUDA(cudaFuncSetAttribute(robustness2_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    else GP_CUDA(cudaFuncSetAttribute(robustness2_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     a.tb = tb;
-    // pass 0: the tb low bits; then up to tb-3 further bits per pass (segments stay >= 16 bytes)
+    // pass 0: the tb low bits; every later pass flips its own spread bits: segments of 2^c consecutive ids (128 bytes
+    // when the tile allows, never under 16), all 2^h values of the spread bits on chip
+    const int seg_bits = v1 ? 7 : 6;
     int done = 0;
+    bool first = true;
     while (done < n_bits) {
         if (done == 0) { a.c = tb; a.h = 0; a.hi_pos = tb; a.f0 = 0; done = tb; }
         else {
             int h = n_bits - done;
-            const int hmax = tb - 7 > 1 ? tb - 7 : (tb - 3 > 1 ? tb - 3 : 1);  // keep segments >= 256 B when the tile allows
+            const int hmax = tb - seg_bits > 1 ? tb - seg_bits : (tb - 3 > 1 ? tb - 3 : 1);
             if (h > hmax) h = hmax;
             a.h = h; a.c = tb - h; a.hi_pos = done; a.f0 = a.c; done += h;
         }
         gp_time_begin(GP_KERNEL_ROBUSTNESS, st);
-        robustness_kernel<<<grid, RTHREADS, smem, st>>>(a);
+        if (v1) robustness_kernel<<<grid, RTHREADS, smem, st>>>(a);
+        else {
+            Rob2Args b;
+            b.pheno = a.pheno; b.n_bits = n_bits; b.C = n_classes; b.R = a.R; b.Dl = a.Dl; b.O = a.O;
+            b.hist = first ? reinterpret_cast<unsigned long long*>(d_hist) : nullptr;
+            b.bitmap = a.bitmap; b.tb = a.tb; b.c = a.c; b.h = a.h; b.hi_pos = a.hi_pos; b.f0 = a.f0;
+            if (d_pair_bitmap) robustness2_kernel<true><<<grid, R2THREADS, smem, st>>>(b);
+            else robustness2_kernel<false><<<grid, R2THREADS, smem, st>>>(b);
+        }
         gp_time_end(GP_KERNEL_ROBUSTNESS, st);
         GP_CUDA(cudaGetLastError());
         gp_count_launches(1);
+        first = false;
     }
+    if (v1 && d_hist) return GP_INVALID_ARG;
     return GP_OK;
+}
+
+extern "C" gp_status gp_robustness_partial(const uint16_t* d_pheno, int n_bits, uint32_t n_classes, uint64_t* d_neutral,
+                                           uint64_t* d_deleterious, uint64_t* d_other, uint32_t* d_pair_bitmap,
+                                           int tile_bits, void* stream) {
+    return robustness_passes(d_pheno, n_bits, n_classes, d_neutral, d_deleterious, d_other, nullptr, d_pair_bitmap, tile_bits,
+                             (cudaStream_t)stream);
 }
 
 extern "C" gp_status gp_robustness_cross(const uint16_t* d_mine, const uint16_t* d_partner, uint64_t count,
@@ -543,8 +745,9 @@ extern "C" gp_status gp_pair_bitmap_count(const uint32_t* d_bitmap, uint32_t n_c
     return GP_OK;
 }
 
-extern "C" gp_status gp_robustness(const uint16_t* d_pheno, int n_bits, uint32_t n_classes, uint64_t* d_neutral,
-                                   uint64_t* d_deleterious, uint64_t* d_other, uint64_t* d_pair_count, void* stream) {
+extern "C" gp_status gp_reduce_store(const uint16_t* d_pheno, int n_bits, uint32_t n_classes, uint64_t* d_hist,
+                                     uint64_t* d_neutral, uint64_t* d_deleterious, uint64_t* d_other, uint64_t* d_pair_count,
+                                     void* stream) {
     if (!d_pheno || !d_neutral || !d_deleterious || !d_other) return GP_INVALID_ARG;
     if (n_bits < 1 || n_bits > 40 || n_classes == 0 || n_classes >= NULLP) return GP_INVALID_ARG;
     cudaStream_t st = (cudaStream_t)stream;
@@ -552,16 +755,22 @@ extern "C" gp_status gp_robustness(const uint16_t* d_pheno, int n_bits, uint32_t
     GP_CUDA(cudaMemsetAsync(d_neutral, 0, cb, st));
     GP_CUDA(cudaMemsetAsync(d_deleterious, 0, cb, st));
     GP_CUDA(cudaMemsetAsync(d_other, 0, cb, st));
+    if (d_hist) GP_CUDA(cudaMemsetAsync(d_hist, 0, cb + sizeof(uint64_t), st));
     uint32_t* bitmap = nullptr;
     if (d_pair_count) {
         const uint64_t n_words = gp_pair_bitmap_words(n_classes);
         GP_CUDA(cudaMallocAsync(&bitmap, n_words * 4, st));
         GP_CUDA(cudaMemsetAsync(bitmap, 0, n_words * 4, st));
     }
-    gp_status stt = gp_robustness_partial(d_pheno, n_bits, n_classes, d_neutral, d_deleterious, d_other, bitmap, 0, stream);
+    gp_status stt = robustness_passes(d_pheno, n_bits, n_classes, d_neutral, d_deleterious, d_other, d_hist, bitmap, 0, st);
     if (stt == GP_OK && d_pair_count) stt = gp_pair_bitmap_count(bitmap, n_classes, d_pair_count, stream);
     if (bitmap) cudaFreeAsync(bitmap, st);
     return stt;
+}
+
+extern "C" gp_status gp_robustness(const uint16_t* d_pheno, int n_bits, uint32_t n_classes, uint64_t* d_neutral,
+                                   uint64_t* d_deleterious, uint64_t* d_other, uint64_t* d_pair_count, void* stream) {
+    return gp_reduce_store(d_pheno, n_bits, n_classes, nullptr, d_neutral, d_deleterious, d_other, d_pair_count, stream);
 }
 
 extern "C" gp_status gp_threshold_sweep(const uint16_t* d_pheno, const int16_t* d_gap, uint64_t count, uint32_t n_classes,

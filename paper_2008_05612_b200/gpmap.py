@@ -57,6 +57,7 @@ SIGNATURES = {
     "gp_seeded_sequences": (ctypes.c_int, [ctypes.c_uint64, ctypes.c_uint64, ctypes.c_uint64, ctypes.c_int, _u8p]),
     "gp_designability": (ctypes.c_int, [_vp, ctypes.c_uint64, ctypes.c_uint32, _vp, _vp]),
     "gp_robustness": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_uint32, _vp, _vp, _vp, _vp, _vp]),
+    "gp_reduce_store": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_uint32, _vp, _vp, _vp, _vp, _vp, _vp]),
     "gp_pair_bitmap_words": (ctypes.c_uint64, [ctypes.c_uint32]),
     "gp_robustness_partial": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_uint32, _vp, _vp, _vp, _vp, ctypes.c_int, _vp]),
     "gp_robustness_cross": (ctypes.c_int, [_vp, _vp, ctypes.c_uint64, ctypes.c_uint32, _vp, _vp, _vp, _vp, _vp]),
@@ -349,6 +350,19 @@ def robustness(pheno, n_bits, n_classes, want_pairs=True, stream=None):
     _check(lib().gp_robustness(_dptr(pheno, torch.uint16), n_bits, n_classes, _dptr(out[0]), _dptr(out[1]), _dptr(out[2]),
                                _dptr(pc), _stream(stream)), "gp_robustness")
     return out[0], out[1], out[2], pc
+
+
+def reduce_store(pheno, n_bits, n_classes, want_pairs=True, stream=None):
+    """gp_reduce_store: (hist, R, D, O, pair_count) — designability and the neighbour pass in one sweep."""
+    import torch
+    if pheno.numel() != 1 << n_bits:
+        raise ValueError("gp_reduce_store needs the full store of 2^n_bits entries")
+    hist = torch.empty(n_classes + 1, dtype=torch.int64, device=pheno.device)
+    out = torch.empty((3, n_classes), dtype=torch.int64, device=pheno.device)
+    pc = torch.empty(1, dtype=torch.int64, device=pheno.device) if want_pairs else None
+    _check(lib().gp_reduce_store(_dptr(pheno, torch.uint16), n_bits, n_classes, _dptr(hist), _dptr(out[0]), _dptr(out[1]),
+                                 _dptr(out[2]), _dptr(pc), _stream(stream)), "gp_reduce_store")
+    return hist, out[0], out[1], out[2], pc
 
 
 def pair_bitmap(n_classes, device="cuda"):

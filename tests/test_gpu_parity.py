@@ -239,12 +239,12 @@ def test_enumerate_host_end_to_end(oracle_structures):
     assert gpmap.launch_count() > 0
 
 
-@pytest.mark.parametrize("tile_bits", [4, 7, 10, 15])
+@pytest.mark.parametrize("tile_bits", [4, 7, 10, 15, 16])
 def test_robustness_tile_sizes_agree_with_oracle(tile_bits):
     """The bit-tiled neighbour pass gives the same counts for every tile size (small tiles force the multi-pass,
     spread-bit path on small stores), on stores whose size is not a multiple of the pass width."""
     rng = np.random.default_rng(11)
-    for n_bits, C, p_null in [(1, 2, 0.3), (2, 3, 0.3), (3, 5, 0.5), (9, 3, 0.4), (13, 549, 0.6), (18, 28728, 0.57)]:
+    for n_bits, C, p_null in [(1, 2, 0.3), (2, 3, 0.3), (3, 5, 0.5), (9, 3, 0.4), (13, 549, 0.6), (18, 28728, 0.57), (21, 51704, 0.95)]:
         n = 1 << n_bits
         store = rng.integers(0, C, size=n).astype(np.uint16)
         # clustered classes, so that neutral neighbours and equal-class runs exist
@@ -261,6 +261,15 @@ def test_robustness_tile_sizes_agree_with_oracle(tile_bits):
         assert np.array_equal(got[1], Do), (tile_bits, n_bits)
         assert np.array_equal(got[2], Oo), (tile_bits, n_bits)
         assert int(pc) == pco, (tile_bits, n_bits)
+        # without the pair bitmap (other kernel instantiation): same counts
+        rdo2 = torch.zeros((3, C), dtype=torch.int64, device="cuda")
+        gpmap.robustness_partial(ph, n_bits, C, rdo2, None, tile_bits=tile_bits)
+        assert torch.equal(rdo, rdo2), (tile_bits, n_bits)
+    # designability and neighbour pass in one sweep (gp_reduce_store) on the last store
+    hist, R, Dl, Oc, pc2 = gpmap.reduce_store(ph, n_bits, C)
+    assert np.array_equal(hist.cpu().numpy().astype(np.uint64), orc.designability(store, C))
+    assert np.array_equal(R.cpu().numpy().astype(np.uint64), Ro) and np.array_equal(Dl.cpu().numpy().astype(np.uint64), Do)
+    assert np.array_equal(Oc.cpu().numpy().astype(np.uint64), Oo) and int(pc2) == pco
 
 
 @pytest.mark.parametrize("dims,k", [((2, 2, 1), 9), ((3, 3, 1), 9), ((4, 4, 1), 5), ((4, 4, 1), 6), ((4, 4, 1), 8),
