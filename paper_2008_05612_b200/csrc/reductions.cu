@@ -258,17 +258,26 @@ struct Rob2Args {
     int tb, c, h, hi_pos, f0;
 };
 
+constexpr uint32_t ROB2_SLOTS = 4096;   // class-count cache of the second kernel: 64 KB, two probes (slot, slot ^ 1)
+
 __device__ __forceinline__ void rob2_add(const Rob2Args& a, Rob2Slot* cache, uint32_t n_flip, uint32_t p, uint32_t n,
                                          uint32_t r, uint32_t d) {
     if (p >= a.C) return;
-    Rob2Slot* s = cache + ((p * 2654435761u) >> 21);
+    Rob2Slot* s = cache + ((p * 2654435761u) >> 20);
     uint32_t k = s->key;
-    if (k == NULLP) k = atomicCAS(&s->key, NULLP, p), k = (k == NULLP) ? p : k;
+    if (k != p) {
+        if (k == NULLP) k = atomicCAS(&s->key, NULLP, p), k = (k == NULLP) ? p : k;
+        if (k != p) {                       // second probe
+            s = cache + (((p * 2654435761u) >> 20) ^ 1u);
+            k = s->key;
+            if (k == NULLP) k = atomicCAS(&s->key, NULLP, p), k = (k == NULLP) ? p : k;
+        }
+    }
     if (k == p) {
         atomicAdd(&s->n, n);
         if (r) atomicAdd(&s->r, r);
         if (d) atomicAdd(&s->d, d);
-    } else {
+    } else {                                // both slots hold other classes: straight to global memory
         if (r) atomicAdd(&a.R[p], (unsigned long long)r);
         if (d) atomicAdd(&a.Dl[p], (unsigned long long)d);
         const uint32_t o = n * n_flip - r - d;
@@ -279,7 +288,7 @@ __device__ __forceinline__ void rob2_add(const Rob2Args& a, Rob2Slot* cache, uin
 
 __device__ __forceinline__ void rob2_flush(const Rob2Args& a, Rob2Slot* cache, uint32_t n_flip) {
     __syncthreads();
-    for (uint32_t i = threadIdx.x; i < ROB_SLOTS; i += blockDim.x) {
+    for (uint32_t i = threadIdx.x; i < ROB2_SLOTS; i += blockDim.x) {
         const Rob2Slot s = cache[i];
         if (s.key != NULLP) {
             if (s.r) atomicAdd(&a.R[s.key], (unsigned long long)s.r);
@@ -293,28 +302,93 @@ __device__ __forceinline__ void rob2_flush(const Rob2Args& a, Rob2Slot* cache, u
     __syncthreads();
 }
 
+constexpr uint32_t ROB2_PF_SLOTS = 4096;  // per-block filter of recently recorded class pairs (16 KB)
+
+// Pair events are not walked where they are found (a quarter of the lanes would work while the rest wait): a lane
+// that has some pushes ONE record (vector, flipped bit, event byte) into its warp's shared-memory ring, and whenever 32
+// records are pending the whole warp drains them, one record per lane.
+constexpr uint32_t ROB2_RING = 64;   // records per warp
+
+__device__ __forceinline__ void rob2_events(const RobArgs& pa, const uint16_t* seg, uint32_t* pf, uint32_t& last_key, uint32_t rec) {
+    const uint32_t v = rec & 0x1FFFu, flipmask = 1u << ((rec >> 13) & 15u);
+    uint32_t ob = rec >> 17;
+    while (ob) {
+        const uint32_t l = (v << 3) + (__ffs(ob) - 1);
+        ob &= ob - 1;
+        const uint32_t p = seg[l], qq = seg[l ^ flipmask];
+        const uint32_t key = (min(p, qq) << 16) | max(p, qq);
+        if (key != last_key) {
+            last_key = key;
+            uint32_t* slot = pf + ((key * 2654435761u) >> 20);
+            if (*(volatile uint32_t*)slot != key) {   // not seen by this block lately (racy update is harmless: the bitmap is the truth)
+                *(volatile uint32_t*)slot = key;
+                const uint32_t q = key & 0xFFFFu;
+                if (q < pa.C) {                       // fire-and-forget RED.OR: no read of the bitmap, nothing to wait for
+                    const uint64_t bit = (uint64_t)(key >> 16) * pa.C + q;
+                    atomicOr(pa.bitmap + (bit >> 5), 1u << (bit & 31));
+                }
+            }
+        }
+    }
+}
+
+// One flip of one 8-genotype vector: q = the neighbours' class words, Bp = their non-null byte, keep = which of the 8
+// genotypes are the end of their edge that records pair events (the end whose flipped bit is 0).  Called by all 32
+// lanes of the warp together (the ballot).
+template <bool PAIRS>
+__device__ __forceinline__ void rob2_flip(const RobArgs& pa, const uint16_t* seg, uint32_t* pf, uint32_t& last_key,
+                                          uint32_t* ring, uint32_t& head, uint32_t& tail,
+                                          const uint32_t (&m)[4], uint32_t q0, uint32_t q1, uint32_t q2, uint32_t q3,
+                                          uint32_t Bm, uint32_t Bp, uint32_t keep, uint32_t v, uint32_t k,
+                                          const uint32_t* lut, uint32_t (&rne)[4], uint32_t& nn) {
+    const uint32_t e0 = __vminu2(q0 ^ m[0], 0x00010001u), e1 = __vminu2(q1 ^ m[1], 0x00010001u);
+    const uint32_t e2 = __vminu2(q2 ^ m[2], 0x00010001u), e3 = __vminu2(q3 ^ m[3], 0x00010001u);
+    rne[0] += e0; rne[1] += e1; rne[2] += e2; rne[3] += e3;
+    nn += lut[Bp];
+    if (PAIRS) {
+        const uint32_t tt = e0 + (e1 << 2) + (e2 << 4) + (e3 << 6);
+        const uint32_t ob = (tt | (tt >> 15)) & Bp & Bm & keep;     // differs, both ends non-null, recording end
+        const uint32_t has = __ballot_sync(0xFFFFFFFFu, ob != 0);
+        if (has) {
+            const uint32_t lane = threadIdx.x & 31u;
+            if (ob) ring[(tail + __popc(has & ((1u << lane) - 1u))) & (ROB2_RING - 1)] = v | (k << 13) | (ob << 17);
+            tail += __popc(has);
+            if (tail - head >= 32) {
+                __syncwarp();
+                rob2_events(pa, seg, pf, last_key, ring[(head + lane) & (ROB2_RING - 1)]);
+                head += 32;
+                __syncwarp();
+            }
+        }
+    }
+}
+
 template <bool PAIRS>
 __global__ void __launch_bounds__(R2THREADS, 1) robustness2_kernel(Rob2Args a) {
     extern __shared__ __align__(16) uint16_t seg[];
     const uint32_t n_vec = 1u << (a.tb - 3);                       // 16-byte vectors per tile
     uint8_t* nnb = reinterpret_cast<uint8_t*>(seg + ((size_t)1 << a.tb));  // per vector: bit i = genotype i is NOT null
-    uint32_t* lut = reinterpret_cast<uint32_t*>(nnb + n_vec);      // byte -> eight nibbles
+    uint32_t* lut = reinterpret_cast<uint32_t*>(nnb + ((n_vec + 15u) & ~15u));  // byte -> eight nibbles
     Rob2Slot* cache = reinterpret_cast<Rob2Slot*>(lut + 256);
-    uint32_t* pf = reinterpret_cast<uint32_t*>(cache + ROB_SLOTS);
+    uint32_t* pf = reinterpret_cast<uint32_t*>(cache + ROB2_SLOTS);
+    uint32_t* ring = pf + ROB2_PF_SLOTS + (threadIdx.x >> 5) * ROB2_RING;  // this warp's event ring (PAIRS only)
+    uint32_t head = 0, tail = 0;
     for (uint32_t i = threadIdx.x; i < 256; i += blockDim.x) {
         uint32_t x = 0;
         for (int b = 0; b < 8; b++) x |= ((i >> b) & 1u) << (4 * b);
         lut[i] = x;
     }
-    for (uint32_t i = threadIdx.x; i < ROB_SLOTS; i += blockDim.x) cache[i] = Rob2Slot{NULLP, 0, 0, 0};
+    for (uint32_t i = threadIdx.x; i < ROB2_SLOTS; i += blockDim.x) cache[i] = Rob2Slot{NULLP, 0, 0, 0};
     if (PAIRS)
-        for (uint32_t i = threadIdx.x; i < ROB_PF_SLOTS; i += blockDim.x) pf[i] = 0xFFFFFFFFu;
+        for (uint32_t i = threadIdx.x; i < ROB2_PF_SLOTS; i += blockDim.x) pf[i] = 0xFFFFFFFFu;
     uint32_t tiles_done = 0, last_key = 0xFFFFFFFFu;
     unsigned long long nulls = 0;
     const uint64_t n_tiles = 1ULL << (a.n_bits - a.tb);
     const uint32_t cmask = (1u << a.c) - 1u;
     const int lo_outer = a.hi_pos - a.c;                           // outer-index bits that sit below the spread bits
     const uint32_t n_flip = (uint32_t)(a.tb - a.f0);
+    const int k_lo = a.f0 < 3 ? 3 : a.f0;                          // first flip that needs a partner vector
+    const int k_mid = k_lo + 8 < a.tb ? k_lo + 8 : a.tb;           // nibble counters hold 8 flips each
     const uint4* sv = reinterpret_cast<const uint4*>(seg);
     const RobArgs pa = {a.pheno, a.n_bits, a.C, a.R, a.Dl, a.O, a.bitmap, a.tb, a.c, a.h, a.hi_pos, a.f0};
     for (uint64_t t = blockIdx.x; t < n_tiles; t += gridDim.x) {
@@ -334,52 +408,39 @@ __global__ void __launch_bounds__(R2THREADS, 1) robustness2_kernel(Rob2Args a) {
             nulls += 8 - __popc(nb);
         }
         __syncthreads();
-        for (uint32_t v = threadIdx.x; v < n_vec; v += R2THREADS) {
-            const uint32_t Bm = nnb[v];
-            if (Bm == 0) continue;                                  // all 8 null: nothing to count
-            const uint4 mv = sv[v];
+        for (uint32_t v0 = 0; v0 < n_vec; v0 += R2THREADS) {       // uniform trip count: the warp stays converged
+            const uint32_t v = v0 + threadIdx.x;
+            const bool live = v < n_vec;
+            const uint32_t Bm = live ? nnb[v] : 0u;
+            if (__all_sync(0xFFFFFFFFu, Bm == 0)) continue;         // the warp's 256 genotypes are all null: nothing to count
+            const uint4 mv = live ? sv[v] : make_uint4(~0u, ~0u, ~0u, ~0u);
             const uint32_t m[4] = {mv.x, mv.y, mv.z, mv.w};
             uint32_t rne[4] = {0, 0, 0, 0};                        // per half: flips whose neighbour differs (class or null)
-            uint32_t nnA = 0, nnB = 0;                             // per nibble: non-null neighbours (flips < 8 / >= 8 of this pass)
-            for (int k = a.f0; k < a.tb; k++) {
-                uint32_t q[4], Bp;
-                if (k == 0) {
-#pragma unroll
-                    for (int w = 0; w < 4; w++) q[w] = __funnelshift_l(m[w], m[w], 16);
-                    Bp = ((Bm & 0x55u) << 1) | ((Bm >> 1) & 0x55u);
-                } else if (k == 1) {
-                    q[0] = m[1]; q[1] = m[0]; q[2] = m[3]; q[3] = m[2];
-                    Bp = ((Bm & 0x33u) << 2) | ((Bm >> 2) & 0x33u);
-                } else if (k == 2) {
-                    q[0] = m[2]; q[1] = m[3]; q[2] = m[0]; q[3] = m[1];
-                    Bp = ((Bm & 0x0Fu) << 4) | (Bm >> 4);
-                } else {
-                    const uint32_t pv = v ^ (1u << (k - 3));
-                    const uint4 x = sv[pv];
-                    q[0] = x.x; q[1] = x.y; q[2] = x.z; q[3] = x.w;
-                    Bp = nnb[pv];
-                }
-                const uint32_t e0 = __vminu2(q[0] ^ m[0], 0x00010001u), e1 = __vminu2(q[1] ^ m[1], 0x00010001u);
-                const uint32_t e2 = __vminu2(q[2] ^ m[2], 0x00010001u), e3 = __vminu2(q[3] ^ m[3], 0x00010001u);
-                rne[0] += e0; rne[1] += e1; rne[2] += e2; rne[3] += e3;
-                const uint32_t sp = lut[Bp];
-                if (k - a.f0 < 8) nnA += sp; else nnB += sp;
-                if (PAIRS) {
-                    const uint32_t tt = e0 + (e1 << 2) + (e2 << 4) + (e3 << 6);
-                    // differs, both ends non-null; every such edge is met from both ends: keep the end whose flipped bit is 0
-                    uint32_t ob = (tt | (tt >> 15)) & Bp & Bm;
-                    ob &= k == 0 ? 0x55u : k == 1 ? 0x33u : k == 2 ? 0x0Fu : (((v >> (k - 3)) & 1u) ? 0u : 0xFFu);
-                    while (ob) {
-                        const uint32_t l = (v << 3) + (__ffs(ob) - 1);
-                        ob &= ob - 1;
-                        uint32_t p = seg[l], qq = seg[l ^ (1u << k)];
-                        if (qq < p) { const uint32_t x = p; p = qq; qq = x; }
-                        const uint32_t key = (p << 16) | qq;
-                        if (key != last_key) { last_key = key; note_pair(pa, pf, p, qq); }
-                    }
-                }
+            uint32_t nnL = 0, nnA = 0, nnB = 0;                    // per nibble: non-null neighbours (in-register flips / first 8 / rest)
+            if (a.f0 == 0) {                                       // flips of local bits 0-2 stay inside the vector
+                rob2_flip<PAIRS>(pa, seg, pf, last_key, ring, head, tail, m, __funnelshift_l(m[0], m[0], 16),
+                                 __funnelshift_l(m[1], m[1], 16), __funnelshift_l(m[2], m[2], 16), __funnelshift_l(m[3], m[3], 16),
+                                 Bm, ((Bm & 0x55u) << 1) | ((Bm >> 1) & 0x55u), 0x55u, v, 0u, lut, rne, nnL);
+                rob2_flip<PAIRS>(pa, seg, pf, last_key, ring, head, tail, m, m[1], m[0], m[3], m[2], Bm,
+                                 ((Bm & 0x33u) << 2) | ((Bm >> 2) & 0x33u), 0x33u, v, 1u, lut, rne, nnL);
+                rob2_flip<PAIRS>(pa, seg, pf, last_key, ring, head, tail, m, m[2], m[3], m[0], m[1], Bm,
+                                 ((Bm & 0x0Fu) << 4) | (Bm >> 4), 0x0Fu, v, 2u, lut, rne, nnL);
             }
-            // per genotype: differs = rne half, non-null neighbours = nibble of nnA + nnB;
+#pragma unroll 4
+            for (int k = k_lo; k < k_mid; k++) {
+                const uint32_t pv = (v ^ (1u << (k - 3))) & (n_vec - 1);
+                const uint4 x = sv[pv];
+                rob2_flip<PAIRS>(pa, seg, pf, last_key, ring, head, tail, m, x.x, x.y, x.z, x.w, Bm, nnb[pv],
+                                 pv > v ? 0xFFu : 0u, v, (uint32_t)k, lut, rne, nnA);
+            }
+#pragma unroll 4
+            for (int k = k_mid; k < a.tb; k++) {
+                const uint32_t pv = (v ^ (1u << (k - 3))) & (n_vec - 1);
+                const uint4 x = sv[pv];
+                rob2_flip<PAIRS>(pa, seg, pf, last_key, ring, head, tail, m, x.x, x.y, x.z, x.w, Bm, nnb[pv],
+                                 pv > v ? 0xFFu : 0u, v, (uint32_t)k, lut, rne, nnB);
+            }
+            // per genotype: differs = rne half, non-null neighbours = nibbles of nnL + nnA + nnB;
             // neutral = flips - differs; to null = flips - non-null neighbours.  Runs of equal class are merged.
             uint32_t run = 0, r_acc = 0, d_acc = 0;
 #pragma unroll
@@ -388,12 +449,19 @@ __global__ void __launch_bounds__(R2THREADS, 1) robustness2_kernel(Rob2Args a) {
                 if (p == NULLP) continue;
                 run++;
                 r_acc += n_flip - ((rne[j >> 1] >> (16 * (j & 1))) & 0xFFFFu);
-                d_acc += n_flip - ((nnA >> (4 * j)) & 15u) - ((nnB >> (4 * j)) & 15u);
+                d_acc += n_flip - ((nnL >> (4 * j)) & 15u) - ((nnA >> (4 * j)) & 15u) - ((nnB >> (4 * j)) & 15u);
                 const uint32_t nxt = j < 7 ? (m[(j + 1) >> 1] >> (16 * ((j + 1) & 1))) & 0xFFFFu : NULLP;
                 if (nxt == p) continue;
                 rob2_add(a, cache, n_flip, p, run, r_acc, d_acc);
                 run = 0; r_acc = 0; d_acc = 0;
             }
+        }
+        if (PAIRS && tail != head) {                                // events left in the ring: the tile is about to be replaced
+            __syncwarp();
+            const uint32_t lane = threadIdx.x & 31u;
+            if (lane < tail - head) rob2_events(pa, seg, pf, last_key, ring[(head + lane) & (ROB2_RING - 1)]);
+            head = tail;
+            __syncwarp();
         }
         if (++tiles_done % ROB_FLUSH_TILES == 0) rob2_flush(a, cache, n_flip);
     }
@@ -656,8 +724,8 @@ static gp_status robustness_passes(const uint16_t* d_pheno, int n_bits, uint32_t
     const uint64_t cap = (uint64_t)sm_count() * (v1 ? 2 : 1);
     const unsigned grid = (unsigned)(n_tiles < cap ? n_tiles : cap);
     const size_t smem = v1 ? ((size_t)2 << tb) + ROB_SLOTS * sizeof(RobSlot) + ROB_PF_SLOTS * sizeof(uint32_t)
-                           : ((size_t)2 << tb) + ((size_t)1 << (tb - 3)) + 1024 + ROB_SLOTS * sizeof(Rob2Slot) +
-                                 ROB_PF_SLOTS * sizeof(uint32_t);
+                           : ((size_t)2 << tb) + ((((size_t)1 << (tb - 3)) + 15) & ~(size_t)15) + 1024 + ROB2_SLOTS * sizeof(Rob2Slot) +
+                                 ROB2_PF_SLOTS * sizeof(uint32_t) + (R2THREADS / 32) * ROB2_RING * sizeof(uint32_t);
     if (v1) GP_CUDA(cudaFuncSetAttribute(robustness_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     else if (d_pair_bitmap) GP_CUDA(cudaFuncSetAttribute(robustness2_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     else GP_CUDA(cudaFuncSetAttribute(robustness2_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
