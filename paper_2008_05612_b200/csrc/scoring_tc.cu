@@ -823,7 +823,7 @@ struct Plan {
     uint32_t n_tiles = 0;
     size_t tile_bytes = 0, img_bytes = 0, smem = 0;
     tc::scoring_fn kernel = nullptr;
-    int sms = 0;
+    int sms = 0, threads = 0;
 };
 
 gp_status make_plan(const gp_structures_s* s, const int* mon, int fb, uint32_t n_columns, Plan& p) {
@@ -836,6 +836,7 @@ gp_status make_plan(const gp_structures_s* s, const int* mon, int fb, uint32_t n
     p.tile_bytes = (size_t)TM * (p.narrow ? 64 : 128);
     p.img_bytes = (size_t)p.n_tiles * p.tile_bytes;
     p.smem = (size_t)(MT + NSTAGE) * p.tile_bytes + sizeof(Barriers) + ROWB * sizeof(uint32_t) + 1024 + 64;
+    p.threads = THREADS;
     p.kernel = p.narrow ? scoring_for<64>(p.k_steps) : scoring_for<128>(p.k_steps);
     int dev = 0;
     GP_CUDA(cudaGetDevice(&dev));
@@ -890,7 +891,7 @@ gp_status gp_launch_scoring_tc(const gp_structures_s* s, const gp_hp_params& hp,
         a.hrec = nullptr; a.n_snap = p.n_tiles;
         const unsigned grid = a.n_items < (uint32_t)p.sms ? a.n_items : (uint32_t)p.sms;
         gp_time_begin(GP_KERNEL_SCORING, st);
-        p.kernel<<<grid, THREADS, p.smem, st>>>(a, p.cols);
+        p.kernel<<<grid, p.threads, p.smem, st>>>(a, p.cols);
         gp_time_end(GP_KERNEL_SCORING, st);
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) { gp_set_cuda_error(e, "scoring launch"); result = GP_CUDA_ERROR; break; }
@@ -1001,7 +1002,7 @@ static gp_status gp_launch_map_range(const gp_structures_s* s, const gp_hp_param
         a.hrec = d_rec; a.n_snap = s->n_snap;
         const unsigned grid = a.n_items < (uint32_t)p.sms ? a.n_items : (uint32_t)p.sms;
         gp_time_begin(GP_KERNEL_SCORING, st);
-        p.kernel<<<grid, THREADS, p.smem, st>>>(a, p.cols);
+        p.kernel<<<grid, p.threads, p.smem, st>>>(a, p.cols);
         gp_time_end(GP_KERNEL_SCORING, st);
         CombArgs ca;
         ca.hrec = d_rec; ca.units = s->d_units; ca.class_sym = s->d_class_sym;
