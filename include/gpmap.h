@@ -135,12 +135,20 @@ gp_status gp_enumerate_map_range(const gp_structures_t* s, const gp_energies* en
 gp_status gp_enumerate_simple(const gp_structures_t* s, const gp_energies* en, uint64_t g_begin, uint64_t g_count,
                               uint16_t* d_pheno, int16_t* d_gap, void* stream);
 
-/* a8. Explicit sequences (the paper's SeqRnd path, :510-516, :762-775; its sampling runs :195-204): d_seqs[count][N]
- * letters < alphabet (2 or 20).  Two-letter sequences whose energies fit the int8 weights (same bound as gp_enumerate)
- * run on the tensor cores with the full 2 + N + P feature columns; everything else on the CUDA-core kernel. */
+/* a8 / f3. Explicit sequences (the paper's SeqRnd path, :510-516, :762-775; its sampling runs :195-204 Table 3):
+ * d_seqs[count][N] letters < alphabet (2..20; a letter outside the alphabet is read as the last letter), e symmetric
+ * alphabet x alphabet.  Three kernels, chosen per call, all exact:
+ *   - two-letter sequences whose energies fit the int8 weights (same bound as gp_enumerate): tensor cores, the full
+ *     2 + N + P feature columns against the per-energy weight image (sequence_kernel);
+ *   - any alphabet with (emax - emin) <= 8191 and NBP * (emax - emin) <= 32000 (the seeded 20-letter matrix on every
+ *     BASELINE lattice): tensor cores, the P pair energies of a sequence as two int8 limbs against the 0/-1 contact
+ *     incidence matrix of the lattice (seq20_kernel), limbs recombined on the TMEM read-out;
+ *   - everything else, batches under 128 sequences, and gp_tuning.seq_tensor = 0: the CUDA-core kernel.
+ * The first call on a handle that needs an image allocates it (cudaMalloc). */
 gp_status gp_enumerate_seqs(const gp_structures_t* s, const gp_energies* en, const uint8_t* d_seqs, uint64_t count,
                             uint16_t* d_pheno, int16_t* d_gap, void* stream);
-/* a8. Sequences first..first+count-1 of the counter-based 20-letter generator of DESIGN.md section 4, drawn on chip. */
+/* a8. Sequences first..first+count-1 of the counter-based 20-letter generator of DESIGN.md section 4, drawn on chip; same
+ * kernel choice as gp_enumerate_seqs. */
 gp_status gp_enumerate_seeded(const gp_structures_t* s, const gp_energies* en, uint64_t seed, uint64_t first,
                               uint64_t count, uint16_t* d_pheno, int16_t* d_gap, void* stream);
 /* Host helpers for the same generator: the seeded 20x20 matrix and sequences. */

@@ -6,8 +6,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _ROOT = os.path.dirname(_HERE)
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libgpmap.so")
-SOURCES = ["api.cu", "host_structures.cpp", "scoring_simple.cu", "scoring_tc.cu", "reductions.cu"]
-HEADERS = ["gpmap_internal.h", "device_common.cuh"]
+SOURCES = ["api.cu", "host_structures.cpp", "scoring_simple.cu", "scoring_tc.cu", "scoring_seq20.cu", "reductions.cu"]
+HEADERS = ["gpmap_internal.h", "device_common.cuh", "tc_common.cuh"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-I" + os.path.join(_ROOT, "include"), "-I" + CSRC]
 

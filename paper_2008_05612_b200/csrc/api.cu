@@ -157,6 +157,10 @@ void gp_release_device(gp_structures_s* s) {
         if (w.ready) cudaEventDestroy((cudaEvent_t)w.ready);
     }
     s->wimgs.clear();
+    cudaFree(s->d_pair_img);
+    s->d_pair_img = nullptr;
+    if (s->pair_img_ready) cudaEventDestroy((cudaEvent_t)s->pair_img_ready);
+    s->pair_img_ready = nullptr;
     cudaFree(s->d_units);
     s->d_units = nullptr;
     cudaFree(s->d_host_store);

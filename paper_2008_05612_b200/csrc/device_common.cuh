@@ -47,3 +47,6 @@ gp_status gp_launch_scoring_tc(const gp_structures_s* s, const gp_hp_params& hp,
                                uint16_t* d_pheno, int16_t* d_gap, cudaStream_t st);
 gp_status gp_launch_sequences_tc(const gp_structures_s* s, const gp_hp_params& hp, const uint8_t* d_seqs, uint64_t count,
                                  uint16_t* d_pheno, int16_t* d_gap, cudaStream_t st);
+// scoring_seq20.cu
+gp_status gp_launch_seq20_tc(const gp_structures_s* s, const gp_energies* en, int seeded, const uint8_t* d_seqs, uint64_t seed,
+                             uint64_t first, uint64_t count, uint16_t* d_pheno, int16_t* d_gap, cudaStream_t st);

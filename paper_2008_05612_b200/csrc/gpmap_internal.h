@@ -48,6 +48,8 @@ struct gp_structures_s {
     // of the synchronous gp_enumerate_host.  Compute calls take everything else from the stream-ordered pool.
     mutable std::mutex mu;
     mutable std::vector<gp_weight_image> wimgs;
+    mutable int8_t* d_pair_img = nullptr;    // 0/-1 contact-incidence image of seq20_kernel (lattice only), built once
+    mutable void* pair_img_ready = nullptr;  // cudaEvent_t
     mutable void* d_host_store = nullptr;
     mutable size_t host_store_bytes = 0;
 };

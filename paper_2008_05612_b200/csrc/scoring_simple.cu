@@ -53,7 +53,7 @@ __global__ void __launch_bounds__(128) score_simple_kernel(SimpleArgs a, const i
                 uint32_t l = 0;
                 if (live[h]) {
                     if (SRC == SRC_BITS) l = (uint32_t)(((a.first + q[h]) >> k) & 1ULL);
-                    else if (SRC == SRC_SEQS) l = a.seqs[q[h] * a.N + k];
+                    else if (SRC == SRC_SEQS) l = min((uint32_t)a.seqs[q[h] * a.N + k], (uint32_t)a.alphabet - 1u);  // outside the alphabet = the last letter
                     else l = gp_letter20(a.seed, a.first + q[h], k);
                 }
                 let[(k * 2 + h) * BD + tid] = (uint8_t)l;
@@ -154,6 +154,25 @@ extern "C" gp_status gp_enumerate_simple(const gp_structures_t* s, const gp_ener
     return launch_simple(s, en, SRC_BITS, nullptr, 0, g_begin, g_count, d_pheno, d_gap, (cudaStream_t)stream);
 }
 
+// any-alphabet sequences: tensor cores (scoring_seq20.cu) when the handle's tuning allows, the batch is worth a launch and
+// the energies are eligible; the CUDA-core kernel otherwise.  Arguments are validated here for both.
+static gp_status seqs_any_alphabet(const gp_structures_t* s, const gp_energies* en, int seeded, const uint8_t* d_seqs,
+                                   uint64_t seed, uint64_t first, uint64_t count, uint16_t* d_pheno, int16_t* d_gap,
+                                   cudaStream_t st) {
+    if (s && en && en->e && d_pheno && s->tuning.seq_tensor && count >= 128 && s->device >= 0 && en->alphabet >= 2 &&
+        en->alphabet <= 20 && en->threshold >= 1 && (seeded ? en->alphabet == 20 : d_seqs != nullptr)) {
+        bool symmetric = true;
+        for (int i = 0; i < en->alphabet && symmetric; i++)
+            for (int j = 0; j < i; j++)
+                if (en->e[i * en->alphabet + j] != en->e[j * en->alphabet + i]) { symmetric = false; break; }
+        if (symmetric) {
+            gp_status stt = gp_launch_seq20_tc(s, en, seeded, d_seqs, seed, first, count, d_pheno, d_gap, st);
+            if (stt != GP_UNSUPPORTED_LATTICE) return stt;
+        }
+    }
+    return launch_simple(s, en, seeded ? SRC_SEEDED : SRC_SEQS, d_seqs, seed, first, count, d_pheno, d_gap, st);
+}
+
 extern "C" gp_status gp_enumerate_seqs(const gp_structures_t* s, const gp_energies* en, const uint8_t* d_seqs,
                                        uint64_t count, uint16_t* d_pheno, int16_t* d_gap, void* stream) {
     // two-letter sequences whose energies fit the int8 weights go to the tensor cores (sequence_kernel)
@@ -163,10 +182,10 @@ extern "C" gp_status gp_enumerate_seqs(const gp_structures_t* s, const gp_energi
         gp_status st = gp_launch_sequences_tc(s, hp, d_seqs, count, d_pheno, d_gap, (cudaStream_t)stream);
         if (st != GP_UNSUPPORTED_LATTICE) return st;
     }
-    return launch_simple(s, en, SRC_SEQS, d_seqs, 0, 0, count, d_pheno, d_gap, (cudaStream_t)stream);
+    return seqs_any_alphabet(s, en, 0, d_seqs, 0, 0, count, d_pheno, d_gap, (cudaStream_t)stream);
 }
 
 extern "C" gp_status gp_enumerate_seeded(const gp_structures_t* s, const gp_energies* en, uint64_t seed, uint64_t first,
                                          uint64_t count, uint16_t* d_pheno, int16_t* d_gap, void* stream) {
-    return launch_simple(s, en, SRC_SEEDED, nullptr, seed, first, count, d_pheno, d_gap, (cudaStream_t)stream);
+    return seqs_any_alphabet(s, en, 1, nullptr, seed, first, count, d_pheno, d_gap, (cudaStream_t)stream);
 }

@@ -239,28 +239,66 @@ def test_threshold_sweep(oracle_structures):
     assert f2.tolist() == [16, 16] and h2[:, 0].tolist() == [16, 16]
 
 
-@pytest.mark.parametrize("dims,count", [((6, 6, 1), 2049), ((5, 5, 1), 3000), ((3, 3, 3), 600)])
-def test_twenty_letter_cuda_core_path_on_large_lattices(oracle_structures, dims, count):
-    """a8 off the 4x4 box (the paper's MJ rows are 6x6 and 3x3x3): seeded 20-letter sequences and the
-    seeded matrix, every sequence against all directed structures, ids and gaps against the oracle; then explicit
-    sequences with another matrix and a threshold."""
+@pytest.mark.parametrize("tensor", [1, 0])
+@pytest.mark.parametrize("dims,count", [((6, 6, 1), 2049), ((5, 5, 1), 3000), ((3, 3, 3), 600), ((4, 4, 1), 1000)])
+def test_twenty_letter_sequences_on_large_lattices(oracle_structures, dims, count, tensor):
+    """a8 / f3 off the 4x4 box (the paper's MJ rows are 6x6 and 3x3x3): seeded 20-letter sequences and
+    the seeded matrix, every sequence against all directed structures, ids and gaps against the oracle — on the tensor
+    cores (seq20_kernel: two int8 limbs against the 0/-1 contact incidence matrix) and on the CUDA-core kernel; then
+    explicit sequences with another matrix (positive entries too) and a threshold; then a matrix whose spread is beyond
+    the limbs' int16 range, which must fall back to the CUDA-core kernel and still be exact."""
     S, O = lib_structures(dims), oracle_structures(*dims)
-    seed = workloads.SEED
-    M = gpmap.seeded_matrix(seed)
-    first = (1 << 33) + 12345
-    ph = torch.empty(count, dtype=torch.uint16, device="cuda")
-    gap = torch.empty(count, dtype=torch.int16, device="cuda")
-    S.enumerate_seeded(seed, first, count, ph, gap, e=M)
-    seqs = orc.seeded_sequences(seed, first, count, S.N)
-    assert np.array_equal(gpmap.seeded_sequences(seed, first, 64, S.N), seqs[:64])
-    ph_o, gap_o = O.enumerate_seqs(seqs, orc.seeded_matrix(seed), 20)
-    assert np.array_equal(ph.cpu().numpy(), ph_o), dims
-    assert np.array_equal(gap.cpu().numpy().astype(np.int32), np.maximum(gap_o, -32768)), dims
-    seqs2 = workloads.random_sequences(count // 2, S.N, 20, seed=3)
-    M2 = workloads.random_symmetric_matrix(20, -300, 40)
-    ph2 = torch.empty(count // 2, dtype=torch.uint16, device="cuda")
-    S.enumerate_seqs(torch.from_numpy(seqs2).cuda(), ph2, None, e=M2, alphabet=20, threshold=4)
-    assert np.array_equal(ph2.cpu().numpy(), O.enumerate_seqs(seqs2, M2, 20, threshold=4, want_gap=False)), dims
+    S.tune(seq_tensor=tensor)
+    try:
+        seed = workloads.SEED
+        M = gpmap.seeded_matrix(seed)
+        first = (1 << 33) + 12345
+        ph = torch.empty(count, dtype=torch.uint16, device="cuda")
+        gap = torch.empty(count, dtype=torch.int16, device="cuda")
+        S.enumerate_seeded(seed, first, count, ph, gap, e=M)
+        seqs = orc.seeded_sequences(seed, first, count, S.N)
+        assert np.array_equal(gpmap.seeded_sequences(seed, first, 64, S.N), seqs[:64])
+        ph_o, gap_o = O.enumerate_seqs(seqs, orc.seeded_matrix(seed), 20)
+        assert np.array_equal(ph.cpu().numpy(), ph_o), dims
+        assert np.array_equal(gap.cpu().numpy().astype(np.int32), np.maximum(gap_o, -32768)), dims
+        n2 = count // 2
+        seqs2 = workloads.random_sequences(n2, S.N, 20, seed=3)
+        seqs2[0, :] = 7                                       # a homopolymer: every structure ties -> null
+        M2 = workloads.random_symmetric_matrix(20, -300, 40)
+        ph2 = torch.empty(n2, dtype=torch.uint16, device="cuda")
+        gap2 = torch.empty(n2, dtype=torch.int16, device="cuda")
+        S.enumerate_seqs(torch.from_numpy(seqs2).cuda(), ph2, gap2, e=M2, alphabet=20, threshold=4)
+        ph2_o, gap2_o = O.enumerate_seqs(seqs2, M2, 20, threshold=4)
+        assert np.array_equal(ph2.cpu().numpy(), ph2_o), dims
+        assert np.array_equal(gap2.cpu().numpy().astype(np.int32), np.maximum(gap2_o, -32768)), dims
+        if S.D > 1:
+            assert ph2_o[0] == 0xFFFF
+        # a 7-letter alphabet with a wide spread: (emax - emin) * NBP > 32000, CUDA-core fallback inside the same call
+        wide = int(30000 // S.NBP)
+        M3 = workloads.random_symmetric_matrix(7, -wide, wide, seed=9)
+        if (int(M3.max()) - int(M3.min())) * S.NBP > 32000:
+            seqs3 = workloads.random_sequences(300, S.N, 7, seed=4)
+            ph3 = torch.empty(300, dtype=torch.uint16, device="cuda")
+            S.enumerate_seqs(torch.from_numpy(seqs3).cuda(), ph3, None, e=M3, alphabet=7)
+            assert np.array_equal(ph3.cpu().numpy(), O.enumerate_seqs(seqs3, M3, 7, want_gap=False)), dims
+    finally:
+        S.tune(seq_tensor=1)
+
+
+def test_twenty_letter_paths_agree_on_a_large_batch():
+    """2^17 seeded 20-letter sequences on 6x6: tensor-core and CUDA-core kernels give identical ids and gaps."""
+    S = lib_structures((6, 6, 1))
+    n = 1 << 17
+    M = gpmap.seeded_matrix(workloads.SEED)
+    out = []
+    for tensor in (1, 0):
+        S.tune(seq_tensor=tensor)
+        ph = torch.empty(n, dtype=torch.uint16, device="cuda")
+        gap = torch.empty(n, dtype=torch.int16, device="cuda")
+        S.enumerate_seeded(workloads.SEED, 77, n, ph, gap, e=M)
+        out.append((ph, gap))
+    S.tune(seq_tensor=1)
+    assert torch.equal(out[0][0].view(torch.int16), out[1][0].view(torch.int16)) and torch.equal(out[0][1], out[1][1])
 
 
 def test_small_explicit_hp_batches_take_the_cuda_core_branch(oracle_structures):

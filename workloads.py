@@ -39,6 +39,7 @@ def random_sequences(count, n, alphabet, seed=SEED):
 
 
 def random_symmetric_matrix(alphabet, lo, hi, seed=SEED):
+    """Symmetric integer matrix, entries uniform in [lo, hi] (a stand-in for a contact-energy table)."""
     rng = np.random.default_rng(seed + 1)
     m = rng.integers(lo, hi + 1, size=(alphabet, alphabet), dtype=np.int32)
     return np.triu(m) + np.triu(m, 1).T
