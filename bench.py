@@ -297,14 +297,14 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
-def workload_config(lattice, G, D, C, K, n):
+def workload_config(lattice, G, D, C, K, n, parallelism="independent prefix tiles per rank, no collective"):
     """The `config` object: identical keys in both arms."""
     return {"workload": "%s HP genotype-prefix tile: 2^%d genotypes x %d directed structures, then designability + "
                         "neighbour pass over the tile" % (lattice, G, D),
             "lattice": lattice, "log2_genotypes": G, "D": D, "C": C, "features_K": K,
             "l2": "inputs larger than L2 (per step: %.0f MB phenotype tile, fresh seeded prefix, weight images rebuilt)"
                   % (2.0 * n / 1e6),
-            "parallelism": "independent prefix tiles per rank, no collective"}
+            "parallelism": parallelism}
 
 
 def full_map_leg(lattice, stream, cpu_check=True):
@@ -438,12 +438,14 @@ def run_rows(args):
             t = dev_time(lambda: S.enumerate_seqs(seqs[:c], ph[:c], None, e=e, alphabet=2), reps=1)
             rows.append(dict(row="f3 sampling, random HP sequences (%s)" % label, config="%s, %d sequences" % (name, c), seconds=t,
                              evals_per_s=c * S.D / t, seconds_per_sequence=t / c, paper_gpu_seconds_per_sequence=paper_hp))
-        S.tune(seq_tensor=1)
-        c = 1 << 17
         M = gpmap.seeded_matrix(SEED)
-        t = dev_time(lambda: S.enumerate_seeded(SEED, 0, c, ph[:c], e=M), reps=1)
-        rows.append(dict(row="f3 sampling, seeded 20-letter sequences", config="%s, %d sequences" % (name, c), seconds=t,
-                         evals_per_s=c * S.D / t, seconds_per_sequence=t / c, paper_gpu_seconds_per_sequence=paper_mj))
+        for label, on, c in (("tensor cores, two int8 limbs", 1, 1 << 20), ("CUDA cores", 0, 1 << 17)):
+            S.tune(seq_tensor=on)
+            t = dev_time(lambda: S.enumerate_seeded(SEED, 0, c, ph[:c], e=M), reps=1)
+            rows.append(dict(row="f3 sampling, seeded 20-letter sequences (%s)" % label, config="%s, %d sequences" % (name, c),
+                             seconds=t, evals_per_s=c * S.D / t, seconds_per_sequence=t / c,
+                             paper_gpu_seconds_per_sequence=paper_mj))
+        S.tune(seq_tensor=1)
         del seqs, ph
     S = structs["4x4"]
     M = gpmap.seeded_matrix(SEED)
@@ -451,8 +453,14 @@ def run_rows(args):
     ph = torch.empty(n, dtype=torch.uint16, device="cuda")
     t = dev_time(lambda: S.enumerate_seeded(SEED, 0, n, ph, e=M), reps=1)
     hist = gpmap.designability(ph, S.C)
-    rows.append(dict(row="a8 gp_enumerate_seeded (20 letters, seeded matrix)", config="4x4, 2^30 sequences", seconds=t,
+    rows.append(dict(row="a8 gp_enumerate_seeded (20 letters, seeded matrix; tensor cores)", config="4x4, 2^30 sequences", seconds=t,
                      evals_per_s=n * S.D / t, folding_fraction=1.0 - hist[S.C].item() / n))
+    S.tune(seq_tensor=0)
+    m = 1 << 28
+    t = dev_time(lambda: S.enumerate_seeded(SEED, 0, m, ph[:m], e=M), reps=1)
+    rows.append(dict(row="a8 gp_enumerate_seeded (20 letters, seeded matrix; CUDA cores)", config="4x4, 2^28 sequences", seconds=t,
+                     evals_per_s=m * S.D / t))
+    S.tune(seq_tensor=1)
     for r in rows:
         print(json.dumps(r), flush=True)
     if args.out:
@@ -496,7 +504,19 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
+    # N > 1: the step is ONE sub-cube of 2^(G+q) genotypes sharded over the ranks on its top q bits:
+    # rank-local scoring, rank-local neighbour pass, hypercube exchange of the shards for the q rank-selecting bits,
+    # all_reduce of the counts, OR-reduce of the pair bitmap.  Per-rank work is fixed: weak scaling.
+    sharded = world > 1 and (world & (world - 1)) == 0 and G + world.bit_length() - 1 <= N and not args.full
+    if sharded:
+        from paper_2008_05612_b200 import sharding
+        ops, comm, q = sharding.LibOps(), sharding.DistComm(), world.bit_length() - 1
+
     def step(i):
+        if sharded:
+            base = tile_begin(i, 0, 1, G + q, N)
+            S.enumerate(base + rank * n, n, pheno, stream=stream)                      # a1-a4 on the rank's shard
+            return sharding.reduce_store_sharded(ops, comm, pheno, G + q, C)           # a5 + a6 across the shards
         b = tile_begin(i, rank, world, G, N)
         if args.full:
             S.enumerate_map(pheno, stream=stream)                     # a1-a4, whole map through the reversal identity
@@ -531,7 +551,7 @@ def run_ours(args):
         t = torch.tensor([ms], dtype=torch.float64, device="cuda")
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         ms = float(t.item())
-    folding = int(n - hist[C].item())
+    folding = int(n - hist[C].item()) if not sharded else None
     evals_step = float(n) * D * world
     value = evals_step * args.steps / (ms * 1e-3)
 
@@ -588,6 +608,11 @@ def run_ours(args):
                 "peak_source": "gp_probe_i8_peak(k_steps=%d): MMA-only tcgen05.mma kind::i8 stream, measured in this run" % k_steps,
                 "peak_i8_measured": {"TOPs": peak_i8, "clk_per_mma": probe_clk, "sm_mhz": probe_mhz},
                 "frac_issued": achieved * ops_issued / ops_exec / peak_i8,
+                # the MMA-only probe draws more power and runs at a lower SM clock than the scoring kernel does; per clock
+                # (probe peak scaled to the clock sampled during the timed region) the issued fraction is what the ncu
+                # tensor-pipe-active counter measures
+                "frac_issued_per_clock": (achieved * ops_issued / ops_exec / (peak_i8 * clocks["sm_mhz"] / probe_mhz)
+                                          if clocks and clocks.get("sm_mhz") and probe_mhz else None),
                 "ncu_tensor_active": prof["tensor_active_pct"] / 100.0 if prof and prof["tensor_active_pct"] is not None else None,
                 "frac_of_nominal_4500": achieved / 4500.0, "frac_of_2x_bf16_burst": achieved / (2.0 * bf16_burst),
                 "frac_of_2x_bf16_sustained": achieved / (2.0 * bf16_sus), "bf16_peaks_source": src,
@@ -650,9 +675,13 @@ def run_ours(args):
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "s8 x s8 -> s32", "data": "synthetic",
-            "config": workload_config(args.lattice, G, D, C, S.K, n),
+            "config": workload_config(args.lattice, G, D, C, S.K, n, *(["one sub-cube of 2^%d genotypes per step sharded over %d ranks on its top %d "
+                                                                        "bits: local scoring, hypercube shard exchange for the neighbour pass "
+                                                                        "(%d bytes sent per rank and step), all_reduce of counts, OR-reduce of the "
+                                                                        "pair bitmap" % (G + q, world, q, sharding.exchange_bytes_per_rank(G + q, world, C))]
+                                                                       if sharded else [])),
             "full_map_wall_s_extrapolated_from_tiles": total_evals_map / value * world if value else None,
-            "folding_fraction_last_tile": folding / float(n),
+            "folding_fraction_last_tile": folding / float(n) if folding is not None else None,
             "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline, "other_kernels": other,
             "whole_map_3x3x3": whole, "full_6x6": full, "cpu_baseline": cpu}
     print(json.dumps(line), flush=True)

@@ -73,7 +73,7 @@ class LibOps:
         self.g.pair_bitmap_or(dst, src, n_classes)
 
     def pair_bitmap_count(self, bitmap, n_classes):
-        return int(self.g.pair_bitmap_count(bitmap, n_classes).item())
+        return self.g.pair_bitmap_count(bitmap, n_classes)   # device tensor: no host synchronisation on the path
 
 
 class DistComm:

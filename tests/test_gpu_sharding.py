@@ -34,6 +34,7 @@ def test_sharded_5x5_map_equals_single_rank(world):
              for r in range(world)]
     hist, R, D, O, pairs = sharding.combine_partials(ops, parts, C)
     assert torch.equal(hist, hist1) and torch.equal(R, R1) and torch.equal(D, D1) and torch.equal(O, O1)
+    pairs = int(pairs)
     assert pairs == int(pc1)
     gold = read_whole_maps()["5x5"]
     assert (int(R.sum()), int(D.sum()), int(O.sum()), pairs) == (gold["sumR"], gold["sumD"], gold["sumO"], gold["pairs"])
