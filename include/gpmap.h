@@ -79,7 +79,7 @@ typedef struct {
     int32_t fold_bits;   /* gp_enumerate: low genotype bits kept as contraction columns, 9..22 (default 15)          */
     int32_t sym_bits;    /* gp_enumerate_map*: k, monomers free at each chain end inside one image, 5..11 (default 7) */
     int32_t narrow_rows; /* 1 (default): 64-byte operand rows when the folded contraction has at most 64 columns     */
-    int32_t seq_tensor;  /* 1 (default): gp_enumerate_seqs runs on the tensor cores where it can; 0: CUDA cores      */
+    int32_t seq_tensor;  /* gp_enumerate_seqs / _seeded: 1 (default) tensor cores where they pay, 2 wherever eligible, 0 never */
 } gp_tuning;
 gp_status gp_tuning_get(const gp_structures_t* s, gp_tuning* out);
 /* GP_INVALID_ARG if a field is out of range (nothing is changed then).  Rebuilds the handle's unit table of
@@ -143,6 +143,8 @@ gp_status gp_enumerate_simple(const gp_structures_t* s, const gp_energies* en, u
  *   - any alphabet with (emax - emin) <= 8191 and NBP * (emax - emin) <= 32000 (the seeded 20-letter matrix on every
  *     BASELINE lattice): tensor cores, the P pair energies of a sequence as two int8 limbs against the 0/-1 contact
  *     incidence matrix of the lattice (seq20_kernel), limbs recombined on the TMEM read-out;
+ *     by default only on lattices with at least 4096 directed structures (the per-sequence limb rows need a long
+ *     structure list to pay; gp_tuning.seq_tensor = 2 takes it wherever eligible);
  *   - everything else, batches under 128 sequences, and gp_tuning.seq_tensor = 0: the CUDA-core kernel.
  * The first call on a handle that needs an image allocates it (cudaMalloc). */
 gp_status gp_enumerate_seqs(const gp_structures_t* s, const gp_energies* en, const uint8_t* d_seqs, uint64_t count,

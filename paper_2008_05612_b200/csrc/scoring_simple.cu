@@ -159,7 +159,10 @@ extern "C" gp_status gp_enumerate_simple(const gp_structures_t* s, const gp_ener
 static gp_status seqs_any_alphabet(const gp_structures_t* s, const gp_energies* en, int seeded, const uint8_t* d_seqs,
                                    uint64_t seed, uint64_t first, uint64_t count, uint16_t* d_pheno, int16_t* d_gap,
                                    cudaStream_t st) {
-    if (s && en && en->e && d_pheno && s->tuning.seq_tensor && count >= 128 && s->device >= 0 && en->alphabet >= 2 &&
+    // auto (1): the limb kernel pays a per-sequence row build that only a long structure list amortises (4x4, D = 69: the
+    // CUDA-core kernel is 3x faster; 6x6 / 3x3x3: the tensor cores are 20x faster)
+    const bool want_tc = s && (s->tuning.seq_tensor == 2 || (s->tuning.seq_tensor == 1 && s->D >= 4096));
+    if (want_tc && en && en->e && d_pheno && count >= 128 && s->device >= 0 && en->alphabet >= 2 &&
         en->alphabet <= 20 && en->threshold >= 1 && (seeded ? en->alphabet == 20 : d_seqs != nullptr)) {
         bool symmetric = true;
         for (int i = 0; i < en->alphabet && symmetric; i++)

@@ -693,7 +693,7 @@ extern "C" gp_status gp_tuning_get(const gp_structures_t* s, gp_tuning* out) {
 extern "C" gp_status gp_tuning_set(gp_structures_t* s, const gp_tuning* t) {
     if (!s || !t) return GP_INVALID_ARG;
     if (t->fold_bits < 9 || t->fold_bits > tc::MAX_FB || t->sym_bits < 5 || 2 * t->sym_bits > tc::MAX_FB) return GP_INVALID_ARG;
-    if ((t->narrow_rows | 1) != 1 || (t->seq_tensor | 1) != 1) return GP_INVALID_ARG;
+    if ((t->narrow_rows | 1) != 1 || t->seq_tensor < 0 || t->seq_tensor > 2) return GP_INVALID_ARG;
     const bool rebuild = t->sym_bits != s->tuning.sym_bits;
     const gp_tuning old = s->tuning;
     s->tuning = *t;

@@ -50,7 +50,7 @@ def test_tuning_and_map_units_host_side():
     pairs first; every genotype of the map belongs to exactly one unit."""
     S = gpmap.Structures(4, 4)
     assert S.tuning() == dict(fold_bits=15, sym_bits=7, narrow_rows=1, seq_tensor=1)
-    for bad in (dict(fold_bits=8), dict(fold_bits=23), dict(sym_bits=4), dict(sym_bits=12), dict(narrow_rows=2)):
+    for bad in (dict(fold_bits=8), dict(fold_bits=23), dict(sym_bits=4), dict(sym_bits=12), dict(narrow_rows=2), dict(seq_tensor=3)):
         with pytest.raises(gpmap.GpError) as ei:
             S.tune(**bad)
         assert ei.value.status == 1 and S.tuning()["fold_bits"] == 15
