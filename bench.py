@@ -439,7 +439,7 @@ def run_rows(args):
             rows.append(dict(row="f3 sampling, random HP sequences (%s)" % label, config="%s, %d sequences" % (name, c), seconds=t,
                              evals_per_s=c * S.D / t, seconds_per_sequence=t / c, paper_gpu_seconds_per_sequence=paper_hp))
         M = gpmap.seeded_matrix(SEED)
-        for label, on, c in (("tensor cores, two int8 limbs", 1, 1 << 20), ("CUDA cores", 0, 1 << 17)):
+        for label, on, c in (("tensor cores, two int8 limbs", 2, 1 << 20), ("CUDA cores", 0, 1 << 17)):
             S.tune(seq_tensor=on)
             t = dev_time(lambda: S.enumerate_seeded(SEED, 0, c, ph[:c], e=M), reps=1)
             rows.append(dict(row="f3 sampling, seeded 20-letter sequences (%s)" % label, config="%s, %d sequences" % (name, c),
@@ -453,13 +453,13 @@ def run_rows(args):
     ph = torch.empty(n, dtype=torch.uint16, device="cuda")
     t = dev_time(lambda: S.enumerate_seeded(SEED, 0, n, ph, e=M), reps=1)
     hist = gpmap.designability(ph, S.C)
-    rows.append(dict(row="a8 gp_enumerate_seeded (20 letters, seeded matrix; tensor cores)", config="4x4, 2^30 sequences", seconds=t,
-                     evals_per_s=n * S.D / t, folding_fraction=1.0 - hist[S.C].item() / n))
-    S.tune(seq_tensor=0)
+    rows.append(dict(row="a8 gp_enumerate_seeded (20 letters, seeded matrix; default = CUDA cores at D = 69)", config="4x4, 2^30 sequences",
+                     seconds=t, evals_per_s=n * S.D / t, folding_fraction=1.0 - hist[S.C].item() / n))
+    S.tune(seq_tensor=2)
     m = 1 << 28
     t = dev_time(lambda: S.enumerate_seeded(SEED, 0, m, ph[:m], e=M), reps=1)
-    rows.append(dict(row="a8 gp_enumerate_seeded (20 letters, seeded matrix; CUDA cores)", config="4x4, 2^28 sequences", seconds=t,
-                     evals_per_s=m * S.D / t))
+    rows.append(dict(row="a8 gp_enumerate_seeded (20 letters, seeded matrix; forced onto the tensor cores)", config="4x4, 2^28 sequences",
+                     seconds=t, evals_per_s=m * S.D / t))
     S.tune(seq_tensor=1)
     for r in rows:
         print(json.dumps(r), flush=True)
