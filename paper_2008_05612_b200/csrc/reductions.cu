@@ -63,15 +63,12 @@ __global__ void __launch_bounds__(1024) hist_kernel(const uint16_t* __restrict__
 // ---------------------------------------------------------------------------------------------------------------
 // a6. Neighbour pass, bit-tiled.  The n_bits flips are handled in passes; each pass reads the
 // store ONCE.  A block stages a tile of 2^tb phenotypes in shared memory: 2^h segments (all values of the h "spread"
-// genotype bits hi_pos..hi_pos+h-1) of 2^c consecutive ids each (c = tb - h >= 3, so a segment is >= 16 B and loads
-// stay vectorised / coalesced).  Pass 0 has h = 0 and flips the tb low bits; every later pass flips its own h spread
-// bits, all on chip.  n_bits = 36, tb = 15: 15 + 8 + 8 + 5 bits = 4 passes instead of 24 partner sweeps.
-// A thread owns 8 consecutive ids (one 16-byte shared-memory vector); flips of local bits 0-2 stay inside the vector,
-// higher local bits are one LDS.128 of the partner vector.
+// genotype bits hi_pos..hi_pos+h-1) of 2^c consecutive ids each (c = tb - h; 128-byte segments when the tile allows,
+// never under 16 bytes, so loads stay vectorised / coalesced).  Pass 0 has h = 0 and flips the tb low bits; every later
+// pass flips its own h spread bits, all on chip.  n_bits = 36, tb = 16: 16 + 10 + 10 bits = 3 passes instead of 20
+// partner sweeps.  A thread owns 8 consecutive ids (one 16-byte shared-memory vector); flips of local bits 0-2 stay
+// inside the vector, higher local bits are one LDS.128 of the partner vector.
 // ---------------------------------------------------------------------------------------------------------------
-constexpr int ROB_TB_MAX = 15;      // 2^15 phenotypes = 64 KB of shared memory per block, two blocks per SM
-constexpr int RTHREADS = 512;
-
 struct RobArgs {
     const uint16_t* pheno;
     int n_bits;
@@ -81,26 +78,15 @@ struct RobArgs {
     int tb, c, h, hi_pos, f0;  // tile bits, contiguous low bits, spread bits, their position, first local bit to flip
 };
 
-constexpr uint32_t ROB_PF_SLOTS = 1024;  // per-block filter of recently recorded class pairs (shared memory)
-
-__device__ __forceinline__ void note_pair(const RobArgs& a, uint32_t* pf, uint32_t p, uint32_t q) {
+// record the connected pair (p, q) in the C x C bitmap (tiny-store and cross-shard kernels; the tile kernel has its own
+// filtered path)
+__device__ __forceinline__ void note_pair(const RobArgs& a, uint32_t p, uint32_t q) {
     if (q < p) { const uint32_t t = p; p = q; q = t; }
     if (q >= a.C) return;
-    if (pf) {
-        const uint32_t key = (p << 16) | q;
-        uint32_t* slot = pf + ((key * 2654435761u) >> 22);
-        if (*(volatile uint32_t*)slot == key) return;  // seen by this block already (racy update is harmless: the bitmap is the truth)
-        *(volatile uint32_t*)slot = key;
-    }
-    uint64_t bit = (uint64_t)p * a.C + q;
+    const uint64_t bit = (uint64_t)p * a.C + q;
     uint32_t* w = a.bitmap + (bit >> 5);
-    uint32_t m = 1u << (bit & 31);
+    const uint32_t m = 1u << (bit & 31);
     if (!(*(volatile uint32_t*)w & m)) atomicOr(w, m);
-}
-
-// bit 15 / bit 31 of the result are set iff the low / high 16-bit half of x is zero (exact: no carry crosses the halves)
-__device__ __forceinline__ uint32_t zero_halves(uint32_t x) {
-    return ~(((x & 0x7FFF7FFFu) + 0x7FFF7FFFu) | x) & 0x80008000u;
 }
 
 __device__ __forceinline__ void unpack8(const uint4& x, uint32_t (&q)[8]) {
@@ -108,134 +94,10 @@ __device__ __forceinline__ void unpack8(const uint4& x, uint32_t (&q)[8]) {
     q[4] = x.z & 0xFFFF; q[5] = x.z >> 16; q[6] = x.w & 0xFFFF; q[7] = x.w >> 16;
 }
 
-// Per-block direct-mapped cache of per-class counts in shared memory: 3 shared atomics per flushed run instead of 3
-// 64-bit global atomics (which serialise in L2 on the popular classes).  A run whose slot is taken by another class
-// goes straight to global memory.  The cache is written back every ROB_FLUSH_TILES tiles (u32 counters) and at the end.
-constexpr uint32_t ROB_SLOTS = 2048;
-constexpr uint32_t ROB_FLUSH_TILES = 64;
-struct RobSlot { uint32_t key, r, d, o; };
-
-__device__ __forceinline__ void rob_add(const RobArgs& a, RobSlot* cache, uint32_t p, uint32_t r, uint32_t d, uint32_t o) {
-    if (p >= a.C) return;                            // an id the caller's n_classes does not cover: skipped, like hist_kernel
-    RobSlot* s = cache + ((p * 2654435761u) >> 21);  // 11 bits
-    uint32_t k = s->key;
-    if (k == NULLP) k = atomicCAS(&s->key, NULLP, p), k = (k == NULLP) ? p : k;
-    if (k == p) {
-        if (r) atomicAdd(&s->r, r);
-        if (d) atomicAdd(&s->d, d);
-        if (o) atomicAdd(&s->o, o);
-    } else {
-        if (r) atomicAdd(&a.R[p], (unsigned long long)r);
-        if (d) atomicAdd(&a.Dl[p], (unsigned long long)d);
-        if (o) atomicAdd(&a.O[p], (unsigned long long)o);
-    }
-}
-
-__device__ __forceinline__ void rob_flush(const RobArgs& a, RobSlot* cache) {
-    __syncthreads();
-    for (uint32_t i = threadIdx.x; i < ROB_SLOTS; i += blockDim.x) {
-        RobSlot s = cache[i];
-        if (s.key != NULLP) {
-            if (s.r) atomicAdd(&a.R[s.key], (unsigned long long)s.r);
-            if (s.d) atomicAdd(&a.Dl[s.key], (unsigned long long)s.d);
-            if (s.o) atomicAdd(&a.O[s.key], (unsigned long long)s.o);
-        }
-        cache[i] = RobSlot{NULLP, 0, 0, 0};
-    }
-    __syncthreads();
-}
-
-__global__ void __launch_bounds__(RTHREADS, 2) robustness_kernel(RobArgs a) {
-    extern __shared__ __align__(16) uint16_t seg[];
-    RobSlot* cache = reinterpret_cast<RobSlot*>(seg + ((size_t)1 << a.tb));
-    uint32_t* pf = reinterpret_cast<uint32_t*>(cache + ROB_SLOTS);
-    for (uint32_t i = threadIdx.x; i < ROB_SLOTS; i += blockDim.x) cache[i] = RobSlot{NULLP, 0, 0, 0};
-    for (uint32_t i = threadIdx.x; i < ROB_PF_SLOTS; i += blockDim.x) pf[i] = 0xFFFFFFFFu;
-    uint32_t tiles_done = 0;
-    const uint32_t n_vec = 1u << (a.tb - 3);                       // 16-byte vectors per tile
-    const uint64_t n_tiles = 1ULL << (a.n_bits - a.tb);
-    const uint32_t cmask = (1u << a.c) - 1u;
-    const int lo_outer = a.hi_pos - a.c;                           // outer-index bits that sit below the spread bits
-    const int n_flip = a.tb - a.f0;
-    uint4* sv = reinterpret_cast<uint4*>(seg);
-    for (uint64_t t = blockIdx.x; t < n_tiles; t += gridDim.x) {
-        const uint64_t base = ((t & ((1ULL << lo_outer) - 1ULL)) << a.c) | ((t >> lo_outer) << (a.hi_pos + a.h));
-        __syncthreads();
-        for (uint32_t v = threadIdx.x; v < n_vec; v += RTHREADS) {
-            const uint32_t l = v << 3;
-            const uint64_t g = base | (l & cmask) | ((uint64_t)(l >> a.c) << a.hi_pos);
-            sv[v] = __ldg(reinterpret_cast<const uint4*>(a.pheno + g));
-        }
-        __syncthreads();
-        for (uint32_t v = threadIdx.x; v < n_vec; v += RTHREADS) {
-            // 8 genotypes as 4 words of two 16-bit class ids; counters packed the same way (a count is at most 36)
-            const uint4 mv = sv[v];
-            const uint32_t m[4] = {mv.x, mv.y, mv.z, mv.w};
-            uint32_t mnz[4], rc[4] = {0, 0, 0, 0}, dc[4] = {0, 0, 0, 0};
-#pragma unroll
-            for (int w = 0; w < 4; w++) mnz[w] = zero_halves(~m[w]);          // which of mine are null
-            if ((mnz[0] & mnz[1] & mnz[2] & mnz[3]) == 0x80008000u) continue;  // all 8 null
-            for (int k = a.f0; k < a.tb; k++) {
-                uint32_t q[4];
-                if (k == 0) {
-#pragma unroll
-                    for (int w = 0; w < 4; w++) q[w] = __funnelshift_l(m[w], m[w], 16);
-                } else if (k == 1) {
-                    q[0] = m[1]; q[1] = m[0]; q[2] = m[3]; q[3] = m[2];
-                } else if (k == 2) {
-                    q[0] = m[2]; q[1] = m[3]; q[2] = m[0]; q[3] = m[1];
-                } else {
-                    const uint4 x = sv[v ^ (1u << (k - 3))];
-                    q[0] = x.x; q[1] = x.y; q[2] = x.z; q[3] = x.w;
-                }
-                uint32_t other = 0, ez[4], nz[4];
-#pragma unroll
-                for (int w = 0; w < 4; w++) {
-                    ez[w] = zero_halves(q[w] ^ m[w]);     // neighbour in the same class
-                    nz[w] = zero_halves(~q[w]);           // neighbour null
-                    rc[w] += ez[w] >> 15;
-                    dc[w] += nz[w] >> 15;
-                    other |= ~(ez[w] | nz[w] | mnz[w]) & 0x80008000u;
-                }
-                if (a.bitmap && other) {
-                    // every edge between two different non-null classes is met from both ends: keep the end whose
-                    // flipped bit is 0, gather the flagged genotypes into one 8-bit mask and walk it
-                    uint32_t ob = 0;
-#pragma unroll
-                    for (int w = 0; w < 4; w++) {
-                        const uint32_t o = ~(ez[w] | nz[w] | mnz[w]);
-                        ob |= (((o >> 15) & 1u) | ((o >> 30) & 2u)) << (2 * w);
-                    }
-                    ob &= k == 0 ? 0x55u : k == 1 ? 0x33u : k == 2 ? 0x0Fu : (((v >> (k - 3)) & 1u) ? 0u : 0xFFu);
-                    while (ob) {
-                        const uint32_t l = (v << 3) + (__ffs(ob) - 1);
-                        ob &= ob - 1;
-                        note_pair(a, pf, seg[l], seg[l ^ (1u << k)]);
-                    }
-                }
-            }
-            // flush, merging runs of equal class among the 8 genotypes; other = flips - neutral - deleterious
-            uint32_t run = 0, r_acc = 0, d_acc = 0;
-#pragma unroll
-            for (int j = 0; j < 8; j++) {
-                const uint32_t p = (m[j >> 1] >> (16 * (j & 1))) & 0xFFFFu;
-                if (p == NULLP) continue;
-                run++;
-                r_acc += (rc[j >> 1] >> (16 * (j & 1))) & 0xFFFFu;
-                d_acc += (dc[j >> 1] >> (16 * (j & 1))) & 0xFFFFu;
-                const uint32_t nxt = j < 7 ? (m[(j + 1) >> 1] >> (16 * ((j + 1) & 1))) & 0xFFFFu : NULLP;
-                if (nxt == p) continue;
-                rob_add(a, cache, p, r_acc, d_acc, run * (uint32_t)n_flip - r_acc - d_acc);
-                run = 0; r_acc = 0; d_acc = 0;
-            }
-        }
-        if (++tiles_done % ROB_FLUSH_TILES == 0) rob_flush(a, cache);
-    }
-    rob_flush(a, cache);
-}
+constexpr uint32_t ROB_FLUSH_TILES = 64;  // the class-count cache is written back every so many tiles (u32 counters)
 
 // ---------------------------------------------------------------------------------------------------------------
-// a6, second version of the tile kernel.  Same bit-tiling; the per-flip work is cut to what the counts need:
+// a6, the tile kernel.  The per-flip work is cut to what the counts need:
 //   * "differs" per genotype pair = XOR + one unsigned 16x2 min with 1 (VIMNMX.U16x2): 2 ALU ops per two genotypes,
 //     summed in packed halves (rne); neutral = flips - differs - (null neighbours) for a non-null genotype;
 //   * null neighbours come from a per-tile bitmask (one byte per 8-genotype vector, built while staging): the partner
@@ -483,7 +345,7 @@ __global__ void robustness_tiny_kernel(RobArgs a) {
         const uint32_t q = a.pheno[g ^ (1u << k)];
         if (q == p) r++;
         else if (q == NULLP) d++;
-        else { o++; if (a.bitmap) note_pair(a, nullptr, p, q); }
+        else { o++; if (a.bitmap) note_pair(a, p, q); }
     }
     if (r) atomicAdd(&a.R[p], r);
     if (d) atomicAdd(&a.Dl[p], d);
@@ -530,7 +392,7 @@ __global__ void __launch_bounds__(256) robustness_cross_kernel(RobArgs a, const 
         else if (q == NULLP) atomicAdd(&a.Dl[p], 1ULL);
         else {
             atomicAdd(&a.O[p], 1ULL);
-            if (a.bitmap && q < a.C) note_pair(a, nullptr, p, q);
+            if (a.bitmap && q < a.C) note_pair(a, p, q);
         }
     }
 }
@@ -693,8 +555,6 @@ static gp_status robustness_passes(const uint16_t* d_pheno, int n_bits, uint32_t
                                    int tile_bits, cudaStream_t st) {
     if (!d_pheno || !d_neutral || !d_deleterious || !d_other) return GP_INVALID_ARG;
     if (n_bits < 1 || n_bits > 40 || n_classes == 0 || n_classes >= NULLP) return GP_INVALID_ARG;
-    const bool v1 = (tile_bits & 0x100) != 0;  // previous kernel, kept for A/B timing until the new one is profiled
-    tile_bits &= 0xFF;
     if (tile_bits != 0 && (tile_bits < 4 || tile_bits > ROB2_TB_MAX)) return GP_INVALID_ARG;
     if (((uintptr_t)d_pheno & 15) != 0) return GP_INVALID_ARG;
     RobArgs a;
@@ -716,23 +576,19 @@ static gp_status robustness_passes(const uint16_t* d_pheno, int n_bits, uint32_t
         }
         return GP_OK;
     }
-    const int tb_max = v1 ? ROB_TB_MAX : ROB2_TB_MAX;
-    int tb = tile_bits ? tile_bits : tb_max;
-    if (tb > tb_max) tb = tb_max;
+    int tb = tile_bits ? tile_bits : ROB2_TB_MAX;
     if (tb > n_bits) tb = n_bits;
     const uint64_t n_tiles = 1ULL << (n_bits - tb);
-    const uint64_t cap = (uint64_t)sm_count() * (v1 ? 2 : 1);
+    const uint64_t cap = (uint64_t)sm_count();
     const unsigned grid = (unsigned)(n_tiles < cap ? n_tiles : cap);
-    const size_t smem = v1 ? ((size_t)2 << tb) + ROB_SLOTS * sizeof(RobSlot) + ROB_PF_SLOTS * sizeof(uint32_t)
-                           : ((size_t)2 << tb) + ((((size_t)1 << (tb - 3)) + 15) & ~(size_t)15) + 1024 + ROB2_SLOTS * sizeof(Rob2Slot) +
-                                 ROB2_PF_SLOTS * sizeof(uint32_t) + (R2THREADS / 32) * ROB2_RING * sizeof(uint32_t);
-    if (v1) GP_CUDA(cudaFuncSetAttribute(robustness_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    else if (d_pair_bitmap) GP_CUDA(cudaFuncSetAttribute(robustness2_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const size_t smem = ((size_t)2 << tb) + ((((size_t)1 << (tb - 3)) + 15) & ~(size_t)15) + 1024 + ROB2_SLOTS * sizeof(Rob2Slot) +
+                        ROB2_PF_SLOTS * sizeof(uint32_t) + (R2THREADS / 32) * ROB2_RING * sizeof(uint32_t);
+    if (d_pair_bitmap) GP_CUDA(cudaFuncSetAttribute(robustness2_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     else GP_CUDA(cudaFuncSetAttribute(robustness2_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     a.tb = tb;
     // pass 0: the tb low bits; every later pass flips its own spread bits: segments of 2^c consecutive ids (128 bytes
     // when the tile allows, never under 16), all 2^h values of the spread bits on chip
-    const int seg_bits = v1 ? 7 : 6;
+    const int seg_bits = 6;
     int done = 0;
     bool first = true;
     while (done < n_bits) {
@@ -744,8 +600,7 @@ static gp_status robustness_passes(const uint16_t* d_pheno, int n_bits, uint32_t
             a.h = h; a.c = tb - h; a.hi_pos = done; a.f0 = a.c; done += h;
         }
         gp_time_begin(GP_KERNEL_ROBUSTNESS, st);
-        if (v1) robustness_kernel<<<grid, RTHREADS, smem, st>>>(a);
-        else {
+        {
             Rob2Args b;
             b.pheno = a.pheno; b.n_bits = n_bits; b.C = n_classes; b.R = a.R; b.Dl = a.Dl; b.O = a.O;
             b.hist = first ? reinterpret_cast<unsigned long long*>(d_hist) : nullptr;
@@ -758,7 +613,6 @@ static gp_status robustness_passes(const uint16_t* d_pheno, int n_bits, uint32_t
         gp_count_launches(1);
         first = false;
     }
-    if (v1 && d_hist) return GP_INVALID_ARG;
     return GP_OK;
 }
 

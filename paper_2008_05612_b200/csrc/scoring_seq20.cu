@@ -16,8 +16,9 @@
 namespace tc {
 
 constexpr int Q_KB_MAX = 3;                      // 128-byte column blocks per limb set: 2 + P <= 384 columns
-constexpr int Q_STAGES = 6;                      // 16 KB incidence blocks in flight
-constexpr int Q_THREADS = 32 * (2 + 4);          // warp 0 TMA producer, warp 1 MMA issuer, 4 builder / epilogue warps
+constexpr int Q_STAGES_MAX = 6;                  // structure tiles (kb x 16 KB of incidence blocks each) in flight
+constexpr int Q_PARTS = 4;                       // column parts of a structure tile, one epilogue warp each per lane quarter
+constexpr int Q_THREADS = 32 * (2 + 4 * Q_PARTS); // warp 0 TMA producer, warp 1 MMA issuer, 16 builder / epilogue warps
 constexpr int Q_ROWS = TM;                       // sequences per item
 constexpr int V_PAD = 127;                       // value of the pad structures
 constexpr int V_NONE = 32767;
@@ -33,40 +34,40 @@ struct QArgs {
     int16_t* gap;             // nullable
     uint64_t count, first, seed;
     uint32_t n_items, n_tiles;
-    int N, P, kb, ksteps, alphabet, threshold, src;
+    int N, P, kb, ksteps, alphabet, threshold, src, stages;
     int16_t cost[400];        // emax - M[a][b]
 };
 
 struct __align__(16) QBarriers {
-    uint64_t b_full[Q_STAGES], b_empty[Q_STAGES];
+    uint64_t b_full[Q_STAGES_MAX], b_empty[Q_STAGES_MAX];
     uint64_t acc_full[2], acc_empty[2];
     uint64_t a_full, a_empty;
     uint32_t tmem_base;
 };
 
-// 64 accumulator columns as 32 registers of two int16 (see tmem_ld64_pack16)
-__device__ __forceinline__ void tmem_ld32_pack16(uint32_t taddr, uint32_t (&v)[32]) {
+// 32 accumulator columns as 16 registers of two int16
+__device__ __forceinline__ void tmem_ld16_pack16(uint32_t taddr, uint32_t (&v)[16]) {
     asm volatile(
-        "tcgen05.ld.sync.aligned.32x32b.x32.pack::16b.b32 "
-        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
-        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+        "tcgen05.ld.sync.aligned.32x32b.x16.pack::16b.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
         : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]),
-          "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]), "=r"(v[16]),
-          "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]), "=r"(v[24]),
-          "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+          "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
         : "r"(taddr) : "memory");
 }
 
 // the filtered fold of scoring_tc.cu on 64-bit keys: v spans 16 bits here, so v * 2^17 + column needs more than 32
-__device__ __forceinline__ void fold_half_packed64(const uint32_t* w, uint32_t col0, long long& k1, long long& k2, uint32_t& E2) {
-    uint32_t g[8];
+template <int NG>   // NG groups of 8 columns (4 registers each)
+__device__ __forceinline__ void fold_packed64(const uint32_t* w, uint32_t col0, long long& k1, long long& k2, uint32_t& E2) {
+    uint32_t g[NG];
 #pragma unroll
-    for (int s = 0; s < 8; s++)
+    for (int s = 0; s < NG; s++)
         g[s] = __vimin3_s16x2(w[4 * s], w[4 * s + 1], __vmins2(w[4 * s + 2], w[4 * s + 3]));
-    const uint32_t all = __vimin3_s16x2(__vimin3_s16x2(g[0], g[1], g[2]), __vimin3_s16x2(g[3], g[4], g[5]), __vmins2(g[6], g[7]));
+    uint32_t all = g[0];
+#pragma unroll
+    for (int s = 1; s < NG; s++) all = __vmins2(all, g[s]);
     if (__vmins2(all, E2) != E2) {
 #pragma unroll
-        for (int s = 0; s < 8; s++) {
+        for (int s = 0; s < NG; s++) {
             if (__vmins2(g[s], E2) != E2) {
 #pragma unroll
                 for (int j = 0; j < 4; j++) {
@@ -116,20 +117,22 @@ __global__ void __launch_bounds__(Q_THREADS, 1) seq20_kernel(const QArgs a) {
     extern __shared__ unsigned char smem_dyn[];
     unsigned char* smem = reinterpret_cast<unsigned char*>(((uintptr_t)smem_dyn + 1023) & ~(uintptr_t)1023);
     uint8_t* sA = smem;                                           // [lo | hi][kb][16 KB]
-    uint8_t* sB = sA + 2 * a.kb * TILE_BYTES;                     // Q_STAGES x 16 KB
-    QBarriers* bar = reinterpret_cast<QBarriers*>(sB + Q_STAGES * TILE_BYTES);
+    uint8_t* sB = sA + 2 * a.kb * TILE_BYTES;                     // a.stages x kb x 16 KB
+    QBarriers* bar = reinterpret_cast<QBarriers*>(sB + a.stages * a.kb * TILE_BYTES);
+    const uint32_t Q_STAGES = (uint32_t)a.stages;
     uint8_t* let = reinterpret_cast<uint8_t*>(bar + 1);           // [N][128] letters of the item's sequences
     uint8_t* pij = let + a.N * Q_ROWS;                            // [P][2]
     int16_t* cost = reinterpret_cast<int16_t*>(pij + ((2 * a.P + 15) & ~15));
+    long long* merge = reinterpret_cast<long long*>(cost + 400);  // [Q_PARTS][128][2] partial (k1, k2) per item
     constexpr uint32_t IDESC = idesc_for(TN);
 
     const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     for (int i = threadIdx.x; i < 2 * a.P; i += Q_THREADS) pij[i] = a.pair_ij[i];
     for (int i = threadIdx.x; i < a.alphabet * a.alphabet; i += Q_THREADS) cost[i] = a.cost[i];
     if (threadIdx.x == 0) {
-        for (int s = 0; s < Q_STAGES; s++) { mbar_init(&bar->b_full[s], 1); mbar_init(&bar->b_empty[s], 1); }
-        for (int b = 0; b < 2; b++) { mbar_init(&bar->acc_full[b], 1); mbar_init(&bar->acc_empty[b], 4); }
-        mbar_init(&bar->a_full, Q_ROWS);
+        for (uint32_t s = 0; s < Q_STAGES; s++) { mbar_init(&bar->b_full[s], 1); mbar_init(&bar->b_empty[s], 1); }
+        for (int b = 0; b < 2; b++) { mbar_init(&bar->acc_full[b], 1); mbar_init(&bar->acc_empty[b], 4 * Q_PARTS); }
+        mbar_init(&bar->a_full, Q_ROWS * Q_PARTS);
         mbar_init(&bar->a_empty, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -143,25 +146,25 @@ __global__ void __launch_bounds__(Q_THREADS, 1) seq20_kernel(const QArgs a) {
     const uint32_t tmem = bar->tmem_base;
 
     if (warp == 0) {
-        // ===== producer: the kb incidence blocks of every structure tile, once per item =====
+        // ===== producer: one bulk copy per structure tile (its kb incidence blocks are contiguous), once per item =====
+        const uint32_t stage_bytes = (uint32_t)a.kb * TILE_BYTES;
         uint32_t it = 0;
         for (uint32_t item = blockIdx.x; item < a.n_items; item += gridDim.x)
-            for (uint32_t n = 0; n < a.n_tiles; n++)
-                for (int b = 0; b < a.kb; b++, it++) {
-                    const uint32_t s = it % Q_STAGES, ph = (it / Q_STAGES) & 1;
-                    mbar_wait(&bar->b_empty[s], ph ^ 1);
-                    if (elect_one()) {
-                        mbar_expect_tx(&bar->b_full[s], TILE_BYTES);
-                        bulk_g2s(sB + s * TILE_BYTES, a.img + ((uint64_t)n * a.kb + b) * TILE_BYTES, TILE_BYTES, &bar->b_full[s]);
-                    }
-                    __syncwarp();
+            for (uint32_t n = 0; n < a.n_tiles; n++, it++) {
+                const uint32_t s = it % Q_STAGES, ph = (it / Q_STAGES) & 1;
+                mbar_wait(&bar->b_empty[s], ph ^ 1);
+                if (elect_one()) {
+                    mbar_expect_tx(&bar->b_full[s], stage_bytes);
+                    bulk_g2s(sB + s * stage_bytes, a.img + (uint64_t)n * stage_bytes, stage_bytes, &bar->b_full[s]);
                 }
+                __syncwarp();
+            }
     } else if (warp == 1) {
         // ===== MMA issuer: two chains (lo, hi limbs) per structure tile share every incidence block; accumulator pairs
         // double-buffered =====
         const uint64_t a_lo0 = smem_desc(smem_u32(sA)), a_hi0 = smem_desc(smem_u32(sA + a.kb * TILE_BYTES));
         const uint64_t b_desc0 = smem_desc(smem_u32(sB));
-        uint32_t it = 0, tile_no = 0, item_no = 0;
+        uint32_t tile_no = 0, item_no = 0;
         for (uint32_t item = blockIdx.x; item < a.n_items; item += gridDim.x, item_no++) {
             mbar_wait(&bar->a_full, item_no & 1);
             tc_fence_after();
@@ -170,50 +173,53 @@ __global__ void __launch_bounds__(Q_THREADS, 1) seq20_kernel(const QArgs a) {
                 mbar_wait(&bar->acc_empty[buf], ((tile_no >> 1) & 1) ^ 1);
                 tc_fence_after();
                 const uint32_t d_lo = tmem + (2 * buf) * TN, d_hi = d_lo + TN;
-                for (int b = 0; b < a.kb; b++, it++) {
-                    const uint32_t s = it % Q_STAGES, ph = (it / Q_STAGES) & 1;
-                    mbar_wait(&bar->b_full[s], ph);
-                    tc_fence_after();
-                    if (elect_one()) {
-                        const uint64_t bd = b_desc0 + (uint64_t)(s * (TILE_BYTES >> 4));
+                const uint32_t s = tile_no % Q_STAGES, ph = (tile_no / Q_STAGES) & 1;
+                mbar_wait(&bar->b_full[s], ph);
+                tc_fence_after();
+                if (elect_one()) {
+                    const uint64_t bd0 = b_desc0 + (uint64_t)s * (uint64_t)((a.kb * TILE_BYTES) >> 4);
+                    for (int b = 0; b < a.kb; b++) {
                         const uint64_t blk = (uint64_t)((b * TILE_BYTES) >> 4);
                         const int nks = a.ksteps - 4 * b < 4 ? a.ksteps - 4 * b : 4;
                         for (int ks = 0; ks < nks; ks++) {
                             const uint32_t acc = (b | ks) != 0;
-                            mma_i8(d_lo, a_lo0 + blk + 2 * ks, bd + 2 * ks, IDESC, acc);
-                            mma_i8(d_hi, a_hi0 + blk + 2 * ks, bd + 2 * ks, IDESC, acc);
+                            mma_i8(d_lo, a_lo0 + blk + 2 * ks, bd0 + blk + 2 * ks, IDESC, acc);
+                            mma_i8(d_hi, a_hi0 + blk + 2 * ks, bd0 + blk + 2 * ks, IDESC, acc);
                         }
-                        tc_commit(&bar->b_empty[s]);
-                        if (b == a.kb - 1) tc_commit(&bar->acc_full[buf]);
                     }
-                    __syncwarp();
+                    tc_commit(&bar->b_empty[s]);
+                    tc_commit(&bar->acc_full[buf]);
                 }
+                __syncwarp();
             }
             if (elect_one()) tc_commit(&bar->a_empty);
             __syncwarp();
         }
     } else {
-        // ===== limb rows + epilogue: thread = sequence =====
-        const uint32_t quarter = warp & 3;
+        // ===== limb rows + epilogue: 16 warps.  Warp = (TMEM lane quarter, column part): the four warps of a quarter share
+        // the 32 sequences of that quarter and split the 128 columns of every structure tile (one warp per SM
+        // sub-partition cannot hide its own latencies: profiles/r2_seq20_ncu.md); their (k1, k2) are merged per item. =====
+        const uint32_t quarter = warp & 3, part = (warp - 2) >> 2;
         const uint32_t r = quarter * 32 + lane;
-        const uint32_t t_lane = tmem + ((quarter * 32u) << 16);
+        const uint32_t t_lane = tmem + ((quarter * 32u) << 16) + part * 32u;
         uint8_t* my_let = let + r;
         uint32_t tile_no = 0, item_no = 0;
         for (uint32_t item = blockIdx.x; item < a.n_items; item += gridDim.x, item_no++) {
             const uint64_t q = (uint64_t)item * Q_ROWS + r;
-            for (int i = 0; i < a.N; i++) {
+            for (int i = 0; i < a.N; i++) {   // the row's four threads each need all letters: every one writes the same bytes
                 uint32_t l = 0;
                 if (q < a.count) l = SRC == QSRC_SEQS ? a.seqs[q * a.N + i] : gp_letter20(a.seed, a.first + q, i);
                 my_let[i * Q_ROWS] = (uint8_t)min(l, (uint32_t)a.alphabet - 1u);  // a letter outside the alphabet counts as the last one
             }
             mbar_wait(&bar->a_empty, (item_no & 1) ^ 1);
-            for (int b = 0; b < 2 * a.kb; b++)
+            for (int b = part; b < 2 * a.kb; b += Q_PARTS)
 #pragma unroll
                 for (int c16 = 0; c16 < 8; c16++)
                     *reinterpret_cast<uint4*>(sA + b * TILE_BYTES + r * ROWB + c16 * 16) = make_uint4(0, 0, 0, 0);
-            sA[swz(r, 0)] = 1;                                       // constant column (lo limb set only)
+            asm volatile("bar.sync %0, 128;" ::"r"(quarter + 1) : "memory");   // the row is zeroed before its bytes are set
+            if (part == 0) sA[swz(r, 0)] = 1;                        // constant column (lo limb set only)
             uint8_t* sHi = sA + a.kb * TILE_BYTES;
-            for (int p = 0; p < a.P; p++) {
+            for (int p = part; p < a.P; p += Q_PARTS) {
                 const uint32_t c = (uint32_t)cost[my_let[pij[2 * p] * Q_ROWS] * a.alphabet + my_let[pij[2 * p + 1] * Q_ROWS]];
                 const uint32_t col = 2u + p, off = (col >> 7) * TILE_BYTES + swz(r, col & 127u);
                 sA[off] = (uint8_t)(c & 63u);
@@ -229,30 +235,38 @@ __global__ void __launch_bounds__(Q_THREADS, 1) seq20_kernel(const QArgs a) {
                 const uint32_t buf = tile_no & 1;
                 mbar_wait(&bar->acc_full[buf], (tile_no >> 1) & 1);
                 tc_fence_after();
-#pragma unroll 1
-                for (uint32_t h = 0; h < 2; h++) {
-                    uint32_t wl[32], wh[32];
-                    tmem_ld32_pack16(t_lane + (2 * buf) * TN + h * HN, wl);
-                    tmem_ld32_pack16(t_lane + (2 * buf + 1) * TN + h * HN, wh);
-                    tmem_ld_wait();
-                    if (h == 1) {  // both accumulators are in registers: hand the pair back to the MMA warp
-                        tc_fence_before();
-                        __syncwarp();
-                        if (lane == 0) mbar_arrive(&bar->acc_empty[buf]);
-                    }
+                uint32_t wl[16], wh[16];
+                tmem_ld16_pack16(t_lane + (2 * buf) * TN, wl);
+                tmem_ld16_pack16(t_lane + (2 * buf + 1) * TN, wh);
+                tmem_ld_wait();
+                tc_fence_before();       // this warp's share of both accumulators is in registers
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&bar->acc_empty[buf]);
 #pragma unroll
-                    for (int i = 0; i < 32; i++) wl[i] = __vadd2(wl[i], (wh[i] << 6) & 0xFFC0FFC0u);  // v = -(lo + 64 hi), per int16
-                    fold_half_packed64(wl, n * TN + h * HN, k1, k2, E2);
+                for (int i = 0; i < 16; i++) wl[i] = __vadd2(wl[i], (wh[i] << 6) & 0xFFC0FFC0u);  // v = -(lo + 64 hi), per int16
+                fold_packed64<4>(wl, n * TN + part * 32u, k1, k2, E2);
+            }
+            // merge the four column parts of every sequence: the two smallest of eight distinct keys
+            merge[(part * Q_ROWS + r) * 2] = k1;
+            merge[(part * Q_ROWS + r) * 2 + 1] = k2;
+            asm volatile("bar.sync %0, 128;" ::"r"(quarter + 1) : "memory");
+            if (part == 0) {
+#pragma unroll
+                for (int o = 1; o < Q_PARTS; o++) {
+                    const long long x1 = merge[(o * Q_ROWS + r) * 2], x2 = merge[(o * Q_ROWS + r) * 2 + 1];
+                    k2 = min(min(k2, x2), max(k1, x1));
+                    k1 = min(k1, x1);
+                }
+                if (q < a.count) {
+                    const long long e1 = k1 >> KEY_SHIFT, e2 = k2 >> KEY_SHIFT;
+                    const uint32_t col = (uint32_t)(k1 & ((1LL << KEY_SHIFT) - 1));
+                    const bool single = e2 >= V_PAD;   // D = 1: the runner-up is a pad structure
+                    const bool folds = single || (e2 - e1 >= a.threshold);
+                    a.pheno[q] = folds ? a.class_of[col] : (uint16_t)GP_NULL_PHENO;
+                    if (a.gap) a.gap[q] = (int16_t)(single ? GP_GAP_NONE : (e1 - e2 < -32768 ? -32768 : e1 - e2));
                 }
             }
-            if (q < a.count) {
-                const long long e1 = k1 >> KEY_SHIFT, e2 = k2 >> KEY_SHIFT;
-                const uint32_t col = (uint32_t)(k1 & ((1LL << KEY_SHIFT) - 1));
-                const bool single = e2 >= V_PAD;   // D = 1: the runner-up is a pad structure
-                const bool folds = single || (e2 - e1 >= a.threshold);
-                a.pheno[q] = folds ? a.class_of[col] : (uint16_t)GP_NULL_PHENO;
-                if (a.gap) a.gap[q] = (int16_t)(single ? GP_GAP_NONE : (e1 - e2 < -32768 ? -32768 : e1 - e2));
-            }
+            asm volatile("bar.sync %0, 128;" ::"r"(quarter + 1) : "memory");   // merge[] is free again
         }
     }
     tc_fence_before();
@@ -305,8 +319,15 @@ gp_status gp_launch_seq20_tc(const gp_structures_s* s, const gp_energies* en, in
     int dev = 0, sms = 0;
     GP_CUDA(cudaGetDevice(&dev));
     GP_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    const size_t smem = (size_t)(2 * kb + Q_STAGES) * TILE_BYTES + sizeof(QBarriers) + (size_t)s->N * Q_ROWS +
-                        ((2 * (size_t)s->P + 15) & ~(size_t)15) + 800 + 1024 + 64;
+    const size_t aux = sizeof(QBarriers) + (size_t)s->N * Q_ROWS + ((2 * (size_t)s->P + 15) & ~(size_t)15) + 800 +
+                       (size_t)Q_PARTS * Q_ROWS * 16 + 1024 + 64;
+    // a stage holds the kb incidence blocks of one structure tile, fetched by ONE bulk copy (16 KB copies were measured
+    // to deliver a block per 940 clocks and SM, whatever the ring depth: profiles/r2_seq20_ncu.md)
+    int stages = (int)(((227 * 1024 - aux) / TILE_BYTES - 2 * kb) / kb);
+    if (stages > Q_STAGES_MAX) stages = Q_STAGES_MAX;
+    if (stages < 2) return GP_UNSUPPORTED_LATTICE;
+    a.stages = stages;
+    const size_t smem = (size_t)(2 * kb + stages * kb) * TILE_BYTES + aux;
     void (*k)(const QArgs) = seeded ? seq20_kernel<QSRC_SEEDED> : seq20_kernel<QSRC_SEQS>;
     GP_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const unsigned grid = a.n_items < (uint32_t)sms ? a.n_items : (uint32_t)sms;
