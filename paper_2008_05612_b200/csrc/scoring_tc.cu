@@ -134,17 +134,20 @@ __global__ void __launch_bounds__(THREADS, 1) scoring_kernel(const Args a, const
     constexpr uint32_t IDESC = idesc_for(TN);
 
     const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    // the service warps have the highest warp ids: the sub-partition arbiter favours high ids, and their few instructions
+    // per tile are the critical path
+    constexpr uint32_t W_ISS = EPI_WARPS, W_PROD = EPI_WARPS + NISS;
 
     for (uint32_t c = threadIdx.x; c < ROWB; c += THREADS)
         pk[c] = cols_in.val[c] ? ((1u << cols_in.i[c]) | (1u << cols_in.j[c])) : 0xFFFFFFFFu;  // unused column: never all set
     if (threadIdx.x == 0) {
-        for (int s = 0; s < NSTAGE; s++) { mbar_init(&bar->b_full[s], 1); mbar_init(&bar->b_empty[s], 1); }
+        for (int s = 0; s < NSTAGE; s++) { mbar_init(&bar->b_full[s], 1); mbar_init(&bar->b_empty[s], NISS); }
         for (int m = 0; m < MT; m++) { mbar_init(&bar->acc_full[m], 1); mbar_init(&bar->acc_empty[m], 4); }
         mbar_init(&bar->a_full, 32 * EPI_WARPS);
-        mbar_init(&bar->a_empty, 1);
+        mbar_init(&bar->a_empty, NISS);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    if (warp == 1) {  // TMEM: all 512 columns (one CTA per SM)
+    if (warp == W_ISS) {  // TMEM: all 512 columns (one CTA per SM)
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(&bar->tmem_base)) : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
@@ -153,7 +156,7 @@ __global__ void __launch_bounds__(THREADS, 1) scoring_kernel(const Args a, const
     tc_fence_after();
     const uint32_t tmem = bar->tmem_base;
 
-    if (warp == 0) {
+    if (warp == W_PROD) {
         // ===== producer: stream every weight tile of the item's batch image through the ring.  The whole warp runs the
         // loop (uniform control flow); one elected lane issues the copies. =====
         uint32_t it = 0;
@@ -171,8 +174,12 @@ __global__ void __launch_bounds__(THREADS, 1) scoring_kernel(const Args a, const
                 __syncwarp();
             }
         }
-    } else if (warp == 1) {
-        // ===== MMA issuer: warp-uniform loop, one elected lane issues =====
+    } else if (warp >= W_ISS) {
+        // ===== MMA issuers: NISS warps, issuer h owns accumulators h*MT/NISS ..; warp-uniform loop, one elected lane issues.
+        // One issuer's own instruction latencies (wait, fence, elect, two MMAs, commit: 170 clocks per chain and 290 per
+        // tile, clock64 trace in profiles/r2_scoring_ncu.md) were longer than the 528 clocks of tensor work per tile. =====
+        constexpr int MPI = MT / NISS;                  // accumulators per issuer
+        const uint32_t m0 = (warp - W_ISS) * MPI;
         const uint64_t a_desc0 = smem_desc_rb<RB>(smem_u32(sA));
         const uint64_t b_desc0 = smem_desc_rb<RB>(smem_u32(sB));
         uint32_t it = 0, item_no = 0;
@@ -185,7 +192,8 @@ __global__ void __launch_bounds__(THREADS, 1) scoring_kernel(const Args a, const
                 tc_fence_after();
                 const uint64_t bd = b_desc0 + (uint64_t)(s * (TB >> 4));
 #pragma unroll
-                for (int m = 0; m < MT; m++) {
+                for (int j = 0; j < MPI; j++) {
+                    const uint32_t m = m0 + j;
                     mbar_wait(&bar->acc_empty[m], (it & 1) ^ 1);
                     tc_fence_after();
                     if (elect_one()) {
@@ -206,7 +214,7 @@ __global__ void __launch_bounds__(THREADS, 1) scoring_kernel(const Args a, const
         }
     } else {
         // ===== feature build + epilogue: 16 warps; warp group m owns A tile m and accumulator m; thread = genotype row =====
-        const uint32_t m = (warp - 2) >> 2;             // accumulator / A tile of this warp group
+        const uint32_t m = warp >> 2;                   // accumulator / A tile of this warp group
         const uint32_t quarter = warp & 3;              // TMEM lanes 32*quarter .. +31 are the ones this warp may read
         const uint32_t r = quarter * 32 + lane;         // row within the 128-row tile
         const uint32_t t_acc = tmem + ((quarter * 32u) << 16) + m * TN;
@@ -250,7 +258,7 @@ __global__ void __launch_bounds__(THREADS, 1) scoring_kernel(const Args a, const
     }
     tc_fence_before();
     __syncthreads();
-    if (warp == 1) {
+    if (warp == W_ISS) {
         tc_fence_after();
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem) : "memory");
     }

@@ -12,8 +12,9 @@ constexpr int ROWB = 128;             // bytes per operand row = one 128-byte sw
 constexpr int TILE_BYTES = TM * ROWB; // 16 KB, A tile and B stage alike
 constexpr int NSTAGE = 6;
 constexpr int SUPER = MT * TM;        // 512 genotypes
-constexpr int EPI_WARPS = 4 * MT;     // warp group m = warps 2+4m .. 5+4m drains accumulator m
-constexpr int THREADS = 32 * (2 + EPI_WARPS);  // warp 0 TMA producer, warp 1 MMA issuer, then feature build + epilogue
+constexpr int NISS = 2;                // MMA issuer warps of scoring_kernel (each owns MT / NISS accumulators)
+constexpr int EPI_WARPS = 4 * MT;     // warp group m = warps 1+NISS+4m .. drains accumulator m
+constexpr int THREADS = 32 * (1 + NISS + EPI_WARPS);  // warp 0 TMA producer, warps 1..NISS MMA issuers, then feature build + epilogue
 constexpr int MAX_FB = 22;            // 2 + 22 + 100 pairs = 124 <= 128 columns
 constexpr int KEY_SHIFT = 17;         // key = E * 2^17 + column (D < 2^17, |E| < 2^13)
 constexpr int E_NONE = 16383;         // INT32_MAX >> KEY_SHIFT: "no energy yet"
