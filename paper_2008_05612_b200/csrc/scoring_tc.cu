@@ -301,48 +301,65 @@ __device__ __forceinline__ uint32_t image_mid(const uint32_t* units, uint64_t un
     return (paired && (y & 1u)) ? (mid ? (__brev(m) >> (32 - mid)) : 0u) : m;
 }
 
-// One block = one 128-structure tile of one image.  Thread = structure: it accumulates its 128-byte weight row in
-// shared memory (already in the swizzled layout the MMA reads), then the block writes the 16 KB tile out coalesced.
+// One block = one 128-structure tile of IMG_PER_BLOCK consecutive images.  The tile's contact lists and the column
+// tables are staged in shared memory once (the tables are indexed by monomer, different in every thread: as kernel
+// parameters they would be serialised constant-bank reads).  Thread = structure: it accumulates its weight row in shared
+// memory (already in the swizzled layout the MMA reads), then the block writes the tile out coalesced.
+constexpr int IMG_PER_BLOCK = 4;
+
 template <int RB>
-__global__ void __launch_bounds__(TN) build_image_kernel(const ImgArgs a, const Slots slots) {
+__global__ void __launch_bounds__(TN) build_image_kernel(const ImgArgs a, const Slots slots_in, uint32_t n_images) {
     constexpr int TB = TM * RB;
     __shared__ __align__(16) int8_t tile[TB];
+    __shared__ __align__(16) uint8_t s_con[TN * 64];   // contacts of the tile's structures: NBP <= 32 pairs each
+    __shared__ Slots slots;
     const uint32_t r = threadIdx.x, n = blockIdx.x;
-    const uint64_t G = (a.units ? (uint64_t)image_mid(a.units, a.unit_first, a.paired, a.mid, blockIdx.y) : a.gfix_first + blockIdx.y)
-                       << a.gfix_shift;
-    for (uint32_t i = threadIdx.x; i < TB / 16; i += TN) reinterpret_cast<uint4*>(tile)[i] = make_uint4(0, 0, 0, 0);
-    __syncthreads();
     const uint32_t d = n * TN + r;
-    if (d < a.D && a.class_of[d] != GP_NULL_PHENO) {
-        const uint8_t* c = a.contacts + (size_t)d * a.NBP * 2;
-        int bias = 0;
-        for (int k = 0; k < a.NBP; k++) {
-            const int i = c[2 * k], j = c[2 * k + 1];  // i < j
-            const int li = slots.loc[i], lj = slots.loc[j];
-            const int hi = (int)((G >> i) & 1ULL), hj = (int)((G >> j) & 1ULL);
-            if (li >= 0 && lj >= 0) {
-                tile[swz_rb<RB>(r, 2 + li)] += (int8_t)a.lin;
-                tile[swz_rb<RB>(r, 2 + lj)] += (int8_t)a.lin;
-                tile[swz_rb<RB>(r, slots.pair[li * MAX_FB + lj])] = (int8_t)a.quad;
-            } else if (li >= 0) {
-                tile[swz_rb<RB>(r, 2 + li)] += (int8_t)(a.lin + a.quad * hj);
-                bias += a.lin * hj;
-            } else if (lj >= 0) {
-                tile[swz_rb<RB>(r, 2 + lj)] += (int8_t)(a.lin + a.quad * hi);
-                bias += a.lin * hi;
-            } else {
-                bias += a.lin * (hi + hj) + a.quad * hi * hj;
-            }
-        }
-        tile[swz_rb<RB>(r, 0)] = (int8_t)(bias >> 6);   // x 64
-        tile[swz_rb<RB>(r, 1)] = (int8_t)(bias & 63);   // x 1
-    } else {                                     // pad structure: energy E_PAD for every genotype
-        tile[swz_rb<RB>(r, 0)] = 127;
-        tile[swz_rb<RB>(r, 1)] = 63;
+    const int row = a.NBP * 2;
+    {
+        const uint32_t first = n * TN, cnt = (a.D - first < (uint32_t)TN ? a.D - first : (uint32_t)TN) * row;
+        const uint8_t* src = a.contacts + (size_t)first * row;
+        for (uint32_t i = threadIdx.x; i < cnt; i += TN) s_con[i] = src[i];
+        for (uint32_t i = threadIdx.x; i < sizeof(Slots); i += TN)
+            reinterpret_cast<uint8_t*>(&slots)[i] = reinterpret_cast<const uint8_t*>(&slots_in)[i];
     }
-    __syncthreads();
-    uint4* dst = reinterpret_cast<uint4*>(a.img + ((uint64_t)blockIdx.y * a.n_tiles + n) * TB);
-    for (uint32_t i = threadIdx.x; i < TB / 16; i += TN) dst[i] = reinterpret_cast<const uint4*>(tile)[i];
+    const bool real = d < a.D && a.class_of[d] != GP_NULL_PHENO;
+    const uint8_t* c = s_con + r * row;
+    for (uint32_t y = blockIdx.y * IMG_PER_BLOCK; y < n_images && y < (blockIdx.y + 1) * IMG_PER_BLOCK; y++) {
+        const uint64_t G = (a.units ? (uint64_t)image_mid(a.units, a.unit_first, a.paired, a.mid, y) : a.gfix_first + y) << a.gfix_shift;
+        __syncthreads();   // staging done / previous tile written out
+        for (uint32_t i = threadIdx.x; i < TB / 16; i += TN) reinterpret_cast<uint4*>(tile)[i] = make_uint4(0, 0, 0, 0);
+        __syncthreads();
+        if (real) {
+            int bias = 0;
+            for (int k = 0; k < a.NBP; k++) {
+                const int i = c[2 * k], j = c[2 * k + 1];  // i < j
+                const int li = slots.loc[i], lj = slots.loc[j];
+                const int hi = (int)((G >> i) & 1ULL), hj = (int)((G >> j) & 1ULL);
+                if (li >= 0 && lj >= 0) {
+                    tile[swz_rb<RB>(r, 2 + li)] += (int8_t)a.lin;
+                    tile[swz_rb<RB>(r, 2 + lj)] += (int8_t)a.lin;
+                    tile[swz_rb<RB>(r, slots.pair[li * MAX_FB + lj])] = (int8_t)a.quad;
+                } else if (li >= 0) {
+                    tile[swz_rb<RB>(r, 2 + li)] += (int8_t)(a.lin + a.quad * hj);
+                    bias += a.lin * hj;
+                } else if (lj >= 0) {
+                    tile[swz_rb<RB>(r, 2 + lj)] += (int8_t)(a.lin + a.quad * hi);
+                    bias += a.lin * hi;
+                } else {
+                    bias += a.lin * (hi + hj) + a.quad * hi * hj;
+                }
+            }
+            tile[swz_rb<RB>(r, 0)] = (int8_t)(bias >> 6);   // x 64
+            tile[swz_rb<RB>(r, 1)] = (int8_t)(bias & 63);   // x 1
+        } else {                                     // pad structure: energy E_PAD for every genotype
+            tile[swz_rb<RB>(r, 0)] = 127;
+            tile[swz_rb<RB>(r, 1)] = 63;
+        }
+        __syncthreads();
+        uint4* dst = reinterpret_cast<uint4*>(a.img + ((uint64_t)y * a.n_tiles + n) * TB);
+        for (uint32_t i = threadIdx.x; i < TB / 16; i += TN) dst[i] = reinterpret_cast<const uint4*>(tile)[i];
+    }
 }
 
 // Columns of the folded contraction for a set of free monomers mon[0..fb-1] (increasing): 2 bias columns, fb monomer
@@ -729,7 +746,7 @@ struct Plan {
 gp_status make_plan(const gp_structures_s* s, const int* mon, int fb, uint32_t n_columns, Plan& p) {
     using namespace tc;
     p.nc = make_columns(mon, fb, s->N, p.cols, p.slots);
-    if (p.nc > ROWB) return GP_UNSUPPORTED_LATTICE;
+    if (p.nc > ROWB || s->NBP > 32) return GP_UNSUPPORTED_LATTICE;  // build_image_kernel stages 32 contacts per structure
     p.k_steps = (p.nc + 31) / 32;
     p.n_tiles = (n_columns + TN - 1) / TN;
     p.narrow = p.nc <= 64 && s->tuning.narrow_rows;  // at most 64 columns: 64-byte operand rows
@@ -780,8 +797,8 @@ gp_status gp_launch_scoring_tc(const gp_structures_s* s, const gp_hp_params& hp,
         ia.gfix_first = b0; ia.unit_first = 0; ia.paired = 0; ia.mid = 0; ia.gfix_shift = fb; ia.D = s->D; ia.n_tiles = p.n_tiles;
         ia.NBP = s->NBP; ia.lin = hp.lin; ia.quad = hp.quad;
         gp_time_begin(GP_KERNEL_IMAGE, st);
-        if (p.narrow) build_image_kernel<64><<<dim3(p.n_tiles, n_batches), TN, 0, st>>>(ia, p.slots);
-        else build_image_kernel<128><<<dim3(p.n_tiles, n_batches), TN, 0, st>>>(ia, p.slots);
+        if (p.narrow) build_image_kernel<64><<<dim3(p.n_tiles, (n_batches + IMG_PER_BLOCK - 1) / IMG_PER_BLOCK), TN, 0, st>>>(ia, p.slots, n_batches);
+        else build_image_kernel<128><<<dim3(p.n_tiles, (n_batches + IMG_PER_BLOCK - 1) / IMG_PER_BLOCK), TN, 0, st>>>(ia, p.slots, n_batches);
         gp_time_end(GP_KERNEL_IMAGE, st);
         Args a;
         a.img = d_img; a.class_of = s->d_class_of; a.pheno = d_pheno; a.gap = d_gap;
@@ -891,8 +908,8 @@ static gp_status gp_launch_map_range(const gp_structures_s* s, const gp_hp_param
         ia.gfix_first = 0; ia.unit_first = u; ia.paired = paired; ia.mid = mid; ia.gfix_shift = k; ia.D = s->D_sym;
         ia.n_tiles = p.n_tiles; ia.NBP = s->NBP; ia.lin = hp.lin; ia.quad = hp.quad;
         gp_time_begin(GP_KERNEL_IMAGE, st);
-        if (p.narrow) build_image_kernel<64><<<dim3(p.n_tiles, n_img), TN, 0, st>>>(ia, p.slots);
-        else build_image_kernel<128><<<dim3(p.n_tiles, n_img), TN, 0, st>>>(ia, p.slots);
+        if (p.narrow) build_image_kernel<64><<<dim3(p.n_tiles, (n_img + IMG_PER_BLOCK - 1) / IMG_PER_BLOCK), TN, 0, st>>>(ia, p.slots, n_img);
+        else build_image_kernel<128><<<dim3(p.n_tiles, (n_img + IMG_PER_BLOCK - 1) / IMG_PER_BLOCK), TN, 0, st>>>(ia, p.slots, n_img);
         gp_time_end(GP_KERNEL_IMAGE, st);
         Args a;
         a.img = d_img; a.class_of = s->d_class_sym; a.pheno = nullptr; a.gap = nullptr;
