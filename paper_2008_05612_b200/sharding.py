@@ -90,9 +90,9 @@ class DistComm:
         """Swap `chunk` entries at `offset` of the shard with the partner rank; returns the partner's entries."""
         send = mine[offset:offset + chunk]
         recv = torch.empty_like(send)
-        # uint16 has no collective support everywhere: ship the bits as int16
-        ops = [dist.P2POp(dist.isend, send.view(torch.int16), partner_rank, self.group),
-               dist.P2POp(dist.irecv, recv.view(torch.int16), partner_rank, self.group)]
+        # 16-bit integers are not an NCCL data type: ship the bytes
+        ops = [dist.P2POp(dist.isend, send.view(torch.uint8), partner_rank, self.group),
+               dist.P2POp(dist.irecv, recv.view(torch.uint8), partner_rank, self.group)]
         for req in dist.batch_isend_irecv(ops):
             req.wait()
         self.bytes_sent += send.numel() * send.element_size()
