@@ -50,6 +50,8 @@ def parse():
     ap.add_argument("--no-whole-map", action="store_true", help="skip the whole-3x3x3-map leg")
     ap.add_argument("--no-full-map", action="store_true", help="skip the live full 2^36 6x6 enumeration leg (about 2 minutes)")
     ap.add_argument("--fold-bits", type=int, default=0, help="gp_tuning.fold_bits: low genotype bits kept as MMA columns")
+    ap.add_argument("--force-sharded", action="store_true", help="take the sharded multi-rank step (sharding.py over "
+                    "torch.distributed) even with one rank: exercises that code path on a single GPU")
     ap.add_argument("--rows", action="store_true", help="time every row of the hot path on its BASELINE.json config instead")
     ap.add_argument("--out", default="", help="--rows: also write the rows to this JSON file")
     return ap.parse_args()
@@ -480,7 +482,9 @@ def run_ours(args):
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device — the product path has no CPU fallback")
     torch.cuda.set_device(local)
-    if world > 1:
+    if world > 1 or args.force_sharded:
+        if "MASTER_ADDR" not in os.environ:
+            os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT="29531", RANK="0", WORLD_SIZE="1")
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     gpmap.lib()  # fails loudly if libgpmap.so is missing / unbuildable
     if args.rows:
@@ -507,7 +511,7 @@ def run_ours(args):
     # N > 1: the step is ONE sub-cube of 2^(G+q) genotypes sharded over the ranks on its top q bits:
     # rank-local scoring, rank-local neighbour pass, hypercube exchange of the shards for the q rank-selecting bits,
     # all_reduce of the counts, OR-reduce of the pair bitmap.  Per-rank work is fixed: weak scaling.
-    sharded = world > 1 and (world & (world - 1)) == 0 and G + world.bit_length() - 1 <= N and not args.full
+    sharded = (world > 1 or args.force_sharded) and (world & (world - 1)) == 0 and G + world.bit_length() - 1 <= N and not args.full
     if sharded:
         from paper_2008_05612_b200 import sharding
         ops, comm, q = sharding.LibOps(), sharding.DistComm(), world.bit_length() - 1
@@ -685,7 +689,7 @@ def run_ours(args):
             "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline, "other_kernels": other,
             "whole_map_3x3x3": whole, "full_6x6": full, "cpu_baseline": cpu}
     print(json.dumps(line), flush=True)
-    if world > 1:
+    if dist.is_initialized():
         dist.destroy_process_group()
 
 
