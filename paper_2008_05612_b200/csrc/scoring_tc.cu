@@ -764,6 +764,33 @@ gp_status make_plan(const gp_structures_s* s, const int* mon, int fb, uint32_t n
 
 }  // namespace
 
+// Weight images of launch group g + 1 are built on a side stream while the scoring kernel of group g runs on the caller's
+// stream (two image buffers); events tie the side stream in, so that to the caller everything is ordered on `st`.
+struct ImagePipeline {
+    cudaStream_t side = nullptr;
+    cudaEvent_t built[2] = {nullptr, nullptr}, freed[2] = {nullptr, nullptr}, start = nullptr;
+    gp_status open(cudaStream_t st) {   // call after the buffers were allocated on st
+        GP_CUDA(cudaStreamCreateWithFlags(&side, cudaStreamNonBlocking));
+        GP_CUDA(cudaEventCreateWithFlags(&start, cudaEventDisableTiming));
+        for (int b = 0; b < 2; b++) {
+            GP_CUDA(cudaEventCreateWithFlags(&built[b], cudaEventDisableTiming));
+            GP_CUDA(cudaEventCreateWithFlags(&freed[b], cudaEventDisableTiming));
+        }
+        GP_CUDA(cudaEventRecord(start, st));
+        GP_CUDA(cudaStreamWaitEvent(side, start, 0));
+        return GP_OK;
+    }
+    // side stream may overwrite buffer b once the scoring launch that read it (two groups ago) is done
+    void before_build(uint64_t g) { if (g >= 2) cudaStreamWaitEvent(side, freed[g & 1], 0); }
+    void after_build(uint64_t g, cudaStream_t st) { cudaEventRecord(built[g & 1], side); cudaStreamWaitEvent(st, built[g & 1], 0); }
+    void after_scoring(uint64_t g, cudaStream_t st) { cudaEventRecord(freed[g & 1], st); }
+    ~ImagePipeline() {   // destroying a stream / event with work pending is deferred by the runtime
+        for (int b = 0; b < 2; b++) { if (built[b]) cudaEventDestroy(built[b]); if (freed[b]) cudaEventDestroy(freed[b]); }
+        if (start) cudaEventDestroy(start);
+        if (side) cudaStreamDestroy(side);
+    }
+};
+
 gp_status gp_launch_scoring_tc(const gp_structures_s* s, const gp_hp_params& hp, uint64_t g_begin, uint64_t g_count,
                                uint16_t* d_pheno, int16_t* d_gap, cudaStream_t st) {
     using namespace tc;
@@ -778,16 +805,22 @@ gp_status gp_launch_scoring_tc(const gp_structures_s* s, const gp_hp_params& hp,
 
     // batches of 2^fb genotypes share a weight image; a launch covers up to `group` batches
     const uint64_t g_end = g_begin + g_count;
-    uint64_t group = (1024ULL << 20) / p.img_bytes;  // <= 1 GB of images per launch
+    uint64_t group = (512ULL << 20) / p.img_bytes;  // two buffers of <= 512 MB of images: one is built while the other is scored
     if (group < 1) group = 1;
     if (group > 256) group = 256;
     const uint64_t n_batches_all = ((g_end - 1) >> fb) - (g_begin >> fb) + 1;
     if (group > n_batches_all) group = n_batches_all;
-    int8_t* d_img = nullptr;  // per-call working memory from the stream-ordered pool: calls on other streams have their own
-    GP_CUDA(cudaMallocAsync(&d_img, p.img_bytes * (size_t)group, st));
+    int8_t* d_img0 = nullptr;  // per-call working memory from the stream-ordered pool: calls on other streams have their own
+    GP_CUDA(cudaMallocAsync(&d_img0, 2 * p.img_bytes * (size_t)group, st));
+    ImagePipeline pipe;
+    {
+        gp_status ps = pipe.open(st);
+        if (ps != GP_OK) { cudaFreeAsync(d_img0, st); return ps; }
+    }
     uint64_t g = g_begin & ~(uint64_t)(SUPER - 1);  // g_begin is a multiple of gp_tile() = SUPER already
     gp_status result = GP_OK;
-    while (g < g_end) {
+    for (uint64_t grp = 0; g < g_end; grp++) {
+        int8_t* d_img = d_img0 + (grp & 1) * p.img_bytes * (size_t)group;
         const uint64_t b0 = g >> fb;
         uint64_t stop = (b0 + group) << fb;
         if (stop > g_end) stop = g_end;
@@ -796,10 +829,12 @@ gp_status gp_launch_scoring_tc(const gp_structures_s* s, const gp_hp_params& hp,
         ia.contacts = s->d_contacts; ia.class_of = s->d_class_of; ia.img = d_img; ia.units = nullptr;
         ia.gfix_first = b0; ia.unit_first = 0; ia.paired = 0; ia.mid = 0; ia.gfix_shift = fb; ia.D = s->D; ia.n_tiles = p.n_tiles;
         ia.NBP = s->NBP; ia.lin = hp.lin; ia.quad = hp.quad;
-        gp_time_begin(GP_KERNEL_IMAGE, st);
-        if (p.narrow) build_image_kernel<64><<<dim3(p.n_tiles, (n_batches + IMG_PER_BLOCK - 1) / IMG_PER_BLOCK), TN, 0, st>>>(ia, p.slots, n_batches);
-        else build_image_kernel<128><<<dim3(p.n_tiles, (n_batches + IMG_PER_BLOCK - 1) / IMG_PER_BLOCK), TN, 0, st>>>(ia, p.slots, n_batches);
-        gp_time_end(GP_KERNEL_IMAGE, st);
+        pipe.before_build(grp);
+        gp_time_begin(GP_KERNEL_IMAGE, pipe.side);
+        if (p.narrow) build_image_kernel<64><<<dim3(p.n_tiles, (n_batches + IMG_PER_BLOCK - 1) / IMG_PER_BLOCK), TN, 0, pipe.side>>>(ia, p.slots, n_batches);
+        else build_image_kernel<128><<<dim3(p.n_tiles, (n_batches + IMG_PER_BLOCK - 1) / IMG_PER_BLOCK), TN, 0, pipe.side>>>(ia, p.slots, n_batches);
+        gp_time_end(GP_KERNEL_IMAGE, pipe.side);
+        pipe.after_build(grp, st);
         Args a;
         a.img = d_img; a.class_of = s->d_class_of; a.pheno = d_pheno; a.gap = d_gap;
         a.g_first = g; a.g_end = stop; a.out_base = g_begin;
@@ -810,12 +845,13 @@ gp_status gp_launch_scoring_tc(const gp_structures_s* s, const gp_hp_params& hp,
         gp_time_begin(GP_KERNEL_SCORING, st);
         p.kernel<<<grid, p.threads, p.smem, st>>>(a, p.cols);
         gp_time_end(GP_KERNEL_SCORING, st);
+        pipe.after_scoring(grp, st);
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) { gp_set_cuda_error(e, "scoring launch"); result = GP_CUDA_ERROR; break; }
         gp_count_launches(2);
         g = stop;
     }
-    cudaFreeAsync(d_img, st);
+    cudaFreeAsync(d_img0, st);
     return result;
 }
 
@@ -881,7 +917,7 @@ static gp_status gp_launch_map_range(const gp_structures_s* s, const gp_hp_param
     gp_status stt = make_plan(s, mon, fb, s->D_sym, p);
     if (stt != GP_OK) return stt;
     const size_t rec_bytes = sizeof(int4) << fb;
-    size_t group = (1024ULL << 20) / (p.img_bytes + rec_bytes);  // <= 1 GB of images + records per launch
+    size_t group = (1024ULL << 20) / (2 * p.img_bytes + rec_bytes);  // <= 1 GB: two image buffers + one record buffer
     if (group > 512) group = 512;
     group &= ~(size_t)1;
     if (group < 2) group = 2;
@@ -891,13 +927,18 @@ static gp_status gp_launch_map_range(const gp_structures_s* s, const gp_hp_param
         if (group > most) group = (size_t)((most + 1) & ~1ULL);
     }
     char* d_work = nullptr;
-    GP_CUDA(cudaMallocAsync(&d_work, (p.img_bytes + rec_bytes) * group, st));
-    int8_t* d_img = (int8_t*)d_work;
-    int4* d_rec = (int4*)(d_work + p.img_bytes * group);
+    GP_CUDA(cudaMallocAsync(&d_work, (2 * p.img_bytes + rec_bytes) * group, st));
+    int4* d_rec = (int4*)(d_work + 2 * p.img_bytes * group);
+    ImagePipeline pipe;
+    {
+        gp_status ps = pipe.open(st);
+        if (ps != GP_OK) { cudaFreeAsync(d_work, st); return ps; }
+    }
     gp_status result = GP_OK;
     uint64_t u = u_first, images_done = 0;
     const uint64_t u_end = u_first + u_count;
-    while (u < u_end) {
+    for (uint64_t grp = 0; u < u_end; grp++) {
+        int8_t* d_img = (int8_t*)d_work + (grp & 1) * p.img_bytes * group;
         const int paired = u < s->n_pair_units;
         uint64_t stop = paired ? u + group / 2 : u + group;
         const uint64_t limit = paired && s->n_pair_units < u_end ? s->n_pair_units : u_end;
@@ -907,10 +948,12 @@ static gp_status gp_launch_map_range(const gp_structures_s* s, const gp_hp_param
         ia.contacts = s->d_contacts_sym; ia.class_of = s->d_class_sym; ia.img = d_img; ia.units = s->d_units;
         ia.gfix_first = 0; ia.unit_first = u; ia.paired = paired; ia.mid = mid; ia.gfix_shift = k; ia.D = s->D_sym;
         ia.n_tiles = p.n_tiles; ia.NBP = s->NBP; ia.lin = hp.lin; ia.quad = hp.quad;
-        gp_time_begin(GP_KERNEL_IMAGE, st);
-        if (p.narrow) build_image_kernel<64><<<dim3(p.n_tiles, (n_img + IMG_PER_BLOCK - 1) / IMG_PER_BLOCK), TN, 0, st>>>(ia, p.slots, n_img);
-        else build_image_kernel<128><<<dim3(p.n_tiles, (n_img + IMG_PER_BLOCK - 1) / IMG_PER_BLOCK), TN, 0, st>>>(ia, p.slots, n_img);
-        gp_time_end(GP_KERNEL_IMAGE, st);
+        pipe.before_build(grp);
+        gp_time_begin(GP_KERNEL_IMAGE, pipe.side);
+        if (p.narrow) build_image_kernel<64><<<dim3(p.n_tiles, (n_img + IMG_PER_BLOCK - 1) / IMG_PER_BLOCK), TN, 0, pipe.side>>>(ia, p.slots, n_img);
+        else build_image_kernel<128><<<dim3(p.n_tiles, (n_img + IMG_PER_BLOCK - 1) / IMG_PER_BLOCK), TN, 0, pipe.side>>>(ia, p.slots, n_img);
+        gp_time_end(GP_KERNEL_IMAGE, pipe.side);
+        pipe.after_build(grp, st);
         Args a;
         a.img = d_img; a.class_of = s->d_class_sym; a.pheno = nullptr; a.gap = nullptr;
         a.g_first = 0; a.g_end = (uint64_t)n_img << fb; a.out_base = 0;
@@ -921,6 +964,7 @@ static gp_status gp_launch_map_range(const gp_structures_s* s, const gp_hp_param
         gp_time_begin(GP_KERNEL_SCORING, st);
         p.kernel<<<grid, p.threads, p.smem, st>>>(a, p.cols);
         gp_time_end(GP_KERNEL_SCORING, st);
+        pipe.after_scoring(grp, st);
         CombArgs ca;
         ca.hrec = d_rec; ca.units = s->d_units; ca.class_sym = s->d_class_sym;
         ca.pheno = d_pheno; ca.gap = d_gap; ca.unit_first = u; ca.n_images = n_img; ca.paired = paired; ca.mid = mid;
