@@ -89,18 +89,25 @@ class DistComm:
     def exchange(self, mine, partner_rank, chunk, offset):
         """Swap `chunk` entries at `offset` of the shard with the partner rank; returns the partner's entries."""
         send = mine[offset:offset + chunk]
-        recv = torch.empty_like(send)
+        stage = self.backend == "gloo" and send.is_cuda     # gloo moves host memory only: stage device shards through it
+        src = send.cpu() if stage else send
+        recv = torch.empty_like(src)
         # 16-bit integers are not an NCCL data type: ship the bytes
-        ops = [dist.P2POp(dist.isend, send.view(torch.uint8), partner_rank, self.group),
+        ops = [dist.P2POp(dist.isend, src.view(torch.uint8), partner_rank, self.group),
                dist.P2POp(dist.irecv, recv.view(torch.uint8), partner_rank, self.group)]
         for req in dist.batch_isend_irecv(ops):
             req.wait()
         self.bytes_sent += send.numel() * send.element_size()
-        return recv
+        return recv.to(send.device) if stage else recv
 
     def sum_(self, *tensors):
         for t in tensors:
-            dist.all_reduce(t, op=dist.ReduceOp.SUM, group=self.group)
+            if self.backend == "gloo" and t.is_cuda:
+                h = t.cpu()
+                dist.all_reduce(h, op=dist.ReduceOp.SUM, group=self.group)
+                t.copy_(h)
+            else:
+                dist.all_reduce(t, op=dist.ReduceOp.SUM, group=self.group)
             self.bytes_sent += t.numel() * t.element_size()
         return tensors
 
@@ -108,8 +115,11 @@ class DistComm:
         """OR-reduce the pair bitmaps of all ranks, in place."""
         if self.world == 1:
             return bitmap
-        if self.backend == "gloo" and not bitmap.is_cuda:
-            dist.all_reduce(bitmap, op=dist.ReduceOp.BOR, group=self.group)
+        if self.backend == "gloo":
+            h = bitmap.cpu() if bitmap.is_cuda else bitmap
+            dist.all_reduce(h, op=dist.ReduceOp.BOR, group=self.group)
+            if bitmap.is_cuda:
+                bitmap.copy_(h)
         else:
             parts = [torch.empty_like(bitmap) for _ in range(self.world)]
             dist.all_gather(parts, bitmap, group=self.group)

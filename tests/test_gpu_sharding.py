@@ -61,3 +61,48 @@ def test_cross_shard_flip_on_synthetic_stores():
     got = rdo.cpu().numpy().astype(np.uint64)
     assert np.array_equal(got[0], Ro) and np.array_equal(got[1], Do) and np.array_equal(got[2], Oo)
     assert int(gpmap.pair_bitmap_count(bm, C)) == pco
+
+
+def _rank_main(rank, world, port, out):
+    """One rank of a two-process run on the same device: libgpmap for every kernel, torch.distributed (gloo, device
+    shards staged through the host) for every exchange.  The two processes never wait for each other inside a kernel."""
+    import os
+    import torch.distributed as dist
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    torch.cuda.set_device(0)
+    S = gpmap.Structures(5, 5)
+    b, c = sharding.shard_range(S.N, world, rank, gpmap.tile())
+    shard = torch.empty(c, dtype=torch.uint16, device="cuda")
+    S.enumerate(b, c, shard)
+    comm = sharding.DistComm()
+    hist, R, D, O, pairs = sharding.reduce_store_sharded(sharding.LibOps(), comm, shard, S.N, S.C, chunk_entries=1 << 22)
+    out.put((rank, hist.cpu().numpy(), R.cpu().numpy(), D.cpu().numpy(), O.cpu().numpy(), int(pairs), comm.bytes_sent))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_two_processes_with_libgpmap_over_torch_distributed():
+    """reduce_store_sharded end to end: two processes, each scores and reduces its own top-bit shard of the 5x5 map with
+    libgpmap and exchanges shards / counts / bitmap through torch.distributed; every rank ends with the golden whole-map
+    integers."""
+    import socket
+    import torch.multiprocessing as mp
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    ctx = mp.get_context("spawn")
+    out = ctx.Queue()
+    procs = [ctx.Process(target=_rank_main, args=(r, 2, port, out)) for r in range(2)]
+    for p in procs:
+        p.start()
+    results = [out.get(timeout=300) for _ in range(2)]
+    for p in procs:
+        p.join(timeout=120)
+        assert p.exitcode == 0
+    gold = read_whole_maps()["5x5"]
+    for rank, hist, R, D, O, pairs, sent in results:
+        assert int(hist[:-1].sum()) == gold["folding"] and int(hist[-1]) == gold["null"], rank
+        assert (int(R.sum()), int(D.sum()), int(O.sum()), pairs) == (gold["sumR"], gold["sumD"], gold["sumO"], gold["pairs"]), rank
+        assert sent >= 2 << 24                              # one shard swap of 2^24 entries
+    assert np.array_equal(results[0][1], results[1][1]) and np.array_equal(results[0][2], results[1][2])
