@@ -9,13 +9,20 @@
 // recombines  v = acc_lo + 64 acc_hi = -(cost of S) = E - NBP emax  on packed int16 pairs before the same filtered
 // min / second-min / argmin fold as scoring_tc.cu (ties -> null, R6, R7).  Pad structures get v = +127 from a constant
 // column, above every real v <= 0.  Exact integer arithmetic throughout.
+//
+// Bound (profiles/r2_seq20_ncu.md): with one 128-sequence tile per CTA every incidence block feeds only two MMAs (lo, hi),
+// 2 KB of shared-memory ingest per 66-clock MMA = 31 B/clk/SM, and an SM takes 20-25 B/clk from L2 whatever the
+// mechanism (one cp.async.bulk per tile, per block, or a warp of 16-byte cp.async), ring depth or number of SMs running:
+// the kernel is bound by that feed at about 55 % tensor-pipe activity.
 #include <vector>
 
 #include "tc_common.cuh"
 
 namespace tc {
 
-constexpr int Q_KB_MAX = 3;                      // 128-byte column blocks per limb set: 2 + P <= 384 columns
+constexpr int QRB = 64;                          // bytes per operand row of a column block (64-byte swizzle): two K steps
+constexpr int QBLK = TM * QRB;                   // 8 KB: one column block of 128 rows
+constexpr int Q_KB_MAX = 6;                      // column blocks per limb set: 2 + P <= 384 columns
 constexpr int Q_STAGES_MAX = 6;                  // structure tiles (kb x 16 KB of incidence blocks each) in flight
 constexpr int Q_PARTS = 4;                       // column parts of a structure tile, one epilogue warp each per lane quarter
 constexpr int Q_THREADS = 32 * (2 + 4 * Q_PARTS); // warp 0 TMA producer, warp 1 MMA issuer, 16 builder / epilogue warps
@@ -26,7 +33,7 @@ constexpr int V_NONE = 32767;
 enum { QSRC_SEQS = 0, QSRC_SEEDED = 1 };
 
 struct QArgs {
-    const int8_t* img;        // [n_tiles][kb][TILE_BYTES] incidence blocks
+    const int8_t* img;        // [n_tiles][kb][QBLK] incidence blocks
     const uint16_t* class_of;
     const uint8_t* seqs;      // count x N letters (QSRC_SEQS)
     const uint8_t* pair_ij;   // P x 2 monomers of every pair column
@@ -90,25 +97,25 @@ __device__ __forceinline__ void fold_packed64(const uint32_t* w, uint32_t col0, 
 // Incidence image: one block = one 128-structure tile; thread = structure; the column blocks are built one by one.
 __global__ void __launch_bounds__(TN) build_pair_image_kernel(const uint16_t* __restrict__ pairidx, int8_t* __restrict__ img,
                                                               uint32_t D, int NBP, int kb) {
-    __shared__ __align__(16) int8_t tile[TILE_BYTES];
+    __shared__ __align__(16) int8_t tile[QBLK];
     const uint32_t r = threadIdx.x, n = blockIdx.x, d = n * TN + r;
     for (int b = 0; b < kb; b++) {
         __syncthreads();
-        for (uint32_t i = threadIdx.x; i < TILE_BYTES / 16; i += TN) reinterpret_cast<uint4*>(tile)[i] = make_uint4(0, 0, 0, 0);
+        for (uint32_t i = threadIdx.x; i < QBLK / 16; i += TN) reinterpret_cast<uint4*>(tile)[i] = make_uint4(0, 0, 0, 0);
         __syncthreads();
-        const int c0 = b * ROWB;
+        const int c0 = b * QRB;
         if (d < D) {
             const uint16_t* px = pairidx + (size_t)d * NBP;
             for (int k = 0; k < NBP; k++) {
                 const int c = 2 + px[k] - c0;
-                if (c >= 0 && c < ROWB) tile[swz(r, c)] = -1;
+                if (c >= 0 && c < QRB) tile[swz_rb<QRB>(r, c)] = -1;
             }
         } else if (b == 0) {
-            tile[swz(r, 0)] = V_PAD;   // pad structure: the constant column gives it v = +127
+            tile[swz_rb<QRB>(r, 0)] = V_PAD;   // pad structure: the constant column gives it v = +127
         }
         __syncthreads();
-        uint4* dst = reinterpret_cast<uint4*>(img + ((uint64_t)n * kb + b) * TILE_BYTES);
-        for (uint32_t i = threadIdx.x; i < TILE_BYTES / 16; i += TN) dst[i] = reinterpret_cast<const uint4*>(tile)[i];
+        uint4* dst = reinterpret_cast<uint4*>(img + ((uint64_t)n * kb + b) * QBLK);
+        for (uint32_t i = threadIdx.x; i < QBLK / 16; i += TN) dst[i] = reinterpret_cast<const uint4*>(tile)[i];
     }
 }
 
@@ -116,9 +123,9 @@ template <int SRC>
 __global__ void __launch_bounds__(Q_THREADS, 1) seq20_kernel(const QArgs a) {
     extern __shared__ unsigned char smem_dyn[];
     unsigned char* smem = reinterpret_cast<unsigned char*>(((uintptr_t)smem_dyn + 1023) & ~(uintptr_t)1023);
-    uint8_t* sA = smem;                                           // [lo | hi][kb][16 KB]
-    uint8_t* sB = sA + 2 * a.kb * TILE_BYTES;                     // a.stages x kb x 16 KB
-    QBarriers* bar = reinterpret_cast<QBarriers*>(sB + a.stages * a.kb * TILE_BYTES);
+    uint8_t* sA = smem;                                           // [lo | hi][kb][8 KB]
+    uint8_t* sB = sA + 2 * a.kb * QBLK;                           // a.stages x kb x 8 KB
+    QBarriers* bar = reinterpret_cast<QBarriers*>(sB + a.stages * a.kb * QBLK);
     const uint32_t Q_STAGES = (uint32_t)a.stages;
     uint8_t* let = reinterpret_cast<uint8_t*>(bar + 1);           // [N][128] letters of the item's sequences
     uint8_t* pij = let + a.N * Q_ROWS;                            // [P][2]
@@ -147,7 +154,7 @@ __global__ void __launch_bounds__(Q_THREADS, 1) seq20_kernel(const QArgs a) {
 
     if (warp == 0) {
         // ===== producer: one bulk copy per structure tile (its kb incidence blocks are contiguous), once per item =====
-        const uint32_t stage_bytes = (uint32_t)a.kb * TILE_BYTES;
+        const uint32_t stage_bytes = (uint32_t)a.kb * QBLK;
         uint32_t it = 0;
         for (uint32_t item = blockIdx.x; item < a.n_items; item += gridDim.x)
             for (uint32_t n = 0; n < a.n_tiles; n++, it++) {
@@ -162,8 +169,8 @@ __global__ void __launch_bounds__(Q_THREADS, 1) seq20_kernel(const QArgs a) {
     } else if (warp == 1) {
         // ===== MMA issuer: two chains (lo, hi limbs) per structure tile share every incidence block; accumulator pairs
         // double-buffered =====
-        const uint64_t a_lo0 = smem_desc(smem_u32(sA)), a_hi0 = smem_desc(smem_u32(sA + a.kb * TILE_BYTES));
-        const uint64_t b_desc0 = smem_desc(smem_u32(sB));
+        const uint64_t a_lo0 = smem_desc_rb<QRB>(smem_u32(sA)), a_hi0 = smem_desc_rb<QRB>(smem_u32(sA + a.kb * QBLK));
+        const uint64_t b_desc0 = smem_desc_rb<QRB>(smem_u32(sB));
         uint32_t tile_no = 0, item_no = 0;
         for (uint32_t item = blockIdx.x; item < a.n_items; item += gridDim.x, item_no++) {
             mbar_wait(&bar->a_full, item_no & 1);
@@ -177,10 +184,10 @@ __global__ void __launch_bounds__(Q_THREADS, 1) seq20_kernel(const QArgs a) {
                 mbar_wait(&bar->b_full[s], ph);
                 tc_fence_after();
                 if (elect_one()) {
-                    const uint64_t bd0 = b_desc0 + (uint64_t)s * (uint64_t)((a.kb * TILE_BYTES) >> 4);
+                    const uint64_t bd0 = b_desc0 + (uint64_t)s * (uint64_t)((a.kb * QBLK) >> 4);
                     for (int b = 0; b < a.kb; b++) {
-                        const uint64_t blk = (uint64_t)((b * TILE_BYTES) >> 4);
-                        const int nks = a.ksteps - 4 * b < 4 ? a.ksteps - 4 * b : 4;
+                        const uint64_t blk = (uint64_t)((b * QBLK) >> 4);
+                        const int nks = a.ksteps - 2 * b < 2 ? a.ksteps - 2 * b : 2;   // a 64-byte block holds two K steps
                         for (int ks = 0; ks < nks; ks++) {
                             const uint32_t acc = (b | ks) != 0;
                             mma_i8(d_lo, a_lo0 + blk + 2 * ks, bd0 + blk + 2 * ks, IDESC, acc);
@@ -214,14 +221,14 @@ __global__ void __launch_bounds__(Q_THREADS, 1) seq20_kernel(const QArgs a) {
             mbar_wait(&bar->a_empty, (item_no & 1) ^ 1);
             for (int b = part; b < 2 * a.kb; b += Q_PARTS)
 #pragma unroll
-                for (int c16 = 0; c16 < 8; c16++)
-                    *reinterpret_cast<uint4*>(sA + b * TILE_BYTES + r * ROWB + c16 * 16) = make_uint4(0, 0, 0, 0);
+                for (int c16 = 0; c16 < QRB / 16; c16++)
+                    *reinterpret_cast<uint4*>(sA + b * QBLK + r * QRB + c16 * 16) = make_uint4(0, 0, 0, 0);
             asm volatile("bar.sync %0, 128;" ::"r"(quarter + 1) : "memory");   // the row is zeroed before its bytes are set
-            if (part == 0) sA[swz(r, 0)] = 1;                        // constant column (lo limb set only)
-            uint8_t* sHi = sA + a.kb * TILE_BYTES;
+            if (part == 0) sA[swz_rb<QRB>(r, 0)] = 1;                        // constant column (lo limb set only)
+            uint8_t* sHi = sA + a.kb * QBLK;
             for (int p = part; p < a.P; p += Q_PARTS) {
                 const uint32_t c = (uint32_t)cost[my_let[pij[2 * p] * Q_ROWS] * a.alphabet + my_let[pij[2 * p + 1] * Q_ROWS]];
-                const uint32_t col = 2u + p, off = (col >> 7) * TILE_BYTES + swz(r, col & 127u);
+                const uint32_t col = 2u + p, off = (col >> 6) * QBLK + swz_rb<QRB>(r, col & 63u);
                 sA[off] = (uint8_t)(c & 63u);
                 sHi[off] = (uint8_t)(c >> 6);
             }
@@ -285,19 +292,19 @@ gp_status gp_launch_seq20_tc(const gp_structures_s* s, const gp_energies* en, in
                              uint64_t first, uint64_t count, uint16_t* d_pheno, int16_t* d_gap, cudaStream_t st) {
     using namespace tc;
     const int A = en->alphabet, ncol = 2 + s->P;
-    if (ncol > Q_KB_MAX * ROWB || s->N > 64 || s->D >= (1u << KEY_SHIFT) || A < 2 || A > 20) return GP_UNSUPPORTED_LATTICE;
+    if (ncol > Q_KB_MAX * QRB || s->N > 64 || s->D >= (1u << KEY_SHIFT) || A < 2 || A > 20) return GP_UNSUPPORTED_LATTICE;
     int32_t emax = INT32_MIN, emin = INT32_MAX;
     for (int i = 0; i < A * A; i++) { emax = en->e[i] > emax ? en->e[i] : emax; emin = en->e[i] < emin ? en->e[i] : emin; }
     if ((long long)emax - emin > 8191 || ((long long)emax - emin) * s->NBP > 32000) return GP_UNSUPPORTED_LATTICE;
     QArgs a;
     for (int i = 0; i < A * A; i++) a.cost[i] = (int16_t)(emax - en->e[i]);
-    const int kb = (ncol + ROWB - 1) / ROWB;
+    const int kb = (ncol + QRB - 1) / QRB;
     const uint32_t n_tiles = (s->D + TN - 1) / TN;
     {   // incidence image: depends on the lattice only; built once, other streams wait on its event
         std::lock_guard<std::mutex> lk(s->mu);
         if (!s->d_pair_img) {
             int8_t* img = nullptr;
-            GP_CUDA(cudaMalloc(&img, (size_t)n_tiles * kb * TILE_BYTES));  // first use on this handle only
+            GP_CUDA(cudaMalloc(&img, (size_t)n_tiles * kb * QBLK));  // first use on this handle only
             build_pair_image_kernel<<<n_tiles, TN, 0, st>>>(s->d_pairidx, img, s->D, s->NBP, kb);
             cudaError_t e = cudaGetLastError();
             cudaEvent_t ev = nullptr;
@@ -323,11 +330,11 @@ gp_status gp_launch_seq20_tc(const gp_structures_s* s, const gp_energies* en, in
                        (size_t)Q_PARTS * Q_ROWS * 16 + 1024 + 64;
     // a stage holds the kb incidence blocks of one structure tile, fetched by ONE bulk copy (16 KB copies were measured
     // to deliver a block per 940 clocks and SM, whatever the ring depth: profiles/r2_seq20_ncu.md)
-    int stages = (int)(((227 * 1024 - aux) / TILE_BYTES - 2 * kb) / kb);
+    int stages = (int)(((227 * 1024 - aux) / QBLK - 2 * kb) / kb);
     if (stages > Q_STAGES_MAX) stages = Q_STAGES_MAX;
     if (stages < 2) return GP_UNSUPPORTED_LATTICE;
     a.stages = stages;
-    const size_t smem = (size_t)(2 * kb + stages * kb) * TILE_BYTES + aux;
+    const size_t smem = (size_t)(2 * kb + stages * kb) * QBLK + aux;
     void (*k)(const QArgs) = seeded ? seq20_kernel<QSRC_SEEDED> : seq20_kernel<QSRC_SEQS>;
     GP_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const unsigned grid = a.n_items < (uint32_t)sms ? a.n_items : (uint32_t)sms;
