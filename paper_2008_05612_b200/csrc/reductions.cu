@@ -28,16 +28,20 @@ __global__ void __launch_bounds__(1024) hist_kernel(const uint16_t* __restrict__
         for (int u = 0; u < 4; u++) {
             if (i + u * stride >= nvec) break;
             const uint32_t w[4] = {xs[u].x, xs[u].y, xs[u].z, xs[u].w};
+            // nulls: per half min(~id, 1) is 0 exactly for 0xFFFF; four words summed, halves added at the end
+            const uint32_t nn = __vminu2(~w[0], 0x00010001u) + __vminu2(~w[1], 0x00010001u) + __vminu2(~w[2], 0x00010001u) +
+                                __vminu2(~w[3], 0x00010001u);
+            nulls += 8u - (nn & 0xFFFFu) - (nn >> 16);
+            // one compare per id: the null id 0xFFFF is >= C like every id the caller's n_classes does not cover
 #pragma unroll
             for (int j = 0; j < 4; j++) {
-#pragma unroll
-                for (int h = 0; h < 2; h++) {
-                    const uint32_t p = h ? (w[j] >> 16) : (w[j] & 0xFFFFu);
-                    if (p == NULLP) nulls++;
-                    else if (p < C) {
-                        if (use_smem) atomicAdd(&sh[p], 1u);
-                        else atomicAdd(&hist[p], 1ULL);
-                    }
+                const uint32_t p0 = w[j] & 0xFFFFu, p1 = w[j] >> 16;
+                if (use_smem) {
+                    if (p0 < C) atomicAdd(&sh[p0], 1u);
+                    if (p1 < C) atomicAdd(&sh[p1], 1u);
+                } else {
+                    if (p0 < C) atomicAdd(&hist[p0], 1ULL);
+                    if (p1 < C) atomicAdd(&hist[p1], 1ULL);
                 }
             }
         }
