@@ -292,17 +292,20 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * tot / len(times), "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "int32", "data": "synthetic",
-            "config": workload_config(args.lattice, G, O.D, O.C, O.N + sum(1 for i in range(O.N) for j in range(i + 3, O.N, 2)), 1 << G),
+            "config": workload_config(args.lattice, G, O.D, O.C, O.N + sum(1 for i in range(O.N) for j in range(i + 3, O.N, 2)), 1 << G,
+                                      full=args.full),
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
 
 
-def workload_config(lattice, G, D, C, K, n, parallelism="independent prefix tiles per rank, no collective"):
+def workload_config(lattice, G, D, C, K, n, parallelism="independent prefix tiles per rank, no collective", full=False):
     """The `config` object: identical keys in both arms."""
-    return {"workload": "%s HP genotype-prefix tile: 2^%d genotypes x %d directed structures, then designability + "
-                        "neighbour pass over the tile" % (lattice, G, D),
+    return {"workload": ("%s HP whole map (reversal identity): 2^%d genotypes x %d directed structures, then designability + "
+                         "neighbour pass" if full else
+                         "%s HP genotype-prefix tile: 2^%d genotypes x %d directed structures, then designability + "
+                         "neighbour pass over the tile") % (lattice, G, D),
             "lattice": lattice, "log2_genotypes": G, "D": D, "C": C, "features_K": K,
             "l2": "inputs larger than L2 (per step: %.0f MB phenotype tile, fresh seeded prefix, weight images rebuilt)"
                   % (2.0 * n / 1e6),
@@ -684,7 +687,7 @@ def run_ours(args):
                                                                         "bits: local scoring, hypercube shard exchange for the neighbour pass "
                                                                         "(%d bytes sent per rank and step), all_reduce of counts, OR-reduce of the "
                                                                         "pair bitmap" % (G + q, world, q, sharding.exchange_bytes_per_rank(G + q, world, C))]
-                                                                       if sharded else [])),
+                                                                       if sharded else []), full=args.full),
             "full_map_wall_s_extrapolated_from_tiles": total_evals_map / value * world if value else None,
             "folding_fraction_last_tile": folding / float(n) if folding is not None else None,
             "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline, "other_kernels": other,
