@@ -19,7 +19,8 @@
  *     call says it accumulates.  Working memory of a call comes from the device's stream-ordered pool
  *     (cudaMallocAsync on `stream`) and goes back to it on the same stream, so calls on one handle may run
  *     concurrently on different streams and threads; only gp_tuning_set and gp_structures_free must not overlap a
- *     call on the same handle.
+ *     call on the same handle.  A call may run part of its work (building weight images ahead of the scoring kernel)
+ *     on an internal stream of its own; events tie it into `stream`, so the caller sees everything ordered on `stream`.
  *   - Genotype g: bit i of g is the letter of monomer i, 1 = H (R3).  Null phenotype = GP_NULL_PHENO (R7).
  *   - Phenotype ids are reversal-reduced class ids 0..C-1 in the canonical order of DESIGN.md section 3 (R1, R8).
  */
