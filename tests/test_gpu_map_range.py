@@ -337,3 +337,54 @@ def test_full_map_run_survives_an_interruption(oracle_structures, tmp_path, latt
     once = full_map.run(lattice, str(tmp_path / "once"), chunks=3)
     for key in ("folding", "sum_R", "sum_D", "sum_O", "phenotype_pairs", "top5_designability"):
         assert once[key] == summary[key], key
+
+
+def test_threshold_sweep_on_synthetic_stores_with_many_classes():
+    """The global-atomic path of gp_threshold_sweep (bins do not fit shared memory: 3x3x3-sized class count) and ragged
+    counts, against a numpy restatement of the definition (folds iff second_min - min >= threshold)."""
+    rng = np.random.default_rng(21)
+    for n, C, thr in [((1 << 20) + 77, 51704, [1, 2, 5, 9, 30]), (5000, 28728, [3]), (1 << 16, 40, [7, 1, 4])]:
+        ph = rng.integers(0, C, size=n).astype(np.uint16)
+        ph[rng.random(n) < 0.6] = 0xFFFF
+        gap = -rng.integers(1, 40, size=n).astype(np.int16)
+        gap[rng.random(n) < 0.01] = -32768                     # "no second structure": folds at every threshold
+        d_ph = torch.from_numpy(ph.view(np.int16)).cuda().view(torch.uint16)
+        d_gap = torch.from_numpy(gap).cuda()
+        folding, hist = gpmap.threshold_sweep(d_ph, d_gap, C, thr)
+        for row, t in enumerate(thr):
+            ok = (ph != 0xFFFF) & ((gap == -32768) | (-gap.astype(np.int32) >= t))
+            want = np.bincount(ph[ok], minlength=C)
+            assert np.array_equal(hist[row, :C].cpu().numpy(), want), (n, t)
+            assert int(hist[row, C]) == n - int(ok.sum()) and int(folding[row]) == int(ok.sum()), (n, t)
+
+
+def test_int8_peak_probe_is_plausible():
+    """gp_probe_i8_peak: an M128 x N128 x K32 int8 MMA cannot take fewer than 64 clocks; the measured peak must sit between
+    half and all of the nominal 4.5e15 ops/s, and the reported clock between 1 and 2 GHz."""
+    for k_steps in (1, 2, 4):
+        ops, clk, mhz = gpmap.probe_i8_peak(k_steps, 0.05)
+        assert 64.0 <= clk < 80.0, (k_steps, clk)
+        assert 2.2e15 < ops < 4.9e15, (k_steps, ops)
+        assert 1000.0 < mhz < 2100.0, (k_steps, mhz)
+    with pytest.raises(gpmap.GpError):
+        gpmap.probe_i8_peak(5, 0.05)
+
+
+def test_reduce_store_at_the_bench_tile_size(oracle_structures):
+    """gp_reduce_store == gp_designability + gp_robustness on a 2^26-genotype 6x6 tile (the bench step's size: two passes,
+    16 + 10 flips), and on its first 2^17 entries == the oracle's reductions."""
+    S = lib_structures((6, 6, 1))
+    G, n = 26, 1 << 26
+    ph = torch.empty(n, dtype=torch.uint16, device="cuda")
+    S.enumerate(0x2A5 << G, n, ph)
+    hist = gpmap.designability(ph, S.C)
+    R, Dl, Oc, pc = gpmap.robustness(ph, G, S.C)
+    h2, R2, D2, O2, pc2 = gpmap.reduce_store(ph, G, S.C)
+    assert torch.equal(hist, h2) and torch.equal(R, R2) and torch.equal(Dl, D2) and torch.equal(Oc, O2) and int(pc) == int(pc2)
+    small = ph[:1 << 17]
+    store = small.cpu().numpy()
+    h3, R3, D3, O3, pc3 = gpmap.reduce_store(small, 17, S.C)
+    Ro, Do, Oo, pco = orc.robustness(store, 17, S.C)
+    assert np.array_equal(h3.cpu().numpy().astype(np.uint64), orc.designability(store, S.C))
+    assert np.array_equal(R3.cpu().numpy().astype(np.uint64), Ro) and np.array_equal(D3.cpu().numpy().astype(np.uint64), Do)
+    assert np.array_equal(O3.cpu().numpy().astype(np.uint64), Oo) and int(pc3) == pco
