@@ -2,6 +2,7 @@
 pair count.
 
     python -m paper_2008_05612_b200.full_map --lattice 6x6 --out gpurun_out/map_6x6 [--chunks 64] [--resume]
+    torchrun --nproc-per-node 8 -m paper_2008_05612_b200.full_map --lattice 6x6 --out out/map_6x6 --sharded
 
 The map is scored as `chunks` ranges of units through gp_enumerate_map_range (include/gpmap.h; the paper's own 110-day
 job survived by appending results run by run).  After every chunk <out>/progress.json
@@ -136,6 +137,63 @@ def run(lattice, out, chunks=64, sample=1 << 20, seed=200805612, keep_store=Fals
     return (summary, pheno, S) if keep_store else summary
 
 
+def run_sharded(lattice, out, backend=None):
+    """Whole map over the ranks of a torch.distributed job (torchrun, one process per GPU): the store is sharded on the
+    top log2(world) genotype bits (sharding.py).  Every rank scores its own shard with gp_enumerate,
+    reduces it with libgpmap and exchanges shards / counts / pair bitmap; rank 0 writes summary.json.  With 8 GPUs the
+    6x6 store is 17 GB per rank."""
+    import torch
+    import torch.distributed as dist
+    from . import gpmap, sharding
+
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local % max(1, torch.cuda.device_count()))
+    if not dist.is_initialized():
+        dist.init_process_group(backend or ("nccl" if torch.cuda.device_count() >= world else "gloo"))
+    S = gpmap.Structures(*LATTICES[lattice])
+    N, D, C = S.N, S.D, S.C
+    b, c = sharding.shard_range(N, world, rank, gpmap.tile())
+    shard = torch.empty(c, dtype=torch.uint16, device="cuda")
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+    dist.barrier()
+    torch.cuda.synchronize()
+    ev[0].record()
+    step = 1 << 30
+    for off in range(0, c, step):
+        S.enumerate(b + off, min(step, c - off), shard[off:off + step])
+    ev[1].record()
+    comm = sharding.DistComm()
+    hist, R, Dl, Oc, pairs = sharding.reduce_store_sharded(sharding.LibOps(), comm, shard, N, C)
+    ev[2].record()
+    torch.cuda.synchronize()
+    dev = "cpu" if comm.backend == "gloo" else "cuda"
+    t_score = comm.max_(ev[0].elapsed_time(ev[1]) * 1e-3, dev)
+    t_red = comm.max_(ev[1].elapsed_time(ev[2]) * 1e-3, dev)
+    summary = None
+    if rank == 0:
+        hist = hist.cpu().numpy().astype(np.uint64)
+        R, Dl, Oc = (x.cpu().numpy().astype(np.uint64) for x in (R, Dl, Oc))
+        folding = int(hist[:C].sum())
+        summary = {"lattice": lattice, "N": N, "D": D, "C": C, "world": world, "genotypes": 1 << N,
+                   "path": "gp_enumerate per rank (prefix tiles, D columns), sharded reductions",
+                   "seconds": {"scoring": t_score, "reductions_and_exchange": t_red, "total": t_score + t_red},
+                   "evals_per_s_scoring": float(1 << N) * D / t_score,
+                   "bytes_sent_per_rank": comm.bytes_sent, "folding": folding, "null": int(hist[C]),
+                   "sum_R": int(R.sum()), "sum_D": int(Dl.sum()), "sum_O": int(Oc.sum()), "phenotype_pairs": int(pairs),
+                   "checks": {"hist_sums_to_2^N": int(hist.sum()) == 1 << N,
+                              "R+D+O_equals_N_x_folding": int(R.sum() + Dl.sum() + Oc.sum()) == N * folding,
+                              "sum_R_even": int(R.sum()) % 2 == 0, "sum_O_even": int(Oc.sum()) % 2 == 0}}
+        os.makedirs(out, exist_ok=True)
+        np.savez_compressed(os.path.join(out, "counts.npz"), hist=hist, R=R, D=Dl, O=Oc)
+        with open(os.path.join(out, "summary.json"), "w") as f:
+            json.dump(summary, f, indent=1)
+    dist.barrier()
+    S.close()
+    dist.destroy_process_group()
+    return summary
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--lattice", default="6x6", choices=sorted(LATTICES))
@@ -144,7 +202,13 @@ def main():
     ap.add_argument("--resume", action="store_true", help="continue from <out>/progress.json (needs a saved store)")
     ap.add_argument("--checkpoint-store", action="store_true", help="save the store after every chunk (up to 3x3x3)")
     ap.add_argument("--prefix-path", action="store_true", help="score with gp_enumerate instead of gp_enumerate_map_range")
+    ap.add_argument("--sharded", action="store_true", help="run under torchrun: the store sharded over the ranks (sharding.py)")
     a = ap.parse_args()
+    if a.sharded:
+        summary = run_sharded(a.lattice, a.out)
+        if summary is not None:
+            print(json.dumps(summary))
+        raise SystemExit(0 if summary is None or all(summary["checks"].values()) else 1)
     summary = run(a.lattice, a.out, a.chunks, prefix_path=a.prefix_path, resume=a.resume, checkpoint_store=a.checkpoint_store)
     print(json.dumps(summary))
     raise SystemExit(0 if all(v is True or v == 0 for v in summary["checks"].values()) else 1)

@@ -106,3 +106,29 @@ def test_two_processes_with_libgpmap_over_torch_distributed():
         assert (int(R.sum()), int(D.sum()), int(O.sum()), pairs) == (gold["sumR"], gold["sumD"], gold["sumO"], gold["pairs"]), rank
         assert sent >= 2 << 24                              # one shard swap of 2^24 entries
     assert np.array_equal(results[0][1], results[1][1]) and np.array_equal(results[0][2], results[1][2])
+
+
+def test_full_map_cli_sharded_under_torchrun(tmp_path):
+    """`torchrun -m paper_2008_05612_b200.full_map --sharded` with two ranks (gloo between them when the box has one GPU):
+    the summary rank 0 writes carries the golden whole-map integers of the 5x5 lattice and passes its own checks."""
+    import json
+    import os
+    import socket
+    import subprocess
+    import sys
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    out = str(tmp_path / "map")
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), "-m", "paper_2008_05612_b200.full_map", "--lattice", "5x5", "--out", out, "--sharded"]
+    r = subprocess.run(cmd, cwd=root, capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0, r.stderr[-2000:]
+    with open(os.path.join(out, "summary.json")) as f:
+        s = json.load(f)
+    gold = read_whole_maps()["5x5"]
+    assert s["world"] == 2 and all(s["checks"].values())
+    assert (s["folding"], s["null"], s["sum_R"], s["sum_D"], s["sum_O"], s["phenotype_pairs"]) == \
+        (gold["folding"], gold["null"], gold["sumR"], gold["sumD"], gold["sumO"], gold["pairs"])
+    assert s["bytes_sent_per_rank"] >= 2 << 24
