@@ -338,6 +338,142 @@ __global__ void __launch_bounds__(R2THREADS, 1) robustness2_kernel(Rob2Args a) {
     }
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// a6, the tile kernel with a DIRECT class table (used whenever 4 C bytes fit beside a 2^15 tile: every box of the paper).
+// The flips are those of robustness2_kernel; what changes is where the per-genotype counts go.  One 32-bit word per
+// class holds three fields, neutral (10 bits) | to-null (11 bits) | other (11 bits), and every non-null genotype does
+// ONE shared-memory atomic add of its (r, d, o) word (at most 15 flips per pass, so each term is at most 15).  The add
+// returns the old word, from which the carries out of the three fields are known exactly ((old & w) | ((old | w) &
+// ~(old + w))): a carry out of a field is booked in the 64-bit global counters (+2^bits for the field that wrapped,
+// -1 for the field above it that received the carry), so the fields may wrap as often as they like and the table is
+// written back once, when the block has done all its tiles.  No hashing, no probing, no runs, no periodic flush.
+// The genotype count per class (designability) is (r + d + o) / flips; the launcher reads it from per-call totals.
+// ---------------------------------------------------------------------------------------------------------------
+constexpr int ROB3_TB_MAX = 15;
+constexpr uint32_t ROB3_C_MAX = 34304;   // 4 C bytes + 64 KB tile + bitmask + table + pair filter + rings <= 227 KB
+
+__device__ __noinline__ void rob3_carry(const Rob2Args& a, uint32_t p, uint32_t c) {
+    if (c & 0x200u) { atomicAdd(&a.R[p], 1024ULL); atomicAdd(&a.Dl[p], ~0ULL); }
+    if (c & 0x100000u) { atomicAdd(&a.Dl[p], 2048ULL); atomicAdd(&a.O[p], ~0ULL); }
+    if (c & 0x80000000u) atomicAdd(&a.O[p], 2048ULL);
+}
+
+template <bool PAIRS>
+__global__ void __launch_bounds__(R2THREADS, 1) robustness3_kernel(Rob2Args a) {
+    extern __shared__ __align__(16) uint16_t seg[];
+    const uint32_t n_vec = 1u << (a.tb - 3);                       // 16-byte vectors per tile
+    uint8_t* nnb = reinterpret_cast<uint8_t*>(seg + ((size_t)1 << a.tb));  // per vector: bit i = genotype i is NOT null
+    uint32_t* lut = reinterpret_cast<uint32_t*>(nnb + ((n_vec + 15u) & ~15u));  // byte -> eight nibbles
+    uint32_t* tab = lut + 256;                                     // per class: r | d << 10 | o << 21
+    uint32_t* pf = tab + ((a.C + 3u) & ~3u);
+    uint32_t* ring = pf + ROB2_PF_SLOTS + (threadIdx.x >> 5) * ROB2_RING;  // this warp's event ring (PAIRS only)
+    uint32_t head = 0, tail = 0;
+    for (uint32_t i = threadIdx.x; i < 256; i += blockDim.x) {
+        uint32_t x = 0;
+        for (int b = 0; b < 8; b++) x |= ((i >> b) & 1u) << (4 * b);
+        lut[i] = x;
+    }
+    for (uint32_t i = threadIdx.x; i < a.C; i += blockDim.x) tab[i] = 0;
+    if (PAIRS)
+        for (uint32_t i = threadIdx.x; i < ROB2_PF_SLOTS; i += blockDim.x) pf[i] = 0xFFFFFFFFu;
+    uint32_t last_key = 0xFFFFFFFFu;
+    unsigned long long nulls = 0;
+    const uint64_t n_tiles = 1ULL << (a.n_bits - a.tb);
+    const uint32_t cmask = (1u << a.c) - 1u;
+    const int lo_outer = a.hi_pos - a.c;                           // outer-index bits that sit below the spread bits
+    const uint32_t n_flip = (uint32_t)(a.tb - a.f0);
+    const int k_lo = a.f0 < 3 ? 3 : a.f0;                          // first flip that needs a partner vector
+    // word of one genotype = (nf - rn) | (nf - nn) << 10 | (rn - nf + nn) << 21, rn = differing, nn = non-null neighbours
+    const uint32_t w0 = n_flip * (1u + (1u << 10) - (1u << 21)), w_rn = (1u << 21) - 1u, w_nn = (1u << 21) - (1u << 10);
+    const uint4* sv = reinterpret_cast<const uint4*>(seg);
+    const RobArgs pa = {a.pheno, a.n_bits, a.C, a.R, a.Dl, a.O, a.bitmap, a.tb, a.c, a.h, a.hi_pos, a.f0};
+    for (uint64_t t = blockIdx.x; t < n_tiles; t += gridDim.x) {
+        const uint64_t base = ((t & ((1ULL << lo_outer) - 1ULL)) << a.c) | ((t >> lo_outer) << (a.hi_pos + a.h));
+        __syncthreads();
+        for (uint32_t v = threadIdx.x; v < n_vec; v += R2THREADS) {
+            const uint32_t l = v << 3;
+            const uint64_t g = base | (l & cmask) | ((uint64_t)(l >> a.c) << a.hi_pos);
+            const uint4 x = __ldg(reinterpret_cast<const uint4*>(a.pheno + g));
+            reinterpret_cast<uint4*>(seg)[v] = x;
+            const uint32_t n0 = __vminu2(~x.x, 0x00010001u), n1 = __vminu2(~x.y, 0x00010001u);
+            const uint32_t n2 = __vminu2(~x.z, 0x00010001u), n3 = __vminu2(~x.w, 0x00010001u);
+            const uint32_t tt = n0 + (n1 << 2) + (n2 << 4) + (n3 << 6);
+            const uint32_t nb = (tt | (tt >> 15)) & 0xFFu;
+            nnb[v] = (uint8_t)nb;
+            nulls += 8 - __popc(nb);
+        }
+        __syncthreads();
+        for (uint32_t v0 = 0; v0 < n_vec; v0 += R2THREADS) {       // uniform trip count: the warp stays converged
+            const uint32_t v = v0 + threadIdx.x;
+            const bool live = v < n_vec;
+            const uint32_t Bm = live ? nnb[v] : 0u;
+            if (__all_sync(0xFFFFFFFFu, Bm == 0)) continue;         // the warp's 256 genotypes are all null: nothing to count
+            const uint4 mv = live ? sv[v] : make_uint4(~0u, ~0u, ~0u, ~0u);
+            const uint32_t m[4] = {mv.x, mv.y, mv.z, mv.w};
+            uint32_t rne[4] = {0, 0, 0, 0};                        // per half: flips whose neighbour differs (class or null)
+            uint32_t nn = 0;                                       // per nibble: non-null neighbours (at most 15 flips)
+            if (a.f0 == 0) {                                       // flips of local bits 0-2 stay inside the vector
+                rob2_flip<PAIRS>(pa, seg, pf, last_key, ring, head, tail, m, __funnelshift_l(m[0], m[0], 16),
+                                 __funnelshift_l(m[1], m[1], 16), __funnelshift_l(m[2], m[2], 16), __funnelshift_l(m[3], m[3], 16),
+                                 Bm, ((Bm & 0x55u) << 1) | ((Bm >> 1) & 0x55u), 0x55u, v, 0u, lut, rne, nn);
+                rob2_flip<PAIRS>(pa, seg, pf, last_key, ring, head, tail, m, m[1], m[0], m[3], m[2], Bm,
+                                 ((Bm & 0x33u) << 2) | ((Bm >> 2) & 0x33u), 0x33u, v, 1u, lut, rne, nn);
+                rob2_flip<PAIRS>(pa, seg, pf, last_key, ring, head, tail, m, m[2], m[3], m[0], m[1], Bm,
+                                 ((Bm & 0x0Fu) << 4) | (Bm >> 4), 0x0Fu, v, 2u, lut, rne, nn);
+            }
+#pragma unroll 4
+            for (int k = k_lo; k < a.tb; k++) {
+                const uint32_t pv = (v ^ (1u << (k - 3))) & (n_vec - 1);
+                const uint4 x = sv[pv];
+                rob2_flip<PAIRS>(pa, seg, pf, last_key, ring, head, tail, m, x.x, x.y, x.z, x.w, Bm, nnb[pv],
+                                 pv > v ? 0xFFu : 0u, v, (uint32_t)k, lut, rne, nn);
+            }
+            uint32_t old[8], w[8];
+#pragma unroll
+            for (int j = 0; j < 8; j++) {
+                const uint32_t p = (m[j >> 1] >> (16 * (j & 1))) & 0xFFFFu;
+                w[j] = w0 + ((rne[j >> 1] >> (16 * (j & 1))) & 0xFFFFu) * w_rn + ((nn >> (4 * j)) & 15u) * w_nn;
+                old[j] = 0;
+                if (p < a.C) old[j] = atomicAdd(&tab[p], w[j]); else w[j] = 0;
+            }
+#pragma unroll
+            for (int j = 0; j < 8; j++) {
+                const uint32_t c = ((old[j] & w[j]) | ((old[j] | w[j]) & ~(old[j] + w[j]))) & 0x80100200u;
+                if (c) rob3_carry(a, (m[j >> 1] >> (16 * (j & 1))) & 0xFFFFu, c);
+            }
+        }
+        if (PAIRS && tail != head) {                                // events left in the ring: the tile is about to be replaced
+            __syncwarp();
+            const uint32_t lane = threadIdx.x & 31u;
+            if (lane < tail - head) rob2_events(pa, seg, pf, last_key, ring[(head + lane) & (ROB2_RING - 1)]);
+            head = tail;
+            __syncwarp();
+        }
+    }
+    __syncthreads();
+    for (uint32_t i = threadIdx.x; i < a.C; i += blockDim.x) {
+        const uint32_t w = tab[i];
+        if (w & 1023u) atomicAdd(&a.R[i], (unsigned long long)(w & 1023u));
+        if ((w >> 10) & 2047u) atomicAdd(&a.Dl[i], (unsigned long long)((w >> 10) & 2047u));
+        if (w >> 21) atomicAdd(&a.O[i], (unsigned long long)(w >> 21));
+    }
+    if (a.hist) {                                                   // only the null count: the classes come from the totals
+        for (int o = 16; o > 0; o >>= 1) nulls += __shfl_down_sync(0xFFFFFFFFu, nulls, o);
+        if ((threadIdx.x & 31) == 0 && nulls) atomicAdd(&a.hist[a.C], nulls);
+    }
+}
+
+// After a pass whose (R, D, O) went to per-call totals: add them to the caller's arrays; every genotype of class p gave
+// exactly `flips` to r + d + o, so the class's genotype count is the sum / flips.
+__global__ void rob3_finish_kernel(const unsigned long long* tot, uint32_t C, uint32_t flips, unsigned long long* R,
+                                   unsigned long long* Dl, unsigned long long* O, unsigned long long* hist) {
+    const uint32_t p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= C) return;
+    const unsigned long long r = tot[p], d = tot[C + p], o = tot[2 * (size_t)C + p];
+    R[p] += r; Dl[p] += d; O[p] += o;
+    hist[p] += (r + d + o) / flips;
+}
+
 // n_bits < 3 (fewer than 8 genotypes): one thread per genotype, straight from global memory.
 __global__ void robustness_tiny_kernel(RobArgs a) {
     const uint32_t g = threadIdx.x;
@@ -580,27 +716,38 @@ static gp_status robustness_passes(const uint16_t* d_pheno, int n_bits, uint32_t
         }
         return GP_OK;
     }
-    int tb = tile_bits ? tile_bits : ROB2_TB_MAX;
+    // the direct-table kernel whenever the class table fits beside a 2^15 tile; tile_bits = 16 asks for the hashed one
+    const bool direct = n_classes <= ROB3_C_MAX && tile_bits <= ROB3_TB_MAX;
+    int tb = tile_bits ? tile_bits : (direct ? ROB3_TB_MAX : ROB2_TB_MAX);
     if (tb > n_bits) tb = n_bits;
     const uint64_t n_tiles = 1ULL << (n_bits - tb);
     const uint64_t cap = (uint64_t)sm_count();
     const unsigned grid = (unsigned)(n_tiles < cap ? n_tiles : cap);
-    const size_t smem = ((size_t)2 << tb) + ((((size_t)1 << (tb - 3)) + 15) & ~(size_t)15) + 1024 + ROB2_SLOTS * sizeof(Rob2Slot) +
-                        ROB2_PF_SLOTS * sizeof(uint32_t) + (R2THREADS / 32) * ROB2_RING * sizeof(uint32_t);
-    if (d_pair_bitmap) GP_CUDA(cudaFuncSetAttribute(robustness2_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    else GP_CUDA(cudaFuncSetAttribute(robustness2_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const size_t smem_tile = ((size_t)2 << tb) + ((((size_t)1 << (tb - 3)) + 15) & ~(size_t)15) + 1024 +
+                             ROB2_PF_SLOTS * sizeof(uint32_t) + (R2THREADS / 32) * ROB2_RING * sizeof(uint32_t);
+    const size_t smem = smem_tile + (direct ? (size_t)((n_classes + 3u) & ~3u) * 4 : ROB2_SLOTS * sizeof(Rob2Slot));
+    if (direct) {
+        if (d_pair_bitmap) GP_CUDA(cudaFuncSetAttribute(robustness3_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        else GP_CUDA(cudaFuncSetAttribute(robustness3_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    } else {
+        if (d_pair_bitmap) GP_CUDA(cudaFuncSetAttribute(robustness2_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        else GP_CUDA(cudaFuncSetAttribute(robustness2_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    }
     a.tb = tb;
     // pass 0: the tb low bits; every later pass flips its own spread bits: segments of 2^c consecutive ids (128 bytes
-    // when the tile allows, never under 16), all 2^h values of the spread bits on chip
-    const int seg_bits = 6;
+    // with the hashed kernel's 2^16 tiles, 32 or 64 bytes with the direct kernel's 2^15, never under 16), all 2^h values
+    // of the spread bits on chip; the remaining bits are split evenly over the fewest passes
+    const int seg_bits = direct ? 4 : 6;
+    const int hmax = tb - seg_bits > 1 ? tb - seg_bits : (tb - 3 > 1 ? tb - 3 : 1);
+    int passes_left = (n_bits - tb + hmax - 1) / hmax;
+    unsigned long long* tot = nullptr;                  // direct kernel, pass 0 with the histogram: per-call totals
     int done = 0;
     bool first = true;
     while (done < n_bits) {
         if (done == 0) { a.c = tb; a.h = 0; a.hi_pos = tb; a.f0 = 0; done = tb; }
         else {
-            int h = n_bits - done;
-            const int hmax = tb - seg_bits > 1 ? tb - seg_bits : (tb - 3 > 1 ? tb - 3 : 1);
-            if (h > hmax) h = hmax;
+            const int h = (n_bits - done + passes_left - 1) / passes_left;
+            passes_left--;
             a.h = h; a.c = tb - h; a.hi_pos = done; a.f0 = a.c; done += h;
         }
         gp_time_begin(GP_KERNEL_ROBUSTNESS, st);
@@ -609,12 +756,27 @@ static gp_status robustness_passes(const uint16_t* d_pheno, int n_bits, uint32_t
             b.pheno = a.pheno; b.n_bits = n_bits; b.C = n_classes; b.R = a.R; b.Dl = a.Dl; b.O = a.O;
             b.hist = first ? reinterpret_cast<unsigned long long*>(d_hist) : nullptr;
             b.bitmap = a.bitmap; b.tb = a.tb; b.c = a.c; b.h = a.h; b.hi_pos = a.hi_pos; b.f0 = a.f0;
-            if (d_pair_bitmap) robustness2_kernel<true><<<grid, R2THREADS, smem, st>>>(b);
-            else robustness2_kernel<false><<<grid, R2THREADS, smem, st>>>(b);
+            if (direct) {
+                if (b.hist) {
+                    GP_CUDA(cudaMallocAsync(&tot, 3 * (size_t)n_classes * sizeof(unsigned long long), st));
+                    GP_CUDA(cudaMemsetAsync(tot, 0, 3 * (size_t)n_classes * sizeof(unsigned long long), st));
+                    b.R = tot; b.Dl = tot + n_classes; b.O = tot + 2 * (size_t)n_classes;
+                }
+                if (d_pair_bitmap) robustness3_kernel<true><<<grid, R2THREADS, smem, st>>>(b);
+                else robustness3_kernel<false><<<grid, R2THREADS, smem, st>>>(b);
+                if (b.hist) {
+                    rob3_finish_kernel<<<(n_classes + 255) / 256, 256, 0, st>>>(tot, n_classes, (uint32_t)(b.tb - b.f0), a.R, a.Dl, a.O, b.hist);
+                    gp_count_launches(1);
+                }
+            } else {
+                if (d_pair_bitmap) robustness2_kernel<true><<<grid, R2THREADS, smem, st>>>(b);
+                else robustness2_kernel<false><<<grid, R2THREADS, smem, st>>>(b);
+            }
         }
         gp_time_end(GP_KERNEL_ROBUSTNESS, st);
         GP_CUDA(cudaGetLastError());
         gp_count_launches(1);
+        if (tot) { cudaFreeAsync(tot, st); tot = nullptr; }
         first = false;
     }
     return GP_OK;

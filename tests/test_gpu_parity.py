@@ -239,7 +239,7 @@ def test_enumerate_host_end_to_end(oracle_structures):
     assert gpmap.launch_count() > 0
 
 
-@pytest.mark.parametrize("tile_bits", [4, 7, 10, 15, 16])
+@pytest.mark.parametrize("tile_bits", [0, 4, 7, 10, 15, 16])
 def test_robustness_tile_sizes_agree_with_oracle(tile_bits):
     """The bit-tiled neighbour pass gives the same counts for every tile size (small tiles force the multi-pass,
     spread-bit path on small stores), on stores whose size is not a multiple of the pass width."""
@@ -270,6 +270,34 @@ def test_robustness_tile_sizes_agree_with_oracle(tile_bits):
     assert np.array_equal(hist.cpu().numpy().astype(np.uint64), orc.designability(store, C))
     assert np.array_equal(R.cpu().numpy().astype(np.uint64), Ro) and np.array_equal(Dl.cpu().numpy().astype(np.uint64), Do)
     assert np.array_equal(Oc.cpu().numpy().astype(np.uint64), Oo) and int(pc2) == pco
+
+
+@pytest.mark.parametrize("C,p_null", [(1, 0.0), (1, 0.5), (2, 0.1), (3, 0.9), (7, 0.36)])
+def test_neighbour_pass_on_stores_with_very_few_classes(C, p_null):
+    """Stores in which one class holds a large share of the genotypes: the packed per-class words of the direct-table
+    kernel wrap thousands of times and every wrap is booked through the carry path; the fused histogram comes from the
+    per-call totals.  Default tile size and the small-tile multi-pass path, with and without the pair bitmap."""
+    rng = np.random.default_rng(1000 + C)
+    n_bits = 20
+    n = 1 << n_bits
+    store = rng.integers(0, C, size=n).astype(np.uint16)
+    store[rng.random(n) < p_null] = 0xFFFF
+    Ro, Do, Oo, pco = orc.robustness(store, n_bits, C)
+    ph = torch.from_numpy(store.view(np.int16)).cuda().view(torch.uint16)
+    for tile_bits in (0, 12):
+        rdo = torch.zeros((3, C), dtype=torch.int64, device="cuda")
+        bitmap = gpmap.pair_bitmap(C)
+        gpmap.robustness_partial(ph, n_bits, C, rdo, bitmap, tile_bits=tile_bits)
+        got = rdo.cpu().numpy().astype(np.uint64)
+        assert np.array_equal(got[0], Ro) and np.array_equal(got[1], Do) and np.array_equal(got[2], Oo), tile_bits
+        assert int(gpmap.pair_bitmap_count(bitmap, C)) == pco
+        rdo2 = torch.zeros((3, C), dtype=torch.int64, device="cuda")
+        gpmap.robustness_partial(ph, n_bits, C, rdo2, None, tile_bits=tile_bits)
+        assert torch.equal(rdo, rdo2), tile_bits
+    hist, R, Dl, Oc, pc = gpmap.reduce_store(ph, n_bits, C)
+    assert np.array_equal(hist.cpu().numpy().astype(np.uint64), orc.designability(store, C))
+    assert np.array_equal(R.cpu().numpy().astype(np.uint64), Ro) and np.array_equal(Dl.cpu().numpy().astype(np.uint64), Do)
+    assert np.array_equal(Oc.cpu().numpy().astype(np.uint64), Oo) and int(pc) == pco
 
 
 @pytest.mark.parametrize("dims,k", [((2, 2, 1), 9), ((3, 3, 1), 9), ((4, 4, 1), 5), ((4, 4, 1), 6), ((4, 4, 1), 8),
