@@ -403,6 +403,15 @@ __global__ void __launch_bounds__(R2THREADS, 1) robustness3_kernel(Rob2Args a) {
             nulls += 8 - __popc(nb);
         }
         __syncthreads();
+        if (t + gridDim.x < n_tiles) {                              // the next tile of this block: pull it into L2 meanwhile
+            const uint64_t tn = t + gridDim.x;
+            const uint64_t bn = ((tn & ((1ULL << lo_outer) - 1ULL)) << a.c) | ((tn >> lo_outer) << (a.hi_pos + a.h));
+            const uint32_t step = a.c >= 6 ? 64u : (1u << a.c);     // genotypes per prefetch: a 128-byte line or one segment
+            for (uint32_t l = threadIdx.x * step; l < (1u << a.tb); l += R2THREADS * step) {
+                const uint64_t g = bn | (l & cmask) | ((uint64_t)(l >> a.c) << a.hi_pos);
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(a.pheno + g));
+            }
+        }
         for (uint32_t v0 = 0; v0 < n_vec; v0 += R2THREADS) {       // uniform trip count: the warp stays converged
             const uint32_t v = v0 + threadIdx.x;
             const bool live = v < n_vec;
