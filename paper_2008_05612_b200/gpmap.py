@@ -185,7 +185,7 @@ class Structures:
         self.K = L.gp_structures_features(h)
 
     def close(self):
-        if getattr(self, "_h", None):
+        if getattr(self, "_h", None) and lib is not None:   # at interpreter shutdown the module globals are already gone
             lib().gp_structures_free(self._h)
             self._h = None
 
