@@ -301,19 +301,35 @@ __device__ __forceinline__ uint32_t image_mid(const uint32_t* units, uint64_t un
     return (paired && (y & 1u)) ? (mid ? (__brev(m) >> (32 - mid)) : 0u) : m;
 }
 
-// One block = one 128-structure tile of IMG_PER_BLOCK consecutive images.  The tile's contact lists and the column
-// tables are staged in shared memory once (the tables are indexed by monomer, different in every thread: as kernel
-// parameters they would be serialised constant-bank reads).  Thread = structure: it accumulates its weight row in shared
-// memory (already in the swizzled layout the MMA reads), then the block writes the tile out coalesced.
-constexpr int IMG_PER_BLOCK = 4;
+// One block = one 128-structure tile of IMG_PER_BLOCK consecutive images; thread = structure = one weight row.
+// Only the first 2 + fb columns of a row depend on the image (the fixed monomers' letters G); the pair columns do not:
+//   bias          = lin * sum over fixed monomers j of h_j * deg(j)  +  quad * #(contacts between two fixed H monomers)
+//   column 2 + l  = lin * deg(l)  +  quad * popc(G & F_l),   F_l = the fixed monomers in contact with free monomer l
+// (deg = contacts of the monomer in this structure).  The block prepares, once, the image-independent part of the tile
+// in shared memory (already in the swizzled layout the MMA reads) and per thread deg, F_l, the degree bit-planes of the
+// fixed monomers and the list of fixed-fixed contacts; per image a thread then evaluates 2 + fb bytes with popc,
+// overwrites them in its row and its warp copies its 32 rows out, coalesced.  No barrier after the setup.
+constexpr int IMG_PER_BLOCK = 8;
 
 template <int RB>
-__global__ void __launch_bounds__(TN) build_image_kernel(const ImgArgs a, const Slots slots_in, uint32_t n_images) {
+__global__ void build_image_kernel(const ImgArgs a, const Slots slots_in, uint32_t n_images, int fb);
+
+template <int RB>
+size_t build_image_smem(int fb) {
+    return (size_t)TM * RB + TN * 64 + (size_t)fb * TN * 8 + (((size_t)fb * TN + 15) & ~(size_t)15) + 32 * TN * 2 + sizeof(Slots) + 16;
+}
+
+template <int RB>
+__global__ void __launch_bounds__(TN) build_image_kernel(const ImgArgs a, const Slots slots_in, uint32_t n_images, int fb) {
     constexpr int TB = TM * RB;
-    __shared__ __align__(16) int8_t tile[TB];
-    __shared__ __align__(16) uint8_t s_con[TN * 64];   // contacts of the tile's structures: NBP <= 32 pairs each
-    __shared__ Slots slots;
-    const uint32_t r = threadIdx.x, n = blockIdx.x;
+    extern __shared__ __align__(16) unsigned char img_smem[];
+    int8_t* tile = reinterpret_cast<int8_t*>(img_smem);
+    uint8_t* s_con = img_smem + TB;                          // contacts of the tile's structures: NBP <= 32 pairs each
+    uint64_t* maskF = reinterpret_cast<uint64_t*>(s_con + TN * 64);    // [fb][TN]
+    uint8_t* degL = reinterpret_cast<uint8_t*>(maskF + (size_t)fb * TN);   // [fb][TN]
+    uint16_t* ffl = reinterpret_cast<uint16_t*>(degL + (((size_t)fb * TN + 15) & ~(size_t)15));  // [32][TN]: i | j << 8
+    Slots* slots = reinterpret_cast<Slots*>(ffl + 32 * TN);
+    const uint32_t r = threadIdx.x, n = blockIdx.x, lane = r & 31u;
     const uint32_t d = n * TN + r;
     const int row = a.NBP * 2;
     {
@@ -321,44 +337,67 @@ __global__ void __launch_bounds__(TN) build_image_kernel(const ImgArgs a, const 
         const uint8_t* src = a.contacts + (size_t)first * row;
         for (uint32_t i = threadIdx.x; i < cnt; i += TN) s_con[i] = src[i];
         for (uint32_t i = threadIdx.x; i < sizeof(Slots); i += TN)
-            reinterpret_cast<uint8_t*>(&slots)[i] = reinterpret_cast<const uint8_t*>(&slots_in)[i];
-    }
-    const bool real = d < a.D && a.class_of[d] != GP_NULL_PHENO;
-    const uint8_t* c = s_con + r * row;
-    for (uint32_t y = blockIdx.y * IMG_PER_BLOCK; y < n_images && y < (blockIdx.y + 1) * IMG_PER_BLOCK; y++) {
-        const uint64_t G = (a.units ? (uint64_t)image_mid(a.units, a.unit_first, a.paired, a.mid, y) : a.gfix_first + y) << a.gfix_shift;
-        __syncthreads();   // staging done / previous tile written out
+            reinterpret_cast<uint8_t*>(slots)[i] = reinterpret_cast<const uint8_t*>(&slots_in)[i];
         for (uint32_t i = threadIdx.x; i < TB / 16; i += TN) reinterpret_cast<uint4*>(tile)[i] = make_uint4(0, 0, 0, 0);
-        __syncthreads();
-        if (real) {
-            int bias = 0;
-            for (int k = 0; k < a.NBP; k++) {
-                const int i = c[2 * k], j = c[2 * k + 1];  // i < j
-                const int li = slots.loc[i], lj = slots.loc[j];
-                const int hi = (int)((G >> i) & 1ULL), hj = (int)((G >> j) & 1ULL);
-                if (li >= 0 && lj >= 0) {
-                    tile[swz_rb<RB>(r, 2 + li)] += (int8_t)a.lin;
-                    tile[swz_rb<RB>(r, 2 + lj)] += (int8_t)a.lin;
-                    tile[swz_rb<RB>(r, slots.pair[li * MAX_FB + lj])] = (int8_t)a.quad;
-                } else if (li >= 0) {
-                    tile[swz_rb<RB>(r, 2 + li)] += (int8_t)(a.lin + a.quad * hj);
-                    bias += a.lin * hj;
-                } else if (lj >= 0) {
-                    tile[swz_rb<RB>(r, 2 + lj)] += (int8_t)(a.lin + a.quad * hi);
-                    bias += a.lin * hi;
-                } else {
-                    bias += a.lin * (hi + hj) + a.quad * hi * hj;
-                }
-            }
-            tile[swz_rb<RB>(r, 0)] = (int8_t)(bias >> 6);   // x 64
-            tile[swz_rb<RB>(r, 1)] = (int8_t)(bias & 63);   // x 1
-        } else {                                     // pad structure: energy E_PAD for every genotype
-            tile[swz_rb<RB>(r, 0)] = 127;
-            tile[swz_rb<RB>(r, 1)] = 63;
+        for (int l = 0; l < fb; l++) { maskF[l * TN + r] = 0; degL[l * TN + r] = 0; }
+    }
+    __syncthreads();
+    const bool real = d < a.D && a.class_of[d] != GP_NULL_PHENO;
+    uint64_t dm0 = 0, dm1 = 0, dm2 = 0;     // bit-planes of deg(j) over the fixed monomers j (bit j - gfix_shift)
+    int nff = 0;
+    if (real) {
+        const uint8_t* c = s_con + r * row;
+        for (int k = 0; k < a.NBP; k++) {
+            const int i = c[2 * k], j = c[2 * k + 1];  // i < j
+            const int li = slots->loc[i], lj = slots->loc[j];
+            const uint64_t bi = 1ULL << ((i - a.gfix_shift) & 63), bj = 1ULL << ((j - a.gfix_shift) & 63);
+            if (li >= 0) degL[li * TN + r]++;
+            else { const uint64_t c0 = dm0 & bi; dm0 ^= bi; const uint64_t c1 = dm1 & c0; dm1 ^= c0; dm2 ^= c1; }
+            if (lj >= 0) degL[lj * TN + r]++;
+            else { const uint64_t c0 = dm0 & bj; dm0 ^= bj; const uint64_t c1 = dm1 & c0; dm1 ^= c0; dm2 ^= c1; }
+            if (li >= 0 && lj >= 0) tile[swz_rb<RB>(r, slots->pair[li * MAX_FB + lj])] = (int8_t)a.quad;
+            else if (li >= 0) maskF[li * TN + r] |= bj;
+            else if (lj >= 0) maskF[lj * TN + r] |= bi;
+            else ffl[(nff++) * TN + r] = (uint16_t)(((i - a.gfix_shift) & 63) | (((j - a.gfix_shift) & 63) << 8));
         }
-        __syncthreads();
-        uint4* dst = reinterpret_cast<uint4*>(a.img + ((uint64_t)y * a.n_tiles + n) * TB);
-        for (uint32_t i = threadIdx.x; i < TB / 16; i += TN) dst[i] = reinterpret_cast<const uint4*>(tile)[i];
+    } else {                                         // pad structure: energy E_PAD for every genotype
+        tile[swz_rb<RB>(r, 0)] = 127;
+        tile[swz_rb<RB>(r, 1)] = 63;
+    }
+    const int ncol = 2 + fb, nw = (ncol + 3) >> 2;   // image-dependent columns / the 32-bit words that hold them
+    // the last of those words may also hold pair columns: keep its image-independent bytes
+    const uint32_t last_base = *reinterpret_cast<const uint32_t*>(tile + swz_rb<RB>(r, 4 * (nw - 1)));
+    const uint32_t* trow = reinterpret_cast<const uint32_t*>(tile);
+    for (uint32_t y = blockIdx.y * IMG_PER_BLOCK; y < n_images && y < (blockIdx.y + 1) * IMG_PER_BLOCK; y++) {
+        const uint64_t G = a.units ? (uint64_t)image_mid(a.units, a.unit_first, a.paired, a.mid, y) : a.gfix_first + y;
+        if (real) {
+            int bias = a.lin * (__popcll(G & dm0) + 2 * __popcll(G & dm1) + 4 * __popcll(G & dm2));
+            for (int k = 0; k < nff; k++) {
+                const uint32_t e = ffl[k * TN + r];
+                bias += a.quad * (int)((G >> (e & 255u)) & (G >> (e >> 8)) & 1ULL);
+            }
+            for (int w = 0; w < nw; w++) {
+                uint32_t x = w == nw - 1 ? last_base : 0u;
+#pragma unroll
+                for (int b = 0; b < 4; b++) {
+                    const int col = 4 * w + b;
+                    if (col >= ncol) break;
+                    int v;
+                    if (col == 0) v = bias >> 6;          // x 64
+                    else if (col == 1) v = bias & 63;     // x 1
+                    else v = a.lin * (int)degL[(col - 2) * TN + r] + a.quad * __popcll(G & maskF[(col - 2) * TN + r]);
+                    x = (x & ~(0xFFu << (8 * b))) | (((uint32_t)v & 0xFFu) << (8 * b));
+                }
+                *reinterpret_cast<uint32_t*>(tile + swz_rb<RB>(r, 4 * w)) = x;
+            }
+        }
+        __syncwarp();
+        // rows 32 * warp .. + 31 are contiguous in the tile and in the image
+        uint4* dst = reinterpret_cast<uint4*>(a.img + ((uint64_t)y * a.n_tiles + n) * TB) + (r & ~31u) * (RB / 16);
+        const uint4* srcw = reinterpret_cast<const uint4*>(trow) + (r & ~31u) * (RB / 16);
+#pragma unroll
+        for (uint32_t i = 0; i < RB / 16; i++) dst[i * 32 + lane] = srcw[i * 32 + lane];
+        __syncwarp();
     }
 }
 
@@ -817,6 +856,8 @@ gp_status gp_launch_scoring_tc(const gp_structures_s* s, const gp_hp_params& hp,
         gp_status ps = pipe.open(st);
         if (ps != GP_OK) { cudaFreeAsync(d_img0, st); return ps; }
     }
+    if (p.narrow) GP_CUDA(cudaFuncSetAttribute(build_image_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)build_image_smem<64>(fb)));
+    else GP_CUDA(cudaFuncSetAttribute(build_image_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)build_image_smem<128>(fb)));
     uint64_t g = g_begin & ~(uint64_t)(SUPER - 1);  // g_begin is a multiple of gp_tile() = SUPER already
     gp_status result = GP_OK;
     for (uint64_t grp = 0; g < g_end; grp++) {
@@ -831,8 +872,8 @@ gp_status gp_launch_scoring_tc(const gp_structures_s* s, const gp_hp_params& hp,
         ia.NBP = s->NBP; ia.lin = hp.lin; ia.quad = hp.quad;
         pipe.before_build(grp);
         gp_time_begin(GP_KERNEL_IMAGE, pipe.side);
-        if (p.narrow) build_image_kernel<64><<<dim3(p.n_tiles, (n_batches + IMG_PER_BLOCK - 1) / IMG_PER_BLOCK), TN, 0, pipe.side>>>(ia, p.slots, n_batches);
-        else build_image_kernel<128><<<dim3(p.n_tiles, (n_batches + IMG_PER_BLOCK - 1) / IMG_PER_BLOCK), TN, 0, pipe.side>>>(ia, p.slots, n_batches);
+        if (p.narrow) build_image_kernel<64><<<dim3(p.n_tiles, (n_batches + IMG_PER_BLOCK - 1) / IMG_PER_BLOCK), TN, build_image_smem<64>(fb), pipe.side>>>(ia, p.slots, n_batches, fb);
+        else build_image_kernel<128><<<dim3(p.n_tiles, (n_batches + IMG_PER_BLOCK - 1) / IMG_PER_BLOCK), TN, build_image_smem<128>(fb), pipe.side>>>(ia, p.slots, n_batches, fb);
         gp_time_end(GP_KERNEL_IMAGE, pipe.side);
         pipe.after_build(grp, st);
         Args a;
@@ -934,6 +975,8 @@ static gp_status gp_launch_map_range(const gp_structures_s* s, const gp_hp_param
         gp_status ps = pipe.open(st);
         if (ps != GP_OK) { cudaFreeAsync(d_work, st); return ps; }
     }
+    if (p.narrow) GP_CUDA(cudaFuncSetAttribute(build_image_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)build_image_smem<64>(fb)));
+    else GP_CUDA(cudaFuncSetAttribute(build_image_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)build_image_smem<128>(fb)));
     gp_status result = GP_OK;
     uint64_t u = u_first, images_done = 0;
     const uint64_t u_end = u_first + u_count;
@@ -950,8 +993,8 @@ static gp_status gp_launch_map_range(const gp_structures_s* s, const gp_hp_param
         ia.n_tiles = p.n_tiles; ia.NBP = s->NBP; ia.lin = hp.lin; ia.quad = hp.quad;
         pipe.before_build(grp);
         gp_time_begin(GP_KERNEL_IMAGE, pipe.side);
-        if (p.narrow) build_image_kernel<64><<<dim3(p.n_tiles, (n_img + IMG_PER_BLOCK - 1) / IMG_PER_BLOCK), TN, 0, pipe.side>>>(ia, p.slots, n_img);
-        else build_image_kernel<128><<<dim3(p.n_tiles, (n_img + IMG_PER_BLOCK - 1) / IMG_PER_BLOCK), TN, 0, pipe.side>>>(ia, p.slots, n_img);
+        if (p.narrow) build_image_kernel<64><<<dim3(p.n_tiles, (n_img + IMG_PER_BLOCK - 1) / IMG_PER_BLOCK), TN, build_image_smem<64>(fb), pipe.side>>>(ia, p.slots, n_img, fb);
+        else build_image_kernel<128><<<dim3(p.n_tiles, (n_img + IMG_PER_BLOCK - 1) / IMG_PER_BLOCK), TN, build_image_smem<128>(fb), pipe.side>>>(ia, p.slots, n_img, fb);
         gp_time_end(GP_KERNEL_IMAGE, pipe.side);
         pipe.after_build(grp, st);
         Args a;
