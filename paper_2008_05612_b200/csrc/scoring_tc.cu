@@ -309,7 +309,7 @@ __device__ __forceinline__ uint32_t image_mid(const uint32_t* units, uint64_t un
 // in shared memory (already in the swizzled layout the MMA reads) and per thread deg, F_l, the degree bit-planes of the
 // fixed monomers and the list of fixed-fixed contacts; per image a thread then evaluates 2 + fb bytes with popc,
 // overwrites them in its row and its warp copies its 32 rows out, coalesced.  No barrier after the setup.
-constexpr int IMG_PER_BLOCK = 8;
+constexpr int IMG_PER_BLOCK = 32;
 
 template <int RB>
 __global__ void build_image_kernel(const ImgArgs a, const Slots slots_in, uint32_t n_images, int fb);
@@ -376,7 +376,9 @@ __global__ void __launch_bounds__(TN) build_image_kernel(const ImgArgs a, const 
                 const uint32_t e = ffl[k * TN + r];
                 bias += a.quad * (int)((G >> (e & 255u)) & (G >> (e >> 8)) & 1ULL);
             }
-            for (int w = 0; w < nw; w++) {
+#pragma unroll
+            for (int w = 0; w < (2 + MAX_FB + 3) / 4; w++) {
+                if (w >= nw) break;
                 uint32_t x = w == nw - 1 ? last_base : 0u;
 #pragma unroll
                 for (int b = 0; b < 4; b++) {
@@ -830,6 +832,20 @@ struct ImagePipeline {
     }
 };
 
+// Images per launch: the largest count under `cap` whose supertiles fill whole rounds of the persistent grid best
+// (a launch of 59.3 rounds costs 60); `step` keeps pairs of images together on the map path.
+static size_t tc_group_size(size_t cap, size_t step, uint64_t items_per_image, int sms) {
+    if (cap < step) return step;
+    size_t best = cap - cap % step;
+    double best_eff = 0.0;
+    for (size_t g = cap - cap % step; g >= step && g * 4 >= cap * 3; g -= step) {
+        const uint64_t items = g * items_per_image, rounds = (items + sms - 1) / sms;
+        const double eff = (double)items / (double)(rounds * sms);
+        if (eff > best_eff + 1e-9) { best_eff = eff; best = g; }
+    }
+    return best;
+}
+
 gp_status gp_launch_scoring_tc(const gp_structures_s* s, const gp_hp_params& hp, uint64_t g_begin, uint64_t g_count,
                                uint16_t* d_pheno, int16_t* d_gap, cudaStream_t st) {
     using namespace tc;
@@ -844,9 +860,10 @@ gp_status gp_launch_scoring_tc(const gp_structures_s* s, const gp_hp_params& hp,
 
     // batches of 2^fb genotypes share a weight image; a launch covers up to `group` batches
     const uint64_t g_end = g_begin + g_count;
-    uint64_t group = (512ULL << 20) / p.img_bytes;  // two buffers of <= 512 MB of images: one is built while the other is scored
+    uint64_t group = (640ULL << 20) / p.img_bytes;  // two buffers of <= 640 MB of images: one is built while the other is scored
     if (group < 1) group = 1;
     if (group > 256) group = 256;
+    group = tc_group_size((size_t)group, 1, ((1ULL << fb) + SUPER - 1) / SUPER, p.sms);
     const uint64_t n_batches_all = ((g_end - 1) >> fb) - (g_begin >> fb) + 1;
     if (group > n_batches_all) group = n_batches_all;
     int8_t* d_img0 = nullptr;  // per-call working memory from the stream-ordered pool: calls on other streams have their own
@@ -958,9 +975,9 @@ static gp_status gp_launch_map_range(const gp_structures_s* s, const gp_hp_param
     gp_status stt = make_plan(s, mon, fb, s->D_sym, p);
     if (stt != GP_OK) return stt;
     const size_t rec_bytes = sizeof(int4) << fb;
-    size_t group = (1024ULL << 20) / (2 * p.img_bytes + rec_bytes);  // <= 1 GB: two image buffers + one record buffer
+    size_t group = (1280ULL << 20) / (2 * p.img_bytes + rec_bytes);  // <= 1.25 GB: two image buffers + one record buffer
     if (group > 512) group = 512;
-    group &= ~(size_t)1;
+    group = tc_group_size(group, 2, ((1ULL << fb) + SUPER - 1) / SUPER, p.sms);
     if (group < 2) group = 2;
     {   // never more than the range needs
         const uint64_t pairs = u_first < s->n_pair_units ? (u_first + u_count < s->n_pair_units ? u_count : s->n_pair_units - u_first) : 0;
