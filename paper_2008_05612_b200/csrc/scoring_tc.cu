@@ -808,9 +808,9 @@ gp_status make_plan(const gp_structures_s* s, const int* mon, int fb, uint32_t n
 // Weight images of launch group g + 1 are built on a side stream while the scoring kernel of group g runs on the caller's
 // stream (two image buffers); events tie the side stream in, so that to the caller everything is ordered on `st`.
 struct ImagePipeline {
-    cudaStream_t side = nullptr;
-    cudaEvent_t built[2] = {nullptr, nullptr}, freed[2] = {nullptr, nullptr}, start = nullptr;
-    gp_status open(cudaStream_t st) {   // call after the buffers were allocated on st
+    cudaStream_t side = nullptr, post = nullptr;   // post (map path): the combine of group g runs beside the scoring of g + 1
+    cudaEvent_t built[2] = {nullptr, nullptr}, freed[2] = {nullptr, nullptr}, posted[2] = {nullptr, nullptr}, start = nullptr;
+    gp_status open(cudaStream_t st, bool with_post = false) {   // call after the buffers were allocated on st
         GP_CUDA(cudaStreamCreateWithFlags(&side, cudaStreamNonBlocking));
         GP_CUDA(cudaEventCreateWithFlags(&start, cudaEventDisableTiming));
         for (int b = 0; b < 2; b++) {
@@ -819,7 +819,22 @@ struct ImagePipeline {
         }
         GP_CUDA(cudaEventRecord(start, st));
         GP_CUDA(cudaStreamWaitEvent(side, start, 0));
+        if (with_post) {
+            GP_CUDA(cudaStreamCreateWithFlags(&post, cudaStreamNonBlocking));
+            for (int b = 0; b < 2; b++) GP_CUDA(cudaEventCreateWithFlags(&posted[b], cudaEventDisableTiming));
+            GP_CUDA(cudaStreamWaitEvent(post, start, 0));
+        }
         return GP_OK;
+    }
+    // record buffer g & 1 may be overwritten by scoring launch g once the combine of group g - 2 has read it
+    void before_scoring(uint64_t g, cudaStream_t st) { if (post && g >= 2) cudaStreamWaitEvent(st, posted[g & 1], 0); }
+    // the stream the combine of group g goes to (after after_scoring(g)): it waits for that scoring launch
+    cudaStream_t post_stream(uint64_t g) { cudaStreamWaitEvent(post, freed[g & 1], 0); return post; }
+    void after_post(uint64_t g) { cudaEventRecord(posted[g & 1], post); }
+    // the caller's stream continues only after every combine (n_groups launched)
+    void join_post(uint64_t n_groups, cudaStream_t st) {
+        if (!post) return;
+        for (uint64_t g = n_groups >= 2 ? n_groups - 2 : 0; g < n_groups; g++) cudaStreamWaitEvent(st, posted[g & 1], 0);
     }
     // side stream may overwrite buffer b once the scoring launch that read it (two groups ago) is done
     void before_build(uint64_t g) { if (g >= 2) cudaStreamWaitEvent(side, freed[g & 1], 0); }
@@ -827,8 +842,10 @@ struct ImagePipeline {
     void after_scoring(uint64_t g, cudaStream_t st) { cudaEventRecord(freed[g & 1], st); }
     ~ImagePipeline() {   // destroying a stream / event with work pending is deferred by the runtime
         for (int b = 0; b < 2; b++) { if (built[b]) cudaEventDestroy(built[b]); if (freed[b]) cudaEventDestroy(freed[b]); }
+        for (int b = 0; b < 2; b++) if (posted[b]) cudaEventDestroy(posted[b]);
         if (start) cudaEventDestroy(start);
         if (side) cudaStreamDestroy(side);
+        if (post) cudaStreamDestroy(post);
     }
 };
 
@@ -975,7 +992,7 @@ static gp_status gp_launch_map_range(const gp_structures_s* s, const gp_hp_param
     gp_status stt = make_plan(s, mon, fb, s->D_sym, p);
     if (stt != GP_OK) return stt;
     const size_t rec_bytes = sizeof(int4) << fb;
-    size_t group = (1280ULL << 20) / (2 * p.img_bytes + rec_bytes);  // <= 1.25 GB: two image buffers + one record buffer
+    size_t group = (1280ULL << 20) / (2 * p.img_bytes + 2 * rec_bytes);  // <= 1.25 GB: two image buffers + two record buffers
     if (group > 512) group = 512;
     group = tc_group_size(group, 2, ((1ULL << fb) + SUPER - 1) / SUPER, p.sms);
     if (group < 2) group = 2;
@@ -985,17 +1002,17 @@ static gp_status gp_launch_map_range(const gp_structures_s* s, const gp_hp_param
         if (group > most) group = (size_t)((most + 1) & ~1ULL);
     }
     char* d_work = nullptr;
-    GP_CUDA(cudaMallocAsync(&d_work, (2 * p.img_bytes + rec_bytes) * group, st));
-    int4* d_rec = (int4*)(d_work + 2 * p.img_bytes * group);
+    GP_CUDA(cudaMallocAsync(&d_work, (2 * p.img_bytes + 2 * rec_bytes) * group, st));
+    int4* d_rec0 = (int4*)(d_work + 2 * p.img_bytes * group);
     ImagePipeline pipe;
     {
-        gp_status ps = pipe.open(st);
+        gp_status ps = pipe.open(st, true);
         if (ps != GP_OK) { cudaFreeAsync(d_work, st); return ps; }
     }
     if (p.narrow) GP_CUDA(cudaFuncSetAttribute(build_image_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)build_image_smem<64>(fb)));
     else GP_CUDA(cudaFuncSetAttribute(build_image_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)build_image_smem<128>(fb)));
     gp_status result = GP_OK;
-    uint64_t u = u_first, images_done = 0;
+    uint64_t u = u_first, images_done = 0, n_groups = 0;
     const uint64_t u_end = u_first + u_count;
     for (uint64_t grp = 0; u < u_end; grp++) {
         int8_t* d_img = (int8_t*)d_work + (grp & 1) * p.img_bytes * group;
@@ -1019,8 +1036,10 @@ static gp_status gp_launch_map_range(const gp_structures_s* s, const gp_hp_param
         a.g_first = 0; a.g_end = (uint64_t)n_img << fb; a.out_base = 0;
         a.n_items = (uint32_t)((a.g_end + SUPER - 1) / SUPER);
         a.n_tiles = p.n_tiles; a.D = s->D_sym; a.fb = fb; a.k_steps = p.k_steps; a.threshold = hp.threshold;
+        int4* d_rec = d_rec0 + (grp & 1) * (group << fb);
         a.hrec = d_rec; a.n_snap = s->n_snap;
         const unsigned grid = a.n_items < (uint32_t)p.sms ? a.n_items : (uint32_t)p.sms;
+        pipe.before_scoring(grp, st);
         gp_time_begin(GP_KERNEL_SCORING, st);
         p.kernel<<<grid, p.threads, p.smem, st>>>(a, p.cols);
         gp_time_end(GP_KERNEL_SCORING, st);
@@ -1031,12 +1050,15 @@ static gp_status gp_launch_map_range(const gp_structures_s* s, const gp_hp_param
         ca.fb = fb; ca.k = k; ca.N = N; ca.threshold = hp.threshold; ca.compact = compact; ca.compact_base = images_done << fb;
         images_done += n_img;
         const uint64_t work = ((uint64_t)n_img << fb) / 256;
-        combine_kernel<<<(unsigned)(work < (uint64_t)p.sms * 8 ? (work ? work : 1) : (uint64_t)p.sms * 8), 256, 0, st>>>(ca);
+        combine_kernel<<<(unsigned)(work < (uint64_t)p.sms * 8 ? (work ? work : 1) : (uint64_t)p.sms * 8), 256, 0, pipe.post_stream(grp)>>>(ca);
+        pipe.after_post(grp);
+        n_groups = grp + 1;
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) { gp_set_cuda_error(e, "map launch"); result = GP_CUDA_ERROR; break; }
         gp_count_launches(3);
         u = stop;
     }
+    pipe.join_post(n_groups, st);
     cudaFreeAsync(d_work, st);
     return result;
 }
