@@ -809,6 +809,8 @@ gp_status make_plan(const gp_structures_s* s, const int* mon, int fb, uint32_t n
 // stream (two image buffers); events tie the side stream in, so that to the caller everything is ordered on `st`.
 struct ImagePipeline {
     cudaStream_t side = nullptr, post = nullptr;   // post (map path): the combine of group g runs beside the scoring of g + 1
+    cudaStream_t alt = nullptr;   // map path: odd scoring launches go here, so the blocks of launch g + 1 take over the SMs
+                                  // one by one as the blocks of launch g retire (no idle tail at the end of a launch)
     cudaEvent_t built[2] = {nullptr, nullptr}, freed[2] = {nullptr, nullptr}, posted[2] = {nullptr, nullptr}, start = nullptr;
     gp_status open(cudaStream_t st, bool with_post = false) {   // call after the buffers were allocated on st
         GP_CUDA(cudaStreamCreateWithFlags(&side, cudaStreamNonBlocking));
@@ -821,11 +823,14 @@ struct ImagePipeline {
         GP_CUDA(cudaStreamWaitEvent(side, start, 0));
         if (with_post) {
             GP_CUDA(cudaStreamCreateWithFlags(&post, cudaStreamNonBlocking));
+            GP_CUDA(cudaStreamCreateWithFlags(&alt, cudaStreamNonBlocking));
             for (int b = 0; b < 2; b++) GP_CUDA(cudaEventCreateWithFlags(&posted[b], cudaEventDisableTiming));
             GP_CUDA(cudaStreamWaitEvent(post, start, 0));
+            GP_CUDA(cudaStreamWaitEvent(alt, start, 0));
         }
         return GP_OK;
     }
+    cudaStream_t scoring_stream(uint64_t g, cudaStream_t st) { return alt && (g & 1) ? alt : st; }
     // record buffer g & 1 may be overwritten by scoring launch g once the combine of group g - 2 has read it
     void before_scoring(uint64_t g, cudaStream_t st) { if (post && g >= 2) cudaStreamWaitEvent(st, posted[g & 1], 0); }
     // the stream the combine of group g goes to (after after_scoring(g)): it waits for that scoring launch
@@ -846,6 +851,7 @@ struct ImagePipeline {
         if (start) cudaEventDestroy(start);
         if (side) cudaStreamDestroy(side);
         if (post) cudaStreamDestroy(post);
+        if (alt) cudaStreamDestroy(alt);
     }
 };
 
@@ -1030,7 +1036,8 @@ static gp_status gp_launch_map_range(const gp_structures_s* s, const gp_hp_param
         if (p.narrow) build_image_kernel<64><<<dim3(p.n_tiles, (n_img + IMG_PER_BLOCK - 1) / IMG_PER_BLOCK), TN, build_image_smem<64>(fb), pipe.side>>>(ia, p.slots, n_img, fb);
         else build_image_kernel<128><<<dim3(p.n_tiles, (n_img + IMG_PER_BLOCK - 1) / IMG_PER_BLOCK), TN, build_image_smem<128>(fb), pipe.side>>>(ia, p.slots, n_img, fb);
         gp_time_end(GP_KERNEL_IMAGE, pipe.side);
-        pipe.after_build(grp, st);
+        cudaStream_t sg = pipe.scoring_stream(grp, st);
+        pipe.after_build(grp, sg);
         Args a;
         a.img = d_img; a.class_of = s->d_class_sym; a.pheno = nullptr; a.gap = nullptr;
         a.g_first = 0; a.g_end = (uint64_t)n_img << fb; a.out_base = 0;
@@ -1039,11 +1046,11 @@ static gp_status gp_launch_map_range(const gp_structures_s* s, const gp_hp_param
         int4* d_rec = d_rec0 + (grp & 1) * (group << fb);
         a.hrec = d_rec; a.n_snap = s->n_snap;
         const unsigned grid = a.n_items < (uint32_t)p.sms ? a.n_items : (uint32_t)p.sms;
-        pipe.before_scoring(grp, st);
-        gp_time_begin(GP_KERNEL_SCORING, st);
-        p.kernel<<<grid, p.threads, p.smem, st>>>(a, p.cols);
-        gp_time_end(GP_KERNEL_SCORING, st);
-        pipe.after_scoring(grp, st);
+        pipe.before_scoring(grp, sg);
+        gp_time_begin(GP_KERNEL_SCORING, sg);
+        p.kernel<<<grid, p.threads, p.smem, sg>>>(a, p.cols);
+        gp_time_end(GP_KERNEL_SCORING, sg);
+        pipe.after_scoring(grp, sg);
         CombArgs ca;
         ca.hrec = d_rec; ca.units = s->d_units; ca.class_sym = s->d_class_sym;
         ca.pheno = d_pheno; ca.gap = d_gap; ca.unit_first = u; ca.n_images = n_img; ca.paired = paired; ca.mid = mid;
