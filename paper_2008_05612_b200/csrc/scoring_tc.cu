@@ -834,8 +834,12 @@ struct ImagePipeline {
     // record buffer g & 1 may be overwritten by scoring launch g once the combine of group g - 2 has read it
     void before_scoring(uint64_t g, cudaStream_t st) { if (post && g >= 2) cudaStreamWaitEvent(st, posted[g & 1], 0); }
     // the stream the combine of group g goes to (after after_scoring(g)): it waits for that scoring launch
-    cudaStream_t post_stream(uint64_t g) { cudaStreamWaitEvent(post, freed[g & 1], 0); return post; }
-    void after_post(uint64_t g) { cudaEventRecord(posted[g & 1], post); }
+    cudaStream_t post_stream(uint64_t g, cudaStream_t st) {
+        if (!post) return st;
+        cudaStreamWaitEvent(post, freed[g & 1], 0);
+        return post;
+    }
+    void after_post(uint64_t g) { if (post) cudaEventRecord(posted[g & 1], post); }
     // the caller's stream continues only after every combine (n_groups launched)
     void join_post(uint64_t n_groups, cudaStream_t st) {
         if (!post) return;
@@ -1012,7 +1016,7 @@ static gp_status gp_launch_map_range(const gp_structures_s* s, const gp_hp_param
     int4* d_rec0 = (int4*)(d_work + 2 * p.img_bytes * group);
     ImagePipeline pipe;
     {
-        gp_status ps = pipe.open(st, true);
+        gp_status ps = pipe.open(st, u_count >= 1024);   // small ranges: a few launches, not worth two more streams
         if (ps != GP_OK) { cudaFreeAsync(d_work, st); return ps; }
     }
     if (p.narrow) GP_CUDA(cudaFuncSetAttribute(build_image_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)build_image_smem<64>(fb)));
@@ -1057,7 +1061,7 @@ static gp_status gp_launch_map_range(const gp_structures_s* s, const gp_hp_param
         ca.fb = fb; ca.k = k; ca.N = N; ca.threshold = hp.threshold; ca.compact = compact; ca.compact_base = images_done << fb;
         images_done += n_img;
         const uint64_t work = ((uint64_t)n_img << fb) / 256;
-        combine_kernel<<<(unsigned)(work < (uint64_t)p.sms * 8 ? (work ? work : 1) : (uint64_t)p.sms * 8), 256, 0, pipe.post_stream(grp)>>>(ca);
+        combine_kernel<<<(unsigned)(work < (uint64_t)p.sms * 8 ? (work ? work : 1) : (uint64_t)p.sms * 8), 256, 0, pipe.post_stream(grp, st)>>>(ca);
         pipe.after_post(grp);
         n_groups = grp + 1;
         cudaError_t e = cudaGetLastError();
