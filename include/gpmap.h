@@ -42,7 +42,8 @@ typedef enum {
     GP_UNSUPPORTED_LATTICE = 2, /* box with fewer than 2 or more than 64 sites, or more classes than a u16 holds */
     GP_OUT_OF_MEMORY = 3,
     GP_CUDA_ERROR = 4,          /* gp_last_cuda_error() has the CUDA text */
-    GP_RANGE = 5                /* genotype range outside [0, 2^N) or not aligned to gp_tile() */
+    GP_RANGE = 5,               /* genotype range outside [0, 2^N) or not aligned to gp_tile() */
+    GP_TOO_LARGE = 6            /* problem exceeds the fixed scratch array of an entry point that never allocates */
 } gp_status;
 
 typedef struct gp_structures_s gp_structures_t; /* opaque */
@@ -212,6 +213,30 @@ gp_status gp_phi_row(const uint16_t* d_pheno, int n_bits, uint32_t n_classes, ui
 gp_status gp_threshold_sweep(const uint16_t* d_pheno, const int16_t* d_gap, uint64_t count, uint32_t n_classes,
                              const int32_t* thresholds, int n_thresholds, uint64_t* d_folding, uint64_t* d_hist,
                              void* stream);
+
+/* f4 without any allocation: gp_threshold_sweep for callers that must not, or cannot, allocate device memory while
+ * they run.  Who that is: a service that hands its whole device-memory budget out at start-up and treats any later
+ * cudaMalloc / cudaMallocAsync as a fault; code running under a memory pool that has been capped or switched off;
+ * a latency-critical loop where an allocator call (which may take a driver lock or synchronise) is not acceptable.
+ * gp_threshold_sweep needs a per-call table of (n_thresholds + 1) * n_classes 64-bit counters and takes it from the
+ * stream-ordered pool; this entry point keeps that table in a fixed array that is part of the library image instead.
+ *   Same arguments, same results and same asynchrony as gp_threshold_sweep.  The caller still owns every input and
+ *   output (d_pheno, d_gap, d_folding, d_hist are device arrays, thresholds a host array).
+ *   Limit: (n_thresholds + 1) * n_classes <= GP_SWEEP_STATIC_MAX_BINS (2^19 counters = 4 MiB; enough for 16
+ *   thresholds on the 6x6 map's 28 728 classes, or 9 on the 3x3x3 map's 51 704).  Anything larger is refused with
+ *   GP_TOO_LARGE and nothing is launched.  The 4 MiB are held on every GPU on which this process loads the library's
+ *   device code, from that load until the process exits, whether or not this call is ever made.
+ *   Set-up: the first call on each device (with that device current) looks up the device address of the array and
+ *   keeps it; make that first call outside any stream capture.  Later calls on that device do no set-up.
+ *   It calls no cudaMalloc, cudaMallocAsync, cudaFree or other allocating routine; the table is cleared on `stream`
+ *   at the start of every call, so what an earlier call left behind never shows.
+ *   All calls in a process share the one array of a device: two calls whose GPU work can overlap (different streams,
+ *   or different host threads on different streams) race on it and give wrong counts.  Keep them on one stream, or
+ *   order them with events. */
+#define GP_SWEEP_STATIC_MAX_BINS (1u << 19)
+gp_status gp_threshold_sweep_static(const uint16_t* d_pheno, const int16_t* d_gap, uint64_t count, uint32_t n_classes,
+                                    const int32_t* thresholds, int n_thresholds, uint64_t* d_folding, uint64_t* d_hist,
+                                    void* stream);
 
 /* a7. Neutral-network components (:19, R12): d_ncomp[p] = number of connected components of {g : pheno = p} under
  * single-bit flips.  Needs 4 bytes of private scratch per genotype; n_bits <= 30.  Synchronises the stream. */

@@ -75,6 +75,7 @@ extern "C" const char* gp_strerror(gp_status st) {
         case GP_OUT_OF_MEMORY: return "out of memory";
         case GP_CUDA_ERROR: return "CUDA error (see gp_last_cuda_error)";
         case GP_RANGE: return "genotype range or index out of range / misaligned";
+        case GP_TOO_LARGE: return "problem larger than the fixed scratch array of this no-allocation entry point";
     }
     return "unknown status";
 }

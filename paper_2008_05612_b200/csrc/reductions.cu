@@ -946,3 +946,112 @@ extern "C" gp_status gp_nn_components(const uint16_t* d_pheno, int n_bits, uint3
     GP_CUDA(cudaStreamSynchronize(st));
     return GP_OK;
 }
+
+// ---------------------------------------------------------------------------------------------------------------
+// gp_threshold_sweep_static (gpmap.h): the threshold sweep for callers that may not allocate device memory at run
+// time — a process that gave its whole memory budget away at start-up, one whose pool is capped or disabled, a loop
+// that cannot afford an allocator call.  The counter table that gp_threshold_sweep takes from the stream-ordered pool
+// lives here in a file-scope device array of GP_SWEEP_STATIC_MAX_BINS counters (4 MiB, resident on every GPU that
+// loads this code until the process ends).
+//
+// In HOST code `g_sweep_static_bins` is only a handle for the symbol, not a device address: handing it to a kernel
+// would fault, or on a system where the GPU can reach host memory quietly count into the wrong place.  The address a
+// kernel may use comes from cudaGetSymbolAddress, asked once per device with that device current and kept in
+// g_sweep_static_ptr.  sweep_kernel is the same kernel the allocating path launches; only the table it is handed
+// differs.  The slot table of the finish step travels as a kernel parameter, so there is no host-to-device copy either.
+// ---------------------------------------------------------------------------------------------------------------
+static __device__ __align__(256) unsigned long long g_sweep_static_bins[GP_SWEEP_STATIC_MAX_BINS];
+
+namespace {
+
+constexpr int SWEEP_STATIC_DEVICES = 64;  // device ordinals with a remembered address; higher ones are looked up per call
+std::mutex g_sweep_static_mu;
+unsigned long long* g_sweep_static_ptr[SWEEP_STATIC_DEVICES] = {};
+
+struct SweepSlots { int s[SWEEP_MAX]; };
+
+// sweep_finish_kernel with the slot table passed by value.  block t: hist[slots.s[t]][c] = sum_{j > t} bins[j][c]
+__global__ void __launch_bounds__(256) sweep_finish_slots_kernel(const unsigned long long* __restrict__ bins, uint64_t count,
+                                                                 uint32_t C, int n, SweepSlots slots,
+                                                                 unsigned long long* __restrict__ folding,
+                                                                 unsigned long long* __restrict__ hist) {
+    __shared__ unsigned long long part[256];
+    const int t = blockIdx.x, out = slots.s[t];
+    unsigned long long sum = 0;
+    for (uint32_t c = threadIdx.x; c < C; c += blockDim.x) {
+        unsigned long long v = 0;
+        for (int j = t + 1; j <= n; j++) v += bins[(uint64_t)j * C + c];
+        hist[(uint64_t)out * (C + 1) + c] = v;
+        sum += v;
+    }
+    part[threadIdx.x] = sum;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) part[threadIdx.x] += part[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        folding[out] = part[0];
+        hist[(uint64_t)out * (C + 1) + C] = count - part[0];
+    }
+}
+
+// Device address of g_sweep_static_bins on the CURRENT device.  The first call per device does the lookup (this is the
+// set-up the header asks callers to keep outside stream capture); afterwards it is a table read.
+gp_status sweep_static_table(unsigned long long** out) {
+    int dev = -1;
+    GP_CUDA(cudaGetDevice(&dev));
+    const bool remembered = dev >= 0 && dev < SWEEP_STATIC_DEVICES;
+    std::lock_guard<std::mutex> lk(g_sweep_static_mu);
+    if (remembered && g_sweep_static_ptr[dev]) { *out = g_sweep_static_ptr[dev]; return GP_OK; }
+    unsigned long long* p = nullptr;
+    GP_CUDA(cudaGetSymbolAddress((void**)&p, g_sweep_static_bins));
+    if (!p) { gp_set_cuda_error(cudaErrorInvalidSymbol, "gp_threshold_sweep_static: no device address for the scratch array"); return GP_CUDA_ERROR; }
+    if (remembered) g_sweep_static_ptr[dev] = p;
+    *out = p;
+    return GP_OK;
+}
+
+}  // namespace
+
+extern "C" gp_status gp_threshold_sweep_static(const uint16_t* d_pheno, const int16_t* d_gap, uint64_t count,
+                                               uint32_t n_classes, const int32_t* thresholds, int n_thresholds,
+                                               uint64_t* d_folding, uint64_t* d_hist, void* stream) {
+    if ((!d_pheno || !d_gap) && count) return GP_INVALID_ARG;
+    if (!thresholds || !d_folding || !d_hist || n_classes == 0 || n_classes >= NULLP) return GP_INVALID_ARG;
+    if (n_thresholds < 1 || n_thresholds > SWEEP_MAX) return GP_INVALID_ARG;
+    const size_t n_bins = (size_t)(n_thresholds + 1) * n_classes;
+    if (n_bins > GP_SWEEP_STATIC_MAX_BINS) return GP_TOO_LARGE;  // refused before anything is touched or launched
+    cudaStream_t st = (cudaStream_t)stream;
+    // ascending thresholds; slots.s[r] = position of the r-th smallest in the caller's order
+    SweepThr thr;
+    SweepSlots slots;
+    thr.n = n_thresholds;
+    for (int i = 0; i < SWEEP_MAX; i++) { thr.t[i] = 0; slots.s[i] = 0; }
+    for (int i = 0; i < n_thresholds; i++) {
+        if (thresholds[i] < 1) return GP_INVALID_ARG;
+        int r = i;
+        while (r > 0 && thr.t[r - 1] > thresholds[i]) { thr.t[r] = thr.t[r - 1]; slots.s[r] = slots.s[r - 1]; r--; }
+        thr.t[r] = thresholds[i]; slots.s[r] = i;
+    }
+    unsigned long long* bins = nullptr;
+    gp_status stt = sweep_static_table(&bins);
+    if (stt != GP_OK) return stt;
+    // the array keeps whatever the previous call counted: everything this call reads must start at zero
+    GP_CUDA(cudaMemsetAsync(bins, 0, n_bins * sizeof(unsigned long long), st));
+    const size_t smem = n_bins * 4;
+    const int use_smem = smem <= 200 * 1024;
+    if (use_smem) GP_CUDA(cudaFuncSetAttribute(sweep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    if (count) {
+        const uint64_t want = (count + 511) / 512, cap = (uint64_t)sm_count() * (use_smem && smem > 100 * 1024 ? 1 : 2);
+        sweep_kernel<<<(unsigned)(want < cap ? want : cap), 512, use_smem ? smem : 0, st>>>(
+            d_pheno, d_gap, count, n_classes, thr, bins, use_smem);
+        GP_CUDA(cudaGetLastError());
+    }
+    sweep_finish_slots_kernel<<<n_thresholds, 256, 0, st>>>(bins, count, n_classes, n_thresholds, slots,
+                                                            reinterpret_cast<unsigned long long*>(d_folding),
+                                                            reinterpret_cast<unsigned long long*>(d_hist));
+    GP_CUDA(cudaGetLastError());
+    gp_count_launches(count ? 2 : 1);
+    return GP_OK;
+}

@@ -64,6 +64,8 @@ SIGNATURES = {
     "gp_pair_bitmap_or": (ctypes.c_int, [_vp, _vp, ctypes.c_uint32, _vp]),
     "gp_pair_bitmap_count": (ctypes.c_int, [_vp, ctypes.c_uint32, _vp, _vp]),
     "gp_threshold_sweep": (ctypes.c_int, [_vp, _vp, ctypes.c_uint64, ctypes.c_uint32, _i32p, ctypes.c_int, _vp, _vp, _vp]),
+    "gp_threshold_sweep_static": (ctypes.c_int, [_vp, _vp, ctypes.c_uint64, ctypes.c_uint32, _i32p, ctypes.c_int, _vp, _vp,
+                                                 _vp]),
     "gp_phi_row": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_uint32, ctypes.c_uint32, _vp, _vp]),
     "gp_nn_components": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_uint32, _vp, _vp]),
     "gp_enumerate_host": (ctypes.c_int, [_vp, ctypes.POINTER(_Energies), ctypes.c_uint64, ctypes.c_uint64, _vp, _u64p,
@@ -417,6 +419,33 @@ def threshold_sweep(pheno, gap, n_classes, thresholds, stream=None):
     _check(lib().gp_threshold_sweep(_dptr(pheno, torch.uint16), _dptr(gap, torch.int16), pheno.numel(), n_classes,
                                     thr.ctypes.data_as(_i32p), thr.size, _dptr(folding), _dptr(hist), _stream(stream)),
            "gp_threshold_sweep")
+    return folding, hist
+
+
+SWEEP_STATIC_MAX_BINS = 1 << 19  # GP_SWEEP_STATIC_MAX_BINS
+
+
+def threshold_sweep_static(pheno, gap, n_classes, thresholds, stream=None, out=None):
+    """gp_threshold_sweep_static: threshold_sweep for callers that must not allocate device memory while running (a
+    fixed start-up memory budget, a capped or disabled pool, a loop that cannot take an allocator call).  The library
+    counts in a fixed 4 MiB device array of its own, so (len(thresholds) + 1) * n_classes may not exceed
+    SWEEP_STATIC_MAX_BINS (GpError with status 6 otherwise), and calls whose GPU work can overlap must not share a
+    device.  `out` = (folding int64[T], hist int64[T, C+1]) device tensors the caller allocated beforehand; without it
+    this wrapper allocates them through torch, which only the C call itself avoids.  Returns (folding, hist)."""
+    import torch
+    thr = np.ascontiguousarray(thresholds, np.int32)
+    if gap.numel() != pheno.numel():
+        raise ValueError("pheno and gap differ in size")
+    if out is None:
+        out = (torch.empty(thr.size, dtype=torch.int64, device=pheno.device),
+               torch.empty((thr.size, n_classes + 1), dtype=torch.int64, device=pheno.device))
+    folding, hist = out
+    if folding.numel() != thr.size or hist.numel() != thr.size * (n_classes + 1):
+        raise ValueError("out tensors do not match the thresholds / classes")
+    _check(lib().gp_threshold_sweep_static(_dptr(pheno, torch.uint16), _dptr(gap, torch.int16), pheno.numel(), n_classes,
+                                           thr.ctypes.data_as(_i32p), thr.size, _dptr(folding, torch.int64),
+                                           _dptr(hist, torch.int64), _stream(stream)),
+           "gp_threshold_sweep_static")
     return folding, hist
 
 

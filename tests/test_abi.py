@@ -81,7 +81,7 @@ def test_tuning_and_map_units_host_side():
 def test_status_strings_and_tile():
     L = gpmap.lib()
     assert L.gp_strerror(0) == b"ok"
-    assert all(L.gp_strerror(i) for i in range(6))
+    assert all(L.gp_strerror(i) for i in range(7)) and b"scratch" in L.gp_strerror(6)
     assert gpmap.tile() == 512
 
 
