@@ -271,12 +271,20 @@ void oracle_enumerate(void* h, const int32_t* e /*4*/, int32_t threshold, uint64
     }
 }
 
-// explicit sequences seqs[count][N] over `alphabet` letters (the paper's SeqRnd path)
+// explicit sequences seqs[count][N] over `alphabet` letters (the paper's SeqRnd path).  The paper
+// only ever generates letters inside the alphabet (:762-775) and says nothing about others; reading R19: a
+// byte >= alphabet is read as the LAST letter, alphabet - 1, so the look-up e[l1 * alphabet + l2] stays inside e[].
 void oracle_enumerate_seqs(void* h, int alphabet, const int32_t* e, int32_t threshold, const uint8_t* seqs,
                            uint64_t count, uint16_t* pheno, int32_t* gap /*nullable*/) {
     Structures* S = (Structures*)h;
-    for (uint64_t n = 0; n < count; n++)
-        ground_state(S, seqs + n * S->N, alphabet, e, threshold, &pheno[n], gap ? &gap[n] : NULL);
+    uint8_t letters[64];
+    for (uint64_t n = 0; n < count; n++) {
+        for (int i = 0; i < S->N; i++) {
+            uint8_t l = seqs[n * S->N + i];
+            letters[i] = l < alphabet ? l : (uint8_t)(alphabet - 1);
+        }
+        ground_state(S, letters, alphabet, e, threshold, &pheno[n], gap ? &gap[n] : NULL);
+    }
 }
 
 uint64_t oracle_draw(uint64_t seed, uint64_t ctr) { return draw(seed, ctr); }

@@ -132,6 +132,30 @@ def test_hp_embedded_in_20_letters(oracle_structures):
     assert (ph2 == full[g]).all()
 
 
+def test_letters_outside_the_alphabet_read_as_the_last_letter(oracle_structures):
+    """DESIGN.md reading R19 (the paper only generates letters inside the alphabet): a byte >=
+    alphabet in an explicit sequence is the last letter.  Pinned by the coordinate brute force on the clamped letters
+    (a look-up past e[] — what the unclamped listing :537-545 would do — gives other energies), for 2 and 20 letters."""
+    S = oracle_structures(4, 4)
+    _, _, class_of, _, coords = bf.classify((4, 4, 1))
+    rng = np.random.default_rng(1919)
+    M = rng.integers(-750, -49, (20, 20))
+    M = np.minimum(M, M.T).astype(np.int32).reshape(-1)
+    for alphabet, e, wild in ((2, np.array(HP, np.int32), (2, 3, 7, 128, 255)), (20, M, (20, 21, 64, 200, 255))):
+        seqs = rng.integers(0, alphabet, (80, 16)).astype(np.uint8)
+        hit = rng.random(seqs.shape) < 0.3
+        seqs[hit] = rng.choice(wild, int(hit.sum())).astype(np.uint8)
+        seqs[0, :] = 255                                   # every letter outside: the all-last-letter sequence
+        clamped = np.minimum(seqs, alphabet - 1)
+        assert (seqs != clamped).sum() > 200
+        ph, gap = S.enumerate_seqs(seqs, e, alphabet)
+        ph_c, gap_c = S.enumerate_seqs(clamped, e, alphabet)
+        assert (ph == ph_c).all() and (gap == gap_c).all()
+        for n in range(0, 80, 2):
+            want, wgap = bf.ground_state(coords, class_of, clamped[n].tolist(), e.tolist(), alphabet)
+            assert ph[n] == (NULL if want is None else want) and gap[n] == wgap, (alphabet, n)
+
+
 def test_generator():
     # splitmix64 reference stream for seed 0 (public-domain reference implementation's well-known first outputs)
     assert [orc.draw(0, c) for c in range(3)] == [0xE220A8397B1DCDAF, 0x6E789E6AA1B965F4, 0x06C45D188009454F]
