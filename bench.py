@@ -52,6 +52,8 @@ def parse():
     ap.add_argument("--fold-bits", type=int, default=0, help="gp_tuning.fold_bits: low genotype bits kept as MMA columns")
     ap.add_argument("--force-sharded", action="store_true", help="take the sharded multi-rank step (sharding.py over "
                     "torch.distributed) even with one rank: exercises that code path on a single GPU")
+    ap.add_argument("--map-units", type=int, default=0, help="time gp_enumerate_map_range on this many units of the map (compact "
+                                                             "layout, no full store) instead: the map path's kernels on their own")
     ap.add_argument("--rows", action="store_true", help="time every row of the hot path on its BASELINE.json config instead")
     ap.add_argument("--out", default="", help="--rows: also write the rows to this JSON file")
     return ap.parse_args()
@@ -131,12 +133,26 @@ def peaks():
 
 
 
-PROFILE_CSV = os.path.join(ROOT, "profiles", "r2_scoring_ncu_raw.csv")
+PROFILE_CSV = os.path.join(ROOT, "profiles", "r3_scoring_ncu_raw.csv")
+
+
+def folded_columns(mon):
+    """Contraction columns the scoring kernel executes when the monomers `mon` stay free inside one weight image
+    (DESIGN.md 6.1): 2 bias columns + the monomers + the monomer pairs that can touch (odd distance >= 3)."""
+    return 2 + len(mon) + sum(1 for i in range(len(mon)) for j in range(i + 1, len(mon))
+                              if mon[j] - mon[i] >= 3 and (mon[j] - mon[i]) % 2 == 1)
+
+
+def image_bytes(columns, k_exec, narrow_rows):
+    """Bytes of ONE weight image in HBM: 128-row tiles over the structure columns, rows of 64 bytes when the folded
+    contraction fits them (gp_tuning.narrow_rows), else 128 bytes per 128 features."""
+    row = 64 if (narrow_rows and k_exec <= 64) else 128 * ((k_exec + 127) // 128)
+    return ((columns + 127) // 128) * 128 * row
 
 
 def ncu_profile():
     """Tensor-pipe activity and DRAM bytes of one scoring_kernel launch from the committed `ncu --page raw --csv` export
-    (profiles/r2_scoring_ncu_raw.csv; the command is in profiles/r2_scoring_ncu.md): taken under the profiler in a
+    (profiles/r3_scoring_ncu_raw.csv; the command is in profiles/r3_scoring_ncu.md): taken under the profiler in a
     separate run of the same configuration, read here by file parse only.  None if the file is absent."""
     import csv
     try:
@@ -314,7 +330,7 @@ def workload_config(lattice, G, D, C, K, n, parallelism="independent prefix tile
 
 def full_map_leg(lattice, stream, cpu_check=True):
     """BASELINE.json configs[3] live: the WHOLE map of the lattice through gp_enumerate_map_range (chunks of units, so the
-    run can report progress and could resume), gp_designability and gp_robustness over the resident store; device
+    run can report progress and could resume), gp_reduce_store over the resident store; device
     times from CUDA events on the launching stream; invariants; a seeded sample of phenotypes against the oracle."""
     import numpy as np
     import torch
@@ -329,8 +345,11 @@ def full_map_leg(lattice, stream, cpu_check=True):
     pheno = torch.empty(total, dtype=torch.uint16, device="cuda")
     U = S.map_units()
     chunks = 64 if U >= 64 else 1
-    ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
     l0 = gpmap.launch_count()
+    gpmap.kernel_timing(True)
+    for w in range(4):
+        gpmap.kernel_time(w)
     torch.cuda.synchronize()
     t0 = time.perf_counter()
     ev[0].record(stream)
@@ -338,17 +357,43 @@ def full_map_leg(lattice, stream, cpu_check=True):
         u0, u1 = U * c // chunks, U * (c + 1) // chunks
         S.enumerate_map_range(u0, u1 - u0, pheno, stream=stream)
     ev[1].record(stream)
-    hist = gpmap.designability(pheno, C, stream=stream)
+    hist, R, Dl, Oc, pairs = gpmap.reduce_store(pheno, N, C, stream=stream)   # a5 + a6: designability from the first sweep
     ev[2].record(stream)
-    R, Dl, Oc, pairs = gpmap.robustness(pheno, N, C, stream=stream)
-    ev[3].record(stream)
     torch.cuda.synchronize()
     wall = time.perf_counter() - t0
-    t_score, t_hist, t_rob = (ev[i].elapsed_time(ev[i + 1]) * 1e-3 for i in range(3))
+    t_score, t_red = (ev[i].elapsed_time(ev[i + 1]) * 1e-3 for i in range(2))
     launches = gpmap.launch_count() - l0
+    ktime = [gpmap.kernel_time(w) for w in range(4)]
+    gpmap.kernel_timing(False)
     hist = hist.cpu().numpy().astype(np.uint64)
     R, Dl, Oc = (x.cpu().numpy().astype(np.uint64) for x in (R, Dl, Oc))
     folding = int(hist[:C].sum())
+    # the tiled neighbour pass on this store runs geometries the oracle cannot reach (third pass): gp_phi_row, an
+    # untiled kernel of its own, is the independent witness (row[q] = R[q], sum_{p != q} row[p] = O[q], row[C] = D[q])
+    from paper_2008_05612_b200.full_map import phi_row_witness
+    witness = phi_row_witness(gpmap, pheno, N, C, hist, R, Dl, Oc)
+    # map-path roofline of the scoring phase as a whole (image builds, combines and launch tails included): executed int8
+    # ops of the folded contraction over the device time of the phase, against the MMA-only probe of the same K steps
+    k = min(S.tuning()["sym_bits"], N // 2)
+    k_exec = folded_columns(list(range(k)) + list(range(N - k, N)))
+    k_steps = (k_exec + 31) // 32
+    probe_ops, probe_clk, probe_mhz = gpmap.probe_i8_peak(k_steps, 1.0)
+    achieved = 2.0 * k_exec * float(total) * C / t_score / 1e12
+    sc_ms, sc_n = ktime[gpmap.KERNEL_SCORING]
+    im_ms, im_n = ktime[gpmap.KERNEL_IMAGE]
+    img_b = image_bytes(C, k_exec, S.tuning()["narrow_rows"])
+    n_images = float(total) / float(1 << (2 * k))
+    map_roofline = {"kernel": "tc::scoring_kernel (hrec mode) + tc::build_image_kernel + tc::combine_kernel, whole scoring phase",
+                    "bound": "tensor", "achieved": achieved, "peak": probe_ops / 1e12, "unit": "TFLOP/s",
+                    "frac": achieved / (probe_ops / 1e12), "traffic": None,
+                    "peak_source": "gp_probe_i8_peak(k_steps=%d), measured after the map" % k_steps,
+                    "ops_per_eval_executed": 2.0 * k_exec, "ops_per_eval_issued": 64.0 * k_steps,
+                    "frac_issued": achieved * 32.0 * k_steps / k_exec / (probe_ops / 1e12),
+                    "algorithmic_bytes": 2.0 * total, "image_bytes": 2.0 * n_images * img_b,
+                    "scoring_launches": int(sc_n), "scoring_launch_ms_summed": sc_ms, "image_launches": int(im_n),
+                    "image_launch_ms_summed": im_ms,
+                    "note": "launches of a range alternate between two streams and overlap, so the summed per-launch times "
+                            "may exceed the phase time; the fraction uses the phase time"}
     rng = np.random.default_rng(SEED)
     g = rng.integers(0, total, size=1 << 20, dtype=np.uint64)
     rev = np.zeros_like(g)
@@ -359,10 +404,10 @@ def full_map_leg(lattice, stream, cpu_check=True):
     out = {"workload": "%s HP whole map: 2^%d genotypes x %d directed structures (%d representatives scored, reversal "
                        "identity), uint16 store resident in HBM (%.1f GB), designability + neighbour pass + pair count"
                        % (lattice, N, D, C, 2.0 * total / 1e9),
-           "wall_s": wall, "device_s": {"scoring": t_score, "designability": t_hist, "neighbour_pass": t_rob,
-                                        "total": t_score + t_hist + t_rob},
+           "wall_s": wall, "device_s": {"scoring": t_score, "designability_and_neighbour_pass": t_red, "total": t_score + t_red},
            "effective_evals_per_s": float(total) * D / t_score, "executed_evals_per_s": float(total) * C / t_score,
-           "store_GBps": {"designability": 2.0 * total / t_hist / 1e9, "neighbour_pass_algorithmic": 2.0 * total / t_rob / 1e9},
+           "store_GBps": {"reduce_store_algorithmic": 2.0 * total / t_red / 1e9},
+           "roofline": map_roofline,
            "gpu_launches": int(launches), "unit_chunks": chunks,
            "folding": folding, "folding_fraction": folding / total, "designable_classes": int((hist[:C] > 0).sum()),
            "phenotype_pairs": int(pairs.item()), "sum_R": int(R.sum()), "sum_D": int(Dl.sum()), "sum_O": int(Oc.sum()),
@@ -370,6 +415,7 @@ def full_map_leg(lattice, stream, cpu_check=True):
                           "R+D+O_equals_N_x_folding": int(R.sum() + Dl.sum() + Oc.sum()) == N * folding,
                           "sum_R_even": int(R.sum()) % 2 == 0, "sum_O_even": int(Oc.sum()) % 2 == 0,
                           "reversal_symmetry_mismatches_of_2^20": rev_bad}}
+    out["invariants"].update(witness)
     if cpu_check:
         from oracle import gp_oracle as orc
         O = orc.Structures(*LATTICES[lattice])
@@ -383,6 +429,33 @@ def full_map_leg(lattice, stream, cpu_check=True):
     S.close()
     torch.cuda.empty_cache()
     return out
+
+
+def run_map_units(args):
+    """--map-units U: `steps` calls of gp_enumerate_map_range over U units of the lattice's map in the compact layout
+    (a slice of the whole-map run that needs no 2^N store), after `warmup` calls; CUDA-event time.  The committed command
+    behind the map-path ncu captures under profiles/."""
+    import torch
+    from paper_2008_05612_b200 import gpmap
+    S = gpmap.Structures(*LATTICES[args.lattice])
+    U = min(args.map_units, S.map_units())
+    first = (S.map_units() - U) // 3
+    n = int(gpmap.lib().gp_map_range_genotypes(S._h, first, U))
+    ph = torch.empty(n, dtype=torch.uint16, device="cuda")
+    for _ in range(args.warmup):
+        S.enumerate_map_range(first, U, ph, compact=True)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(args.steps):
+        S.enumerate_map_range(first, U, ph, compact=True)
+    e1.record()
+    torch.cuda.synchronize()
+    t = e0.elapsed_time(e1) * 1e-3 / args.steps
+    print(json.dumps({"row": "f1 gp_enumerate_map_range (compact layout)", "lattice": args.lattice, "units": U, "first_unit": first,
+                      "genotypes": n, "seconds_per_call": t, "executed_evals_per_s": float(n) * S.C / t,
+                      "effective_evals_per_s": float(n) * S.D / t, "sym_bits": S.tuning()["sym_bits"]}), flush=True)
+    S.close()
 
 
 def run_rows(args):
@@ -490,9 +563,9 @@ def run_ours(args):
             os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT="29531", RANK="0", WORLD_SIZE="1")
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     gpmap.lib()  # fails loudly if libgpmap.so is missing / unbuildable
-    if args.rows:
+    if args.rows or args.map_units:
         if rank == 0:
-            run_rows(args)
+            run_map_units(args) if args.map_units else run_rows(args)
         return
 
     dims = LATTICES[args.lattice]
@@ -503,7 +576,6 @@ def run_ours(args):
     G = N if args.full else min(args.log2_genotypes, N)
     n = 1 << G
     pheno = torch.empty(n, dtype=torch.uint16, device="cuda")
-    hist = torch.empty(C + 1, dtype=torch.int64, device="cuda")
     stream = torch.cuda.current_stream()
 
     def barrier():
@@ -529,8 +601,9 @@ def run_ours(args):
             S.enumerate_map(pheno, stream=stream)                     # a1-a4, whole map through the reversal identity
         else:
             S.enumerate(b, n, pheno, stream=stream)                   # a1-a4
-        gpmap.designability(pheno, C, hist=hist, stream=stream)       # a5
-        return gpmap.robustness(pheno, G, C, stream=stream)           # a6 (+ pair bitmap)
+        out = gpmap.reduce_store(pheno, G, C, stream=stream)          # a5 + a6 (+ pair bitmap) in one sweep of the store
+        step.hist = out[0]
+        return out
 
     for i in range(args.warmup):
         step(i)
@@ -558,7 +631,7 @@ def run_ours(args):
         t = torch.tensor([ms], dtype=torch.float64, device="cuda")
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         ms = float(t.item())
-    folding = int(n - hist[C].item()) if not sharded else None
+    folding = int(n - step.hist[C].item()) if not sharded else None
     evals_step = float(n) * D * world
     value = evals_step * args.steps / (ms * 1e-3)
 
@@ -597,8 +670,7 @@ def run_ours(args):
         evals_launch = float(n) * C / max(1, sc_n // max(1, args.steps))
     else:
         mon = list(range(min(N, S.tuning()["fold_bits"])))            # low genotype bits kept as contraction columns
-    k_exec = 2 + len(mon) + sum(1 for i in range(len(mon)) for j in range(i + 1, len(mon))
-                                if mon[j] - mon[i] >= 3 and (mon[j] - mon[i]) % 2 == 1)  # bias x2 + monomers + pairs
+    k_exec = folded_columns(mon)                                      # bias x2 + monomers + pairs
     k_steps = (k_exec + 31) // 32
     ops_exec = 2.0 * k_exec                                           # int8 multiply-adds x2 of the folded contraction per evaluation
     ops_issued = 2.0 * 32 * k_steps                                   # what the MMAs issue (columns padded to 32-byte K steps)
@@ -608,10 +680,23 @@ def run_ours(args):
     probe_ops, probe_clk, probe_mhz = gpmap.probe_i8_peak(k_steps, 1.0)
     peak_i8 = probe_ops / 1e12
     prof = ncu_profile()
+    # the ncu capture describes this run's launches only if it is a launch of the same shape: its duration (cold, under
+    # the profiler) must sit near the launch time measured here; otherwise the DRAM figure is dropped, not quoted
+    same_shape = bool(prof and prof["duration_ms"] and dur > 0 and 0.8 < prof["duration_ms"] / (dur * 1e3) < 1.35)
+    genotypes_launch = evals_launch / (C if args.full else D)
+    images_launch = genotypes_launch / float(1 << len(mon))
+    img_b = image_bytes(C if args.full else D, k_exec, S.tuning()["narrow_rows"])
     roofline = {"kernel": "tc::scoring_kernel", "bound": "tensor", "achieved": achieved, "peak": peak_i8, "unit": "TFLOP/s",
                 "frac": achieved / peak_i8,
-                "traffic": prof["dram_bytes"] if prof else None,
-                "traffic_source": (prof["file"] + " (one launch of the same configuration under ncu --set full)") if prof else None,
+                "traffic": prof["dram_bytes"] if same_shape else None,
+                "traffic_source": ((prof["file"] + " (one launch under ncu --set full: %.2f ms there, %.2f ms here)"
+                                    % (prof["duration_ms"], dur * 1e3)) if same_shape else
+                                   ("dropped: the committed capture is not a launch of this shape" if prof else None)),
+                # what the DRAM traffic is made of, computed (not profiled): the phenotypes written, and the per-prefix
+                # weight images that build_image_kernel writes and this kernel reads back once
+                "algorithmic_bytes": 2.0 * genotypes_launch,
+                "image_bytes": 2.0 * images_launch * img_b,
+                "images_per_launch": images_launch, "bytes_per_image": img_b,
                 "peak_source": "gp_probe_i8_peak(k_steps=%d): MMA-only tcgen05.mma kind::i8 stream, measured in this run" % k_steps,
                 "peak_i8_measured": {"TOPs": peak_i8, "clk_per_mma": probe_clk, "sm_mhz": probe_mhz},
                 "frac_issued": achieved * ops_issued / ops_exec / peak_i8,
@@ -632,10 +717,12 @@ def run_ours(args):
     hs_ms, hs_n = ktime[gpmap.KERNEL_HIST]
     im_ms, im_n = ktime[gpmap.KERNEL_IMAGE]
     other = {
-        "robustness_kernel": {"bound": "hbm", "algorithmic_GBps": 2.0 * n / (rb_ms / max(1, rb_n) * 1e-3) / 1e9 if rb_ms else None,
+        "robustness_kernel": {"bound": "alu (instruction-bound, DESIGN.md 6.4; the HBM figure is what one read of the store would need)", "algorithmic_GBps": 2.0 * n / (rb_ms / max(1, rb_n) * 1e-3) / 1e9 if rb_ms else None,
                               "peak": hbm, "avg_launch_ms": rb_ms / max(1, rb_n), "share_of_step": rb_ms / ms},
         "hist_kernel": {"bound": "hbm", "algorithmic_GBps": 2.0 * n / (hs_ms / max(1, hs_n) * 1e-3) / 1e9 if hs_ms else None,
-                        "peak": hbm, "avg_launch_ms": hs_ms / max(1, hs_n), "share_of_step": hs_ms / ms},
+                        "peak": hbm, "avg_launch_ms": hs_ms / max(1, hs_n), "share_of_step": hs_ms / ms, "launches": int(hs_n),
+                        "note": "the step takes designability from gp_reduce_store (first sweep of the neighbour pass): "
+                                "hist_kernel runs only where gp_designability is called on its own"},
         "build_image_kernel": {"avg_launch_ms": im_ms / max(1, im_n), "launches": int(im_n), "share_of_step": im_ms / ms,
                                "note": "runs on a side stream overlapped with the scoring kernel: elapsed, not exclusive, time"},
     }
@@ -655,8 +742,7 @@ def run_ours(args):
                 torch.cuda.synchronize()
                 e0.record(stream)
             S3.enumerate_map(p3, stream=stream)
-            h3 = gpmap.designability(p3, S3.C, stream=stream)
-            gpmap.robustness(p3, 27, S3.C, stream=stream)
+            h3 = gpmap.reduce_store(p3, 27, S3.C, stream=stream)[0]
         e1.record(stream)
         torch.cuda.synchronize()
         sec = e0.elapsed_time(e1) * 1e-3 / reps

@@ -284,9 +284,10 @@ extern "C" gp_status gp_enumerate_host(const gp_structures_t* s, const gp_energi
     uint64_t* d_rdo = d_out + C + 1;
     uint64_t* d_pc = d_rdo + 3 * (size_t)C;
     gp_status st = gp_enumerate(s, en, g_begin, g_count, d_pheno, nullptr, nullptr);
-    if (st == GP_OK) st = gp_designability(d_pheno, g_count, C, d_hist, nullptr);
-    if (st == GP_OK && rdo)
-        st = gp_robustness(d_pheno, n_bits, C, d_rdo, d_rdo + C, d_rdo + 2 * (size_t)C, pair_count ? d_pc : nullptr, nullptr);
+    if (st == GP_OK) {  // with the neighbour pass, its first sweep of the store also counts the classes (gp_reduce_store)
+        if (rdo) st = gp_reduce_store(d_pheno, n_bits, C, d_hist, d_rdo, d_rdo + C, d_rdo + 2 * (size_t)C, pair_count ? d_pc : nullptr, nullptr);
+        else st = gp_designability(d_pheno, g_count, C, d_hist, nullptr);
+    }
     if (st == GP_OK) {
         cudaError_t e = cudaSuccess;
         if (pheno && g_count) e = cudaMemcpy(pheno, d_pheno, g_count * sizeof(uint16_t), cudaMemcpyDeviceToHost);

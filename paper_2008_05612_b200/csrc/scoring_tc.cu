@@ -632,7 +632,7 @@ __global__ void __launch_bounds__(SQ_THREADS, 1) sequence_kernel(const SqArgs a,
             const uint64_t q = (uint64_t)item * SQ_ROWS + m * TM + r;
             unsigned long long h = 1ULL << 63;  // bit 63: the constant-1 feature; bit 62 stays 0 for unused columns
             if (q < a.count)
-                for (int i = 0; i < a.N; i++) h |= (unsigned long long)(a.seqs[q * a.N + i] & 1) << i;
+                for (int i = 0; i < a.N; i++) h |= (unsigned long long)(a.seqs[q * a.N + i] != 0) << i;  // a letter outside {0, 1} is the last letter, H (R19)
             mbar_wait(&bar->a_empty, (item_no & 1) ^ 1);
 #pragma unroll 1
             for (uint32_t c16 = 0; c16 < SQ_MAXCOL / 16; c16++) {

@@ -1,15 +1,18 @@
 """Whole GP map of one lattice on one GPU, in resumable pieces: phenotype store in HBM, designability, neighbour counts,
 pair count.
 
-    python -m paper_2008_05612_b200.full_map --lattice 6x6 --out gpurun_out/map_6x6 [--chunks 64] [--resume]
+    python -m paper_2008_05612_b200.full_map --lattice 6x6 --out gpurun_out/map_6x6 [--chunks 64]
+    python -m paper_2008_05612_b200.full_map --lattice 3x3x3 --out out/map_333 --checkpoint-store [--resume]
     torchrun --nproc-per-node 8 -m paper_2008_05612_b200.full_map --lattice 6x6 --out out/map_6x6 --sharded
 
 The map is scored as `chunks` ranges of units through gp_enumerate_map_range (include/gpmap.h; the paper's own 110-day
 job survived by appending results run by run).  After every chunk <out>/progress.json
 records the units done; with --checkpoint-store the store is also saved (<out>/store.u16, sensible up to 3x3x3), and
---resume continues from the recorded unit instead of starting over.  Then gp_designability and gp_robustness run over
-the resident store and the invariants that need no reference are checked: sum(hist) = 2^N,
-sum(R+D+O) = N x folding, sum R and sum O even, pheno(rev g) = pheno(g) on a seeded sample
+--resume continues from the recorded chunk instead of starting over; --resume without a saved store (or with other
+settings than the interrupted run) is an error, never a silent restart.  Then gp_reduce_store runs over the resident
+store and the invariants that need no reference are checked: sum(hist) = 2^N,
+sum(R+D+O) = N x folding, sum R and sum O even, pheno(rev g) = pheno(g) on a seeded sample, and gp_phi_row of the most
+and least designable class against R / D / O of the tiled neighbour pass
 (tests/test_gpu_map_range.py::test_full_map_run_survives_an_interruption compares such a run with the CPU oracle).
 Writes summary.json and counts.npz (hist, R, D, O).  6x6 needs 137.4 GB for the store (BASELINE.json configs[3])."""
 import argparse
@@ -29,6 +32,25 @@ def bit_reverse(g, n):
     return r
 
 
+def phi_row_witness(gpmap, pheno, n_bits, C, hist, R, Dl, Oc):
+    """An independent witness for the tiled neighbour pass on stores the oracle cannot reach (the 6x6 map's third pass):
+    gp_phi_row — another, untiled kernel — for the most designable class and the rarest non-empty one.  Adjacency is
+    symmetric, so with row[p] = flips leading from class p into q (Eq. 2 numerators):
+    row[q] = R[q], sum_{p != q} row[p] = O[q], row[C] (from null genotypes) = D[q].  Returns {check name: bool}."""
+    designable = np.nonzero(hist[:C])[0]
+    if designable.size == 0:
+        return {}
+    top = int(designable[np.argmax(hist[designable])])
+    rare = int(designable[np.argmin(hist[designable])])
+    out = {}
+    for name, q in (("top", top), ("rarest", rare)):
+        row = gpmap.phi_row(pheno, n_bits, C, q).cpu().numpy().astype(np.uint64)
+        out["phi_row_%s_equals_R" % name] = int(row[q]) == int(R[q])
+        out["phi_row_%s_sums_to_O" % name] = int(row[:C].sum() - row[q]) == int(Oc[q])
+        out["phi_row_%s_from_null_equals_D" % name] = int(row[C]) == int(Dl[q])
+    return out
+
+
 def run(lattice, out, chunks=64, sample=1 << 20, seed=200805612, keep_store=False, prefix_path=False, resume=False,
         checkpoint_store=False, stop_after=None):
     """stop_after = number of chunks after which the run stops as if interrupted (returns None); used by the tests."""
@@ -42,15 +64,23 @@ def run(lattice, out, chunks=64, sample=1 << 20, seed=200805612, keep_store=Fals
     total = 1 << N
     U = S.map_units()
     chunks = max(1, min(chunks, U))
-    pheno = torch.empty(total, dtype=torch.uint16, device="cuda")
     done_chunks, seconds_before = 0, 0.0
-    if resume and os.path.exists(prog_path):
+    if resume:   # never restart silently: a resume that cannot continue is an error the caller must see
+        if not os.path.exists(prog_path):
+            raise RuntimeError("--resume: %s does not exist; start the run without --resume" % prog_path)
         with open(prog_path) as f:
             prog = json.load(f)
         same = (prog.get("lattice"), prog.get("chunks"), prog.get("units"), prog.get("prefix_path")) == (lattice, chunks, U, prefix_path)
-        if same and prog.get("store_saved") and os.path.exists(store_path):
-            pheno.copy_(torch.from_numpy(np.fromfile(store_path, dtype=np.int16)).view(torch.uint16))
-            done_chunks, seconds_before = prog["chunks_done"], prog.get("scoring_seconds", 0.0)
+        if not same:
+            raise RuntimeError("--resume: %s was written by a run with other settings (lattice / chunks / units / path): %r"
+                               % (prog_path, prog))
+        if not (prog.get("store_saved") and os.path.exists(store_path)):
+            raise RuntimeError("--resume: the interrupted run saved no store (%s); only a run started with "
+                               "--checkpoint-store can be resumed" % store_path)
+        done_chunks, seconds_before = prog["chunks_done"], prog.get("scoring_seconds", 0.0)
+    pheno = torch.empty(total, dtype=torch.uint16, device="cuda")
+    if done_chunks:
+        pheno.copy_(torch.from_numpy(np.fromfile(store_path, dtype=np.int16)).view(torch.uint16))
     log = open(os.path.join(out, "progress.log"), "a" if done_chunks else "w")
 
     def say(msg):
@@ -88,19 +118,18 @@ def run(lattice, out, chunks=64, sample=1 << 20, seed=200805612, keep_store=Fals
             log.close()
             S.close()
             return None
-    ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
     ev[0].record()
-    hist = gpmap.designability(pheno, C)
+    hist, R, Dl, Oc, pairs = gpmap.reduce_store(pheno, N, C)   # designability comes out of the neighbour pass's first sweep
     ev[1].record()
-    R, Dl, Oc, pairs = gpmap.robustness(pheno, N, C)
-    ev[2].record()
     torch.cuda.synchronize()
-    t_hist, t_rob = (ev[i].elapsed_time(ev[i + 1]) * 1e-3 for i in range(2))
-    say("scoring %.1f s, designability %.2f s, neighbour pass %.1f s" % (t_score, t_hist, t_rob))
+    t_red = ev[0].elapsed_time(ev[1]) * 1e-3
+    say("scoring %.1f s, designability + neighbour pass %.2f s" % (t_score, t_red))
 
     hist = hist.cpu().numpy().astype(np.uint64)
     R, Dl, Oc = (x.cpu().numpy().astype(np.uint64) for x in (R, Dl, Oc))
     folding = int(hist[:C].sum())
+    witness = phi_row_witness(gpmap, pheno, N, C, hist, R, Dl, Oc)
     rng = np.random.default_rng(seed)
     g = rng.integers(0, total, size=min(sample, total), dtype=np.uint64)
     gi = torch.from_numpy(g.astype(np.int64)).cuda()
@@ -114,14 +143,14 @@ def run(lattice, out, chunks=64, sample=1 << 20, seed=200805612, keep_store=Fals
         "sum_O_even": int(Oc.sum()) % 2 == 0,
         "reversal_symmetry_sample_mismatches": rev_mismatch,
     }
+    checks.update(witness)
     order = np.argsort(hist[:C])[::-1]
     summary = {
         "lattice": lattice, "N": N, "D": D, "C": C, "genotypes": total, "evaluations": float(total) * D,
         "path": "gp_enumerate (prefix tiles, D columns)" if prefix_path else "gp_enumerate_map_range (reversal identity, C columns)",
         "chunks": chunks, "resumed_at_chunk": done_chunks,
         "evaluations_executed": float(total) * (D if prefix_path else C),
-        "seconds": {"scoring": t_score, "designability": t_hist, "neighbour_pass": t_rob,
-                    "total": t_score + t_hist + t_rob},
+        "seconds": {"scoring": t_score, "designability_and_neighbour_pass": t_red, "total": t_score + t_red},
         "evals_per_s_scoring": float(total) * D / t_score,
         "folding": folding, "folding_fraction": folding / total, "null": int(hist[C]),
         "designable_classes": int((hist[:C] > 0).sum()), "top5_designability": [int(hist[i]) for i in order[:5]],

@@ -145,3 +145,24 @@ def test_seeded_generator_matches_recipe():
         assert np.array_equal(gpmap.seeded_sequences(seed, 1 << 40, 50, 36), orc.seeded_sequences(seed, 1 << 40, 50, 36))
     M = gpmap.seeded_matrix(200805612)
     assert M.min() >= -750 and M.max() <= -50 and np.array_equal(M, M.T)
+
+
+def test_full_map_resume_fails_loudly_without_a_saved_store(tmp_path):
+    """full_map --resume never restarts silently (host logic; the checks come before any device work): no progress file,
+    a progress file of a run with other settings, and a run that saved no store are all errors."""
+    import json
+    from paper_2008_05612_b200 import full_map
+    out = str(tmp_path / "map")
+    with pytest.raises(RuntimeError, match="does not exist"):
+        full_map.run("4x4", out, chunks=4, resume=True)
+    S = gpmap.Structures(4, 4)
+    U = S.map_units()
+    S.close()
+    assert U >= 3
+    prog = {"lattice": "4x4", "chunks": 2, "units": U, "prefix_path": False, "chunks_done": 1, "store_saved": False}
+    with open(os.path.join(out, "progress.json"), "w") as f:
+        json.dump(prog, f)
+    with pytest.raises(RuntimeError, match="saved no store"):
+        full_map.run("4x4", out, chunks=2, resume=True)
+    with pytest.raises(RuntimeError, match="other settings"):
+        full_map.run("4x4", out, chunks=3, resume=True)

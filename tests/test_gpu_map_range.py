@@ -371,20 +371,31 @@ def test_int8_peak_probe_is_plausible():
 
 
 def test_reduce_store_at_the_bench_tile_size(oracle_structures):
-    """gp_reduce_store == gp_designability + gp_robustness on a 2^26-genotype 6x6 tile (the bench step's size: two passes,
-    16 + 10 flips), and on its first 2^17 entries == the oracle's reductions."""
+    """gp_reduce_store on a WHOLE 2^26-genotype 6x6 prefix tile — the bench step's tile and the geometry the full 6x6 map
+    runs its second pass with (direct-table kernel, 2^15 on-chip tiles, 11 spread bits in 32-byte segments) — and on its
+    first 2^24 entries (9 spread bits), against the oracle's designability and neighbour pass of the SAME full stores
+    (Eq. 2): histogram, neutral / deleterious / other counts of every class and the pair count.  The
+    two oracle sweeps (about 50 s and 11 s of single-threaded CPU) run side by side in threads (ctypes drops the GIL).
+    gp_designability + gp_robustness, the separate calls, must give the same integers."""
+    from concurrent.futures import ThreadPoolExecutor
     S = lib_structures((6, 6, 1))
     G, n = 26, 1 << 26
     ph = torch.empty(n, dtype=torch.uint16, device="cuda")
     S.enumerate(0x2A5 << G, n, ph)
-    hist = gpmap.designability(ph, S.C)
-    R, Dl, Oc, pc = gpmap.robustness(ph, G, S.C)
-    h2, R2, D2, O2, pc2 = gpmap.reduce_store(ph, G, S.C)
-    assert torch.equal(hist, h2) and torch.equal(R, R2) and torch.equal(Dl, D2) and torch.equal(Oc, O2) and int(pc) == int(pc2)
-    small = ph[:1 << 17]
-    store = small.cpu().numpy()
-    h3, R3, D3, O3, pc3 = gpmap.reduce_store(small, 17, S.C)
-    Ro, Do, Oo, pco = orc.robustness(store, 17, S.C)
-    assert np.array_equal(h3.cpu().numpy().astype(np.uint64), orc.designability(store, S.C))
-    assert np.array_equal(R3.cpu().numpy().astype(np.uint64), Ro) and np.array_equal(D3.cpu().numpy().astype(np.uint64), Do)
-    assert np.array_equal(O3.cpu().numpy().astype(np.uint64), Oo) and int(pc3) == pco
+    store = ph.cpu().numpy()
+    with ThreadPoolExecutor(2) as pool:
+        jobs = {bits: (pool.submit(orc.robustness, store[:1 << bits], bits, S.C),
+                       pool.submit(orc.designability, store[:1 << bits], S.C)) for bits in (26, 24)}
+        got = {bits: gpmap.reduce_store(ph[:1 << bits], bits, S.C) for bits in (26, 24)}
+        hist = gpmap.designability(ph, S.C)
+        R, Dl, Oc, pc = gpmap.robustness(ph, G, S.C)
+        h2, R2, D2, O2, pc2 = got[26]
+        assert torch.equal(hist, h2) and torch.equal(R, R2) and torch.equal(Dl, D2) and torch.equal(Oc, O2) and int(pc) == int(pc2)
+        for bits in (24, 26):
+            (Ro, Do, Oo, pco), ho = jobs[bits][0].result(), jobs[bits][1].result()
+            h3, R3, D3, O3, pc3 = got[bits]
+            assert np.array_equal(h3.cpu().numpy().astype(np.uint64), ho), bits
+            assert np.array_equal(R3.cpu().numpy().astype(np.uint64), Ro), bits
+            assert np.array_equal(D3.cpu().numpy().astype(np.uint64), Do), bits
+            assert np.array_equal(O3.cpu().numpy().astype(np.uint64), Oo), bits
+            assert int(pc3) == pco and pco > 0, bits

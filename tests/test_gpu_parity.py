@@ -410,3 +410,34 @@ def test_explicit_hp_sequences_on_tensor_cores(oracle_structures, dims, count):
     finally:
         S.tune(seq_tensor=1)
     assert torch.equal(a.view(torch.int16), b.view(torch.int16)), dims
+
+
+@pytest.mark.parametrize("dims", [(5, 5, 1), (6, 6, 1)])
+def test_letters_outside_the_alphabet_on_every_sequence_kernel(oracle_structures, dims):
+    """DESIGN.md reading R19: a byte >= alphabet in an explicit sequence is the last letter.  The three sequence kernels
+    (CUDA-core score_simple_kernel, limb seq20_kernel, two-letter sequence_kernel) are picked by gp_tuning.seq_tensor and
+    by the batch size (128 and 256 are the switches), so the same bytes go through every setting and through batches on
+    both sides of each switch: ids and gaps must equal the oracle's every time."""
+    import workloads
+    S, O = lib_structures(dims), oracle_structures(*dims)
+    rng = np.random.default_rng(1900 + S.N)
+    M = orc.seeded_matrix(200805612)
+    for alphabet, e, wild in ((2, np.array(gpmap.HP_ENERGIES, np.int32), (2, 3, 7, 128, 255)), (20, M, (20, 21, 64, 200, 255))):
+        seqs = workloads.random_sequences(700, S.N, alphabet, seed=19)
+        hit = rng.random(seqs.shape) < 0.25
+        seqs[hit] = rng.choice(wild, int(hit.sum())).astype(np.uint8)
+        seqs[5, :] = 255
+        ph_o, gap_o = O.enumerate_seqs(seqs, e, alphabet)
+        assert not np.array_equal(ph_o, O.enumerate_seqs(seqs & 1 if alphabet == 2 else seqs % 20, e, alphabet, want_gap=False))
+        d_seqs = torch.from_numpy(seqs).cuda()
+        try:
+            for tensor in (0, 1, 2):
+                S.tune(seq_tensor=tensor)
+                for count in (100, 200, 300, 700):
+                    ph = torch.empty(count, dtype=torch.uint16, device="cuda")
+                    gap = torch.empty(count, dtype=torch.int16, device="cuda")
+                    S.enumerate_seqs(d_seqs[:count], ph, gap, e=e, alphabet=alphabet)
+                    assert np.array_equal(ph.cpu().numpy(), ph_o[:count]), (dims, alphabet, tensor, count)
+                    assert np.array_equal(gap.cpu().numpy().astype(np.int32), gap_o[:count]), (dims, alphabet, tensor, count)
+        finally:
+            S.tune(seq_tensor=1)
