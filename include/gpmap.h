@@ -256,7 +256,9 @@ uint64_t gp_launch_count(void);
 
 /* Per-kernel device timing for bench.py's roofline line.  While enabled, every launch of the kernels below is
  * bracketed by a CUDA event pair on its own stream.  gp_kernel_time waits for those launches, returns the summed device
- * time in milliseconds and the number of launches since the last query, and forgets them.  Off by default. */
+ * time in milliseconds and the number of launches since the last query, and forgets them.  Off by default.  The sum is
+ * over launches, not wall time: the scoring launches of gp_enumerate_map_range alternate between two streams and overlap,
+ * and the image builder runs beside the scoring kernel, so their sums can exceed the elapsed time of the call. */
 enum { GP_KERNEL_SCORING = 0, GP_KERNEL_IMAGE = 1, GP_KERNEL_HIST = 2, GP_KERNEL_ROBUSTNESS = 3, GP_KERNEL_COUNT = 4 };
 void gp_kernel_timing(int enable);
 gp_status gp_kernel_time(int which, double* ms_total, uint64_t* launches);

@@ -22,25 +22,31 @@ extern "C" uint64_t gp_launch_count(void) { return g_launches.load(std::memory_o
 
 // ---- optional per-kernel timing: one CUDA event pair per launch, on the launching stream ----
 namespace {
-struct EvPair { cudaEvent_t a, b; };
+struct EvPair { cudaEvent_t a, b; uint64_t serial; bool ended; };
 std::mutex g_time_mu;
 bool g_time_on = false;
+uint64_t g_time_serial = 0;
 std::vector<EvPair> g_time_ev[GP_KERNEL_COUNT];
 }  // namespace
 
-void gp_time_begin(int which, cudaStream_t st) {
-    if (!g_time_on) return;
+uint64_t gp_time_begin(int which, cudaStream_t st) {
+    if (!g_time_on) return 0;
     std::lock_guard<std::mutex> lk(g_time_mu);
     EvPair p;
-    if (cudaEventCreate(&p.a) != cudaSuccess) return;
-    if (cudaEventCreate(&p.b) != cudaSuccess) { cudaEventDestroy(p.a); return; }
+    if (cudaEventCreate(&p.a) != cudaSuccess) return 0;
+    if (cudaEventCreate(&p.b) != cudaSuccess) { cudaEventDestroy(p.a); return 0; }
     cudaEventRecord(p.a, st);
+    p.serial = ++g_time_serial;
+    p.ended = false;
     g_time_ev[which].push_back(p);
+    return p.serial;
 }
-void gp_time_end(int which, cudaStream_t st) {
-    if (!g_time_on) return;
+void gp_time_end(int which, uint64_t token, cudaStream_t st) {
+    if (!token) return;
     std::lock_guard<std::mutex> lk(g_time_mu);
-    if (!g_time_ev[which].empty()) cudaEventRecord(g_time_ev[which].back().b, st);
+    std::vector<EvPair>& v = g_time_ev[which];
+    for (size_t i = v.size(); i-- > 0;)   // the pair is near the back; it is gone if gp_kernel_time ran in between
+        if (v[i].serial == token) { cudaEventRecord(v[i].b, st); v[i].ended = true; return; }
 }
 extern "C" void gp_kernel_timing(int enable) {
     std::lock_guard<std::mutex> lk(g_time_mu);
@@ -53,11 +59,13 @@ extern "C" gp_status gp_kernel_time(int which, double* ms_total, uint64_t* launc
     uint64_t n = 0;
     gp_status st = GP_OK;
     for (EvPair& p : g_time_ev[which]) {
-        float ms = 0;
-        cudaError_t e = cudaEventSynchronize(p.b);
-        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, p.a, p.b);
-        if (e == cudaSuccess) { tot += ms; n++; }
-        else { gp_set_cuda_error(e, "gp_kernel_time"); st = GP_CUDA_ERROR; }
+        if (p.ended) {   // a pair whose launch is still between begin and end on another thread is dropped, not waited for
+            float ms = 0;
+            cudaError_t e = cudaEventSynchronize(p.b);
+            if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, p.a, p.b);
+            if (e == cudaSuccess) { tot += ms; n++; }
+            else { gp_set_cuda_error(e, "gp_kernel_time"); st = GP_CUDA_ERROR; }
+        }
         cudaEventDestroy(p.a);
         cudaEventDestroy(p.b);
     }

@@ -8,8 +8,10 @@
 void gp_set_cuda_error(cudaError_t e, const char* where);
 void gp_count_launches(unsigned n);  // feeds gp_launch_count(): every kernel launch of the library is counted
 // Optional per-kernel device timing (gp_kernel_timing / gp_kernel_time): CUDA events around one launch on its stream.
-void gp_time_begin(int which, cudaStream_t st);
-void gp_time_end(int which, cudaStream_t st);
+// gp_time_begin returns a token naming ITS event pair (0 = timing off); gp_time_end records the end on that pair, so
+// calls that run concurrently on one handle from several threads cannot close each other's pairs.
+uint64_t gp_time_begin(int which, cudaStream_t st);
+void gp_time_end(int which, uint64_t token, cudaStream_t st);
 
 #define GP_CUDA(call)                                 \
     do {                                              \
@@ -19,6 +21,30 @@ void gp_time_end(int which, cudaStream_t st);
             return e_ == cudaErrorMemoryAllocation ? GP_OUT_OF_MEMORY : GP_CUDA_ERROR; \
         }                                             \
     } while (0)
+
+// Per-call working memory from the device's stream-ordered pool that finds its way back on EVERY exit path of a call
+// (GP_CUDA returns early).  release() is the normal end: freed in stream order on the call's stream.  A destructor that
+// still holds the block is an error path: other streams of the call (image builder, combine) may have work pending on
+// it, so the device is drained before the block goes back.
+struct gp_pool_mem {
+    void* p = nullptr;
+    cudaStream_t st = nullptr;
+    gp_pool_mem() = default;
+    gp_pool_mem(const gp_pool_mem&) = delete;
+    gp_pool_mem& operator=(const gp_pool_mem&) = delete;
+    cudaError_t alloc(size_t bytes, cudaStream_t s) { st = s; return cudaMallocAsync(&p, bytes, s); }
+    template <class T> T* as() const { return static_cast<T*>(p); }
+    cudaError_t release() {
+        cudaError_t e = p ? cudaFreeAsync(p, st) : cudaSuccess;
+        p = nullptr;
+        return e;
+    }
+    ~gp_pool_mem() {
+        if (!p) return;
+        cudaDeviceSynchronize();
+        cudaFreeAsync(p, st);
+    }
+};
 
 // Validated alphabet-2 energies in the form the kernels use:
 //   E(g,S) = a*NBP + lin * sum_k c_k(S) h_k + quad * #HH-contacts,  lin = b - a, quad = c - 2b + a

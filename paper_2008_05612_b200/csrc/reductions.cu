@@ -546,6 +546,65 @@ __global__ void __launch_bounds__(256) robustness_cross_kernel(RobArgs a, const 
     }
 }
 
+// The same with a per-block class table in shared memory: one packed u32 per class, fields neutral (bits 0-10) |
+// to-null (11-21) | other (22-31), one shared-memory atomic per non-null entry.  A field is emptied through its HALF
+// mark: the one thread whose add takes a field from HALF - 1 to HALF subtracts HALF from the field and books HALF in
+// the global counter.  Until that subtraction lands at most blockDim - 1 further adds can reach the field, so with
+// XT = 512 threads it stays below 2 * HALF (other: 512 + 511 = 1023) and never carries into its neighbour; what is left
+// in the table at the end is flushed class by class.  Global atomics per block: one per HALF entries of a class and
+// field, plus at most three per class seen — instead of one per non-null entry, all ranks hammering the few designable
+// classes (3 x 2^33 entries per rank for 6x6 on 8 GPUs).
+constexpr int XT = 512;
+constexpr uint32_t X_RBITS = 11, X_DBITS = 11, X_OBITS = 10;
+__device__ __forceinline__ void xtab_add(uint32_t* tab, const RobArgs& a, uint32_t p, uint32_t shift, uint32_t bits,
+                                         unsigned long long* global) {
+    const uint32_t half = 1u << (bits - 1), mask = (1u << bits) - 1u;
+    const uint32_t old = atomicAdd(&tab[p], 1u << shift);
+    if (((old >> shift) & mask) + 1u == half) {
+        atomicSub(&tab[p], half << shift);
+        atomicAdd(&global[p], (unsigned long long)half);
+    }
+}
+__global__ void __launch_bounds__(XT, 1) robustness_cross_table_kernel(RobArgs a, const uint16_t* __restrict__ partner,
+                                                                       uint64_t count) {
+    extern __shared__ uint32_t xtab[];
+    for (uint32_t c = threadIdx.x; c < a.C; c += XT) xtab[c] = 0;
+    __syncthreads();
+    auto one = [&](uint32_t p, uint32_t q) {
+        if (p == NULLP || p >= a.C) return;
+        if (q == p) xtab_add(xtab, a, p, 0, X_RBITS, a.R);
+        else if (q == NULLP) xtab_add(xtab, a, p, X_RBITS, X_DBITS, a.Dl);
+        else {
+            xtab_add(xtab, a, p, X_RBITS + X_DBITS, X_OBITS, a.O);
+            if (a.bitmap && q < a.C) note_pair(a, p, q);
+        }
+    };
+    // 16-byte vectors where both shards allow it (they are 2^k-entry device arrays in practice), scalars for the rest
+    const bool vec = (((uintptr_t)a.pheno | (uintptr_t)partner) & 15) == 0;
+    const uint64_t n_vec = vec ? count >> 3 : 0;
+    for (uint64_t v = (uint64_t)blockIdx.x * XT + threadIdx.x; v < n_vec; v += (uint64_t)gridDim.x * XT) {
+        const uint4 x = __ldg(reinterpret_cast<const uint4*>(a.pheno) + v);
+        if (x.x == 0xFFFFFFFFu && x.y == 0xFFFFFFFFu && x.z == 0xFFFFFFFFu && x.w == 0xFFFFFFFFu) continue;  // eight nulls
+        const uint4 y = __ldg(reinterpret_cast<const uint4*>(partner) + v);
+        uint32_t mine[8], theirs[8];
+        unpack8(x, mine);
+        unpack8(y, theirs);
+#pragma unroll
+        for (int j = 0; j < 8; j++) one(mine[j], theirs[j]);
+    }
+    for (uint64_t i = n_vec * 8 + (uint64_t)blockIdx.x * XT + threadIdx.x; i < count; i += (uint64_t)gridDim.x * XT)
+        one(a.pheno[i], partner[i]);
+    __syncthreads();
+    for (uint32_t c = threadIdx.x; c < a.C; c += XT) {
+        const uint32_t w = xtab[c];
+        if (!w) continue;
+        const uint32_t r = w & ((1u << X_RBITS) - 1u), d = (w >> X_RBITS) & ((1u << X_DBITS) - 1u), o = w >> (X_RBITS + X_DBITS);
+        if (r) atomicAdd(&a.R[c], (unsigned long long)r);
+        if (d) atomicAdd(&a.Dl[c], (unsigned long long)d);
+        if (o) atomicAdd(&a.O[c], (unsigned long long)o);
+    }
+}
+
 __global__ void bitmap_or_kernel(uint32_t* __restrict__ dst, const uint32_t* __restrict__ src, uint64_t n_words) {
     for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_words; i += (uint64_t)gridDim.x * blockDim.x) {
         const uint32_t v = src[i];
@@ -688,10 +747,10 @@ extern "C" gp_status gp_designability(const uint16_t* d_pheno, uint64_t count, u
     const uint64_t want = (count / 8 + 1023) / 1024;
     const int per_sm = use_smem ? (int)((224 * 1024) / (smem + 1024) > 2 ? 2 : 1) : 2;
     unsigned grid = (unsigned)(want < (uint64_t)sm_count() * per_sm ? (want ? want : 1) : (uint64_t)sm_count() * per_sm);
-    gp_time_begin(GP_KERNEL_HIST, st);
+    const uint64_t tk1 = gp_time_begin(GP_KERNEL_HIST, st);
     hist_kernel<<<grid, 1024, use_smem ? smem : 0, st>>>(d_pheno, count, n_classes,
                                                          reinterpret_cast<unsigned long long*>(d_hist), use_smem);
-    gp_time_end(GP_KERNEL_HIST, st);
+    gp_time_end(GP_KERNEL_HIST, tk1, st);
     GP_CUDA(cudaGetLastError());
     gp_count_launches(1);
     return GP_OK;
@@ -713,9 +772,9 @@ static gp_status robustness_passes(const uint16_t* d_pheno, int n_bits, uint32_t
     a.O = reinterpret_cast<unsigned long long*>(d_other);
     a.bitmap = d_pair_bitmap;
     if (n_bits < 3) {
-        gp_time_begin(GP_KERNEL_ROBUSTNESS, st);
+        const uint64_t tk2 = gp_time_begin(GP_KERNEL_ROBUSTNESS, st);
         robustness_tiny_kernel<<<1, 32, 0, st>>>(a);
-        gp_time_end(GP_KERNEL_ROBUSTNESS, st);
+        gp_time_end(GP_KERNEL_ROBUSTNESS, tk2, st);
         GP_CUDA(cudaGetLastError());
         gp_count_launches(1);
         if (d_hist) {
@@ -749,7 +808,7 @@ static gp_status robustness_passes(const uint16_t* d_pheno, int n_bits, uint32_t
     const int seg_bits = direct ? 4 : 6;
     const int hmax = tb - seg_bits > 1 ? tb - seg_bits : (tb - 3 > 1 ? tb - 3 : 1);
     int passes_left = (n_bits - tb + hmax - 1) / hmax;
-    unsigned long long* tot = nullptr;                  // direct kernel, pass 0 with the histogram: per-call totals
+    gp_pool_mem tot_mem;                                // direct kernel, pass 0 with the histogram: per-call totals
     int done = 0;
     bool first = true;
     while (done < n_bits) {
@@ -759,7 +818,7 @@ static gp_status robustness_passes(const uint16_t* d_pheno, int n_bits, uint32_t
             passes_left--;
             a.h = h; a.c = tb - h; a.hi_pos = done; a.f0 = a.c; done += h;
         }
-        gp_time_begin(GP_KERNEL_ROBUSTNESS, st);
+        const uint64_t tk3 = gp_time_begin(GP_KERNEL_ROBUSTNESS, st);
         {
             Rob2Args b;
             b.pheno = a.pheno; b.n_bits = n_bits; b.C = n_classes; b.R = a.R; b.Dl = a.Dl; b.O = a.O;
@@ -767,14 +826,15 @@ static gp_status robustness_passes(const uint16_t* d_pheno, int n_bits, uint32_t
             b.bitmap = a.bitmap; b.tb = a.tb; b.c = a.c; b.h = a.h; b.hi_pos = a.hi_pos; b.f0 = a.f0;
             if (direct) {
                 if (b.hist) {
-                    GP_CUDA(cudaMallocAsync(&tot, 3 * (size_t)n_classes * sizeof(unsigned long long), st));
+                    GP_CUDA(tot_mem.alloc(3 * (size_t)n_classes * sizeof(unsigned long long), st));
+                    unsigned long long* tot = tot_mem.as<unsigned long long>();
                     GP_CUDA(cudaMemsetAsync(tot, 0, 3 * (size_t)n_classes * sizeof(unsigned long long), st));
                     b.R = tot; b.Dl = tot + n_classes; b.O = tot + 2 * (size_t)n_classes;
                 }
                 if (d_pair_bitmap) robustness3_kernel<true><<<grid, R2THREADS, smem, st>>>(b);
                 else robustness3_kernel<false><<<grid, R2THREADS, smem, st>>>(b);
                 if (b.hist) {
-                    rob3_finish_kernel<<<(n_classes + 255) / 256, 256, 0, st>>>(tot, n_classes, (uint32_t)(b.tb - b.f0), a.R, a.Dl, a.O, b.hist);
+                    rob3_finish_kernel<<<(n_classes + 255) / 256, 256, 0, st>>>(tot_mem.as<unsigned long long>(), n_classes, (uint32_t)(b.tb - b.f0), a.R, a.Dl, a.O, b.hist);
                     gp_count_launches(1);
                 }
             } else {
@@ -782,10 +842,10 @@ static gp_status robustness_passes(const uint16_t* d_pheno, int n_bits, uint32_t
                 else robustness2_kernel<false><<<grid, R2THREADS, smem, st>>>(b);
             }
         }
-        gp_time_end(GP_KERNEL_ROBUSTNESS, st);
+        gp_time_end(GP_KERNEL_ROBUSTNESS, tk3, st);
         GP_CUDA(cudaGetLastError());
         gp_count_launches(1);
-        if (tot) { cudaFreeAsync(tot, st); tot = nullptr; }
+        GP_CUDA(tot_mem.release());
         first = false;
     }
     return GP_OK;
@@ -811,10 +871,20 @@ extern "C" gp_status gp_robustness_cross(const uint16_t* d_mine, const uint16_t*
     a.Dl = reinterpret_cast<unsigned long long*>(d_deleterious);
     a.O = reinterpret_cast<unsigned long long*>(d_other);
     a.bitmap = d_pair_bitmap;
-    const uint64_t want = (count + 255) / 256, cap = (uint64_t)sm_count() * 8;
-    gp_time_begin(GP_KERNEL_ROBUSTNESS, st);
-    robustness_cross_kernel<<<(unsigned)(want < cap ? want : cap), 256, 0, st>>>(a, d_partner, count);
-    gp_time_end(GP_KERNEL_ROBUSTNESS, st);
+    // the class table in shared memory whenever it fits one block per SM and the shard is long enough to repay zeroing
+    // and flushing it; otherwise one global atomic per non-null entry
+    const size_t table = (size_t)n_classes * sizeof(uint32_t);
+    const bool use_table = table <= 220 * 1024 && count >= 16 * (uint64_t)n_classes;
+    if (use_table) GP_CUDA(cudaFuncSetAttribute(robustness_cross_table_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)table));
+    const uint64_t tk4 = gp_time_begin(GP_KERNEL_ROBUSTNESS, st);
+    if (use_table) {
+        const uint64_t want = (count / 8 + XT - 1) / XT, cap = (uint64_t)sm_count();
+        robustness_cross_table_kernel<<<(unsigned)(want < cap ? (want ? want : 1) : cap), XT, table, st>>>(a, d_partner, count);
+    } else {
+        const uint64_t want = (count + 255) / 256, cap = (uint64_t)sm_count() * 8;
+        robustness_cross_kernel<<<(unsigned)(want < cap ? want : cap), 256, 0, st>>>(a, d_partner, count);
+    }
+    gp_time_end(GP_KERNEL_ROBUSTNESS, tk4, st);
     GP_CUDA(cudaGetLastError());
     gp_count_launches(1);
     return GP_OK;
@@ -853,16 +923,18 @@ extern "C" gp_status gp_reduce_store(const uint16_t* d_pheno, int n_bits, uint32
     GP_CUDA(cudaMemsetAsync(d_deleterious, 0, cb, st));
     GP_CUDA(cudaMemsetAsync(d_other, 0, cb, st));
     if (d_hist) GP_CUDA(cudaMemsetAsync(d_hist, 0, cb + sizeof(uint64_t), st));
-    uint32_t* bitmap = nullptr;
+    gp_pool_mem bitmap_mem;
     if (d_pair_count) {
         const uint64_t n_words = gp_pair_bitmap_words(n_classes);
-        GP_CUDA(cudaMallocAsync(&bitmap, n_words * 4, st));
-        GP_CUDA(cudaMemsetAsync(bitmap, 0, n_words * 4, st));
+        GP_CUDA(bitmap_mem.alloc(n_words * 4, st));
+        GP_CUDA(cudaMemsetAsync(bitmap_mem.p, 0, n_words * 4, st));
     }
+    uint32_t* bitmap = bitmap_mem.as<uint32_t>();
     gp_status stt = robustness_passes(d_pheno, n_bits, n_classes, d_neutral, d_deleterious, d_other, d_hist, bitmap, 0, st);
     if (stt == GP_OK && d_pair_count) stt = gp_pair_bitmap_count(bitmap, n_classes, d_pair_count, stream);
-    if (bitmap) cudaFreeAsync(bitmap, st);
-    return stt;
+    if (stt != GP_OK) return stt;
+    GP_CUDA(bitmap_mem.release());
+    return GP_OK;
 }
 
 extern "C" gp_status gp_robustness(const uint16_t* d_pheno, int n_bits, uint32_t n_classes, uint64_t* d_neutral,
@@ -888,8 +960,9 @@ extern "C" gp_status gp_threshold_sweep(const uint16_t* d_pheno, const int16_t* 
         thr.t[r] = thresholds[i]; slot[r] = i;
     }
     const size_t n_bins = (size_t)(n_thresholds + 1) * n_classes;
-    char* work = nullptr;  // bins | slot table
-    GP_CUDA(cudaMallocAsync(&work, n_bins * 8 + SWEEP_MAX * sizeof(int), st));
+    gp_pool_mem work_mem;  // bins | slot table
+    GP_CUDA(work_mem.alloc(n_bins * 8 + SWEEP_MAX * sizeof(int), st));
+    char* work = work_mem.as<char>();
     unsigned long long* bins = reinterpret_cast<unsigned long long*>(work);
     int* d_slot = reinterpret_cast<int*>(work + n_bins * 8);
     GP_CUDA(cudaMemsetAsync(bins, 0, n_bins * 8, st));
@@ -908,7 +981,7 @@ extern "C" gp_status gp_threshold_sweep(const uint16_t* d_pheno, const int16_t* 
                                                       reinterpret_cast<unsigned long long*>(d_hist));
     GP_CUDA(cudaGetLastError());
     gp_count_launches(count ? 2 : 1);
-    GP_CUDA(cudaFreeAsync(work, st));
+    GP_CUDA(work_mem.release());
     return GP_OK;
 }
 
@@ -933,8 +1006,9 @@ extern "C" gp_status gp_nn_components(const uint16_t* d_pheno, int n_bits, uint3
     if (n_bits < 1 || n_bits > 30) return GP_INVALID_ARG;
     cudaStream_t st = (cudaStream_t)stream;
     const uint64_t n = 1ULL << n_bits;
-    uint32_t* parent = nullptr;
-    GP_CUDA(cudaMallocAsync(&parent, n * sizeof(uint32_t), st));
+    gp_pool_mem parent_mem;
+    GP_CUDA(parent_mem.alloc(n * sizeof(uint32_t), st));
+    uint32_t* parent = parent_mem.as<uint32_t>();
     GP_CUDA(cudaMemsetAsync(d_ncomp, 0, (size_t)n_classes * sizeof(uint32_t), st));
     const unsigned grid = (unsigned)((n + 255) / 256 < (uint64_t)sm_count() * 16 ? (n + 255) / 256 : (uint64_t)sm_count() * 16);
     uf_init_kernel<<<grid, 256, 0, st>>>(parent, n);
@@ -942,7 +1016,7 @@ extern "C" gp_status gp_nn_components(const uint16_t* d_pheno, int n_bits, uint3
     uf_count_kernel<<<grid, 256, 0, st>>>(d_pheno, parent, n, n_classes, d_ncomp);
     GP_CUDA(cudaGetLastError());
     gp_count_launches(3);
-    GP_CUDA(cudaFreeAsync(parent, st));
+    GP_CUDA(parent_mem.release());
     GP_CUDA(cudaStreamSynchronize(st));
     return GP_OK;
 }

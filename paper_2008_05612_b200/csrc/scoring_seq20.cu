@@ -338,9 +338,9 @@ gp_status gp_launch_seq20_tc(const gp_structures_s* s, const gp_energies* en, in
     void (*k)(const QArgs) = seeded ? seq20_kernel<QSRC_SEEDED> : seq20_kernel<QSRC_SEQS>;
     GP_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const unsigned grid = a.n_items < (uint32_t)sms ? a.n_items : (uint32_t)sms;
-    gp_time_begin(GP_KERNEL_SCORING, st);
+    const uint64_t tk1 = gp_time_begin(GP_KERNEL_SCORING, st);
     k<<<grid, Q_THREADS, smem, st>>>(a);
-    gp_time_end(GP_KERNEL_SCORING, st);
+    gp_time_end(GP_KERNEL_SCORING, tk1, st);
     GP_CUDA(cudaGetLastError());
     gp_count_launches(1);
     return GP_OK;

@@ -115,8 +115,9 @@ gp_status launch_simple(const gp_structures_s* s, const gp_energies* en, int src
         }
     if ((long long)(emax - emin) * s->NBP > 65535 || (size_t)s->P * 128 > 65535) return GP_INVALID_ARG;  // packed 16-bit costs / offsets
     if (count == 0) return GP_OK;
-    int16_t* d_e = nullptr;
-    GP_CUDA(cudaMallocAsync(&d_e, sizeof(h_e), st));
+    gp_pool_mem e_mem;
+    GP_CUDA(e_mem.alloc(sizeof(h_e), st));
+    int16_t* d_e = e_mem.as<int16_t>();
     GP_CUDA(cudaMemcpyAsync(d_e, h_e, sizeof(int16_t) * A * A, cudaMemcpyHostToDevice, st));  // pageable: staged before return
 
     SimpleArgs a;
@@ -140,7 +141,7 @@ gp_status launch_simple(const gp_structures_s* s, const gp_energies* en, int src
     k<<<grid, BD, smem, st>>>(a, d_e);
     GP_CUDA(cudaGetLastError());
     gp_count_launches(1);
-    GP_CUDA(cudaFreeAsync(d_e, st));
+    GP_CUDA(e_mem.release());
     return GP_OK;
 }
 

@@ -893,12 +893,13 @@ gp_status gp_launch_scoring_tc(const gp_structures_s* s, const gp_hp_params& hp,
     group = tc_group_size((size_t)group, 1, ((1ULL << fb) + SUPER - 1) / SUPER, p.sms);
     const uint64_t n_batches_all = ((g_end - 1) >> fb) - (g_begin >> fb) + 1;
     if (group > n_batches_all) group = n_batches_all;
-    int8_t* d_img0 = nullptr;  // per-call working memory from the stream-ordered pool: calls on other streams have their own
-    GP_CUDA(cudaMallocAsync(&d_img0, 2 * p.img_bytes * (size_t)group, st));
+    gp_pool_mem work;  // per-call working memory from the stream-ordered pool: calls on other streams have their own
+    GP_CUDA(work.alloc(2 * p.img_bytes * (size_t)group, st));
+    int8_t* d_img0 = work.as<int8_t>();
     ImagePipeline pipe;
     {
         gp_status ps = pipe.open(st);
-        if (ps != GP_OK) { cudaFreeAsync(d_img0, st); return ps; }
+        if (ps != GP_OK) return ps;
     }
     if (p.narrow) GP_CUDA(cudaFuncSetAttribute(build_image_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)build_image_smem<64>(fb)));
     else GP_CUDA(cudaFuncSetAttribute(build_image_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)build_image_smem<128>(fb)));
@@ -915,10 +916,10 @@ gp_status gp_launch_scoring_tc(const gp_structures_s* s, const gp_hp_params& hp,
         ia.gfix_first = b0; ia.unit_first = 0; ia.paired = 0; ia.mid = 0; ia.gfix_shift = fb; ia.D = s->D; ia.n_tiles = p.n_tiles;
         ia.NBP = s->NBP; ia.lin = hp.lin; ia.quad = hp.quad;
         pipe.before_build(grp);
-        gp_time_begin(GP_KERNEL_IMAGE, pipe.side);
+        const uint64_t tk1 = gp_time_begin(GP_KERNEL_IMAGE, pipe.side);
         if (p.narrow) build_image_kernel<64><<<dim3(p.n_tiles, (n_batches + IMG_PER_BLOCK - 1) / IMG_PER_BLOCK), TN, build_image_smem<64>(fb), pipe.side>>>(ia, p.slots, n_batches, fb);
         else build_image_kernel<128><<<dim3(p.n_tiles, (n_batches + IMG_PER_BLOCK - 1) / IMG_PER_BLOCK), TN, build_image_smem<128>(fb), pipe.side>>>(ia, p.slots, n_batches, fb);
-        gp_time_end(GP_KERNEL_IMAGE, pipe.side);
+        gp_time_end(GP_KERNEL_IMAGE, tk1, pipe.side);
         pipe.after_build(grp, st);
         Args a;
         a.img = d_img; a.class_of = s->d_class_of; a.pheno = d_pheno; a.gap = d_gap;
@@ -927,17 +928,18 @@ gp_status gp_launch_scoring_tc(const gp_structures_s* s, const gp_hp_params& hp,
         a.n_tiles = p.n_tiles; a.D = s->D; a.fb = fb; a.k_steps = p.k_steps; a.threshold = hp.threshold;
         a.hrec = nullptr; a.n_snap = p.n_tiles;
         const unsigned grid = a.n_items < (uint32_t)p.sms ? a.n_items : (uint32_t)p.sms;
-        gp_time_begin(GP_KERNEL_SCORING, st);
+        const uint64_t tk2 = gp_time_begin(GP_KERNEL_SCORING, st);
         p.kernel<<<grid, p.threads, p.smem, st>>>(a, p.cols);
-        gp_time_end(GP_KERNEL_SCORING, st);
+        gp_time_end(GP_KERNEL_SCORING, tk2, st);
         pipe.after_scoring(grp, st);
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) { gp_set_cuda_error(e, "scoring launch"); result = GP_CUDA_ERROR; break; }
         gp_count_launches(2);
         g = stop;
     }
-    cudaFreeAsync(d_img0, st);
-    return result;
+    if (result != GP_OK) return result;  // `work` drains the device before it gives the buffers back
+    GP_CUDA(work.release());
+    return GP_OK;
 }
 
 // ---- whole map through the reversal identity E(g, rev S) = E(rev g, S) ---------------
@@ -1011,13 +1013,14 @@ static gp_status gp_launch_map_range(const gp_structures_s* s, const gp_hp_param
         const uint64_t most = 2 * pairs > u_count - pairs ? 2 * pairs : u_count - pairs;
         if (group > most) group = (size_t)((most + 1) & ~1ULL);
     }
-    char* d_work = nullptr;
-    GP_CUDA(cudaMallocAsync(&d_work, (2 * p.img_bytes + 2 * rec_bytes) * group, st));
+    gp_pool_mem work;
+    GP_CUDA(work.alloc((2 * p.img_bytes + 2 * rec_bytes) * group, st));
+    char* d_work = work.as<char>();
     int4* d_rec0 = (int4*)(d_work + 2 * p.img_bytes * group);
     ImagePipeline pipe;
     {
         gp_status ps = pipe.open(st, u_count >= 1024);   // small ranges: a few launches, not worth two more streams
-        if (ps != GP_OK) { cudaFreeAsync(d_work, st); return ps; }
+        if (ps != GP_OK) return ps;
     }
     if (p.narrow) GP_CUDA(cudaFuncSetAttribute(build_image_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)build_image_smem<64>(fb)));
     else GP_CUDA(cudaFuncSetAttribute(build_image_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)build_image_smem<128>(fb)));
@@ -1036,10 +1039,10 @@ static gp_status gp_launch_map_range(const gp_structures_s* s, const gp_hp_param
         ia.gfix_first = 0; ia.unit_first = u; ia.paired = paired; ia.mid = mid; ia.gfix_shift = k; ia.D = s->D_sym;
         ia.n_tiles = p.n_tiles; ia.NBP = s->NBP; ia.lin = hp.lin; ia.quad = hp.quad;
         pipe.before_build(grp);
-        gp_time_begin(GP_KERNEL_IMAGE, pipe.side);
+        const uint64_t tk3 = gp_time_begin(GP_KERNEL_IMAGE, pipe.side);
         if (p.narrow) build_image_kernel<64><<<dim3(p.n_tiles, (n_img + IMG_PER_BLOCK - 1) / IMG_PER_BLOCK), TN, build_image_smem<64>(fb), pipe.side>>>(ia, p.slots, n_img, fb);
         else build_image_kernel<128><<<dim3(p.n_tiles, (n_img + IMG_PER_BLOCK - 1) / IMG_PER_BLOCK), TN, build_image_smem<128>(fb), pipe.side>>>(ia, p.slots, n_img, fb);
-        gp_time_end(GP_KERNEL_IMAGE, pipe.side);
+        gp_time_end(GP_KERNEL_IMAGE, tk3, pipe.side);
         cudaStream_t sg = pipe.scoring_stream(grp, st);
         pipe.after_build(grp, sg);
         Args a;
@@ -1051,9 +1054,9 @@ static gp_status gp_launch_map_range(const gp_structures_s* s, const gp_hp_param
         a.hrec = d_rec; a.n_snap = s->n_snap;
         const unsigned grid = a.n_items < (uint32_t)p.sms ? a.n_items : (uint32_t)p.sms;
         pipe.before_scoring(grp, sg);
-        gp_time_begin(GP_KERNEL_SCORING, sg);
+        const uint64_t tk4 = gp_time_begin(GP_KERNEL_SCORING, sg);
         p.kernel<<<grid, p.threads, p.smem, sg>>>(a, p.cols);
-        gp_time_end(GP_KERNEL_SCORING, sg);
+        gp_time_end(GP_KERNEL_SCORING, tk4, sg);
         pipe.after_scoring(grp, sg);
         CombArgs ca;
         ca.hrec = d_rec; ca.units = s->d_units; ca.class_sym = s->d_class_sym;
@@ -1070,8 +1073,9 @@ static gp_status gp_launch_map_range(const gp_structures_s* s, const gp_hp_param
         u = stop;
     }
     pipe.join_post(n_groups, st);
-    cudaFreeAsync(d_work, st);
-    return result;
+    if (result != GP_OK) return result;  // `work` drains the device before it gives the buffers back
+    GP_CUDA(work.release());
+    return GP_OK;
 }
 
 extern "C" uint64_t gp_map_range_genotypes(const gp_structures_t* s, uint64_t unit_first, uint64_t unit_count) {
@@ -1114,7 +1118,7 @@ gp_status gp_launch_sequences_tc(const gp_structures_s* s, const gp_hp_params& h
     const uint32_t n_tiles = (s->D + TN - 1) / TN;
     // weight image of (lin, quad): cached in the handle, immutable once built; other streams wait on its event
     const int8_t* d_img = nullptr;
-    int8_t* d_private = nullptr;  // cache full: a per-call image from the stream-ordered pool
+    gp_pool_mem private_img;      // cache full: a per-call image from the stream-ordered pool
     {
         std::lock_guard<std::mutex> lk(s->mu);
         for (const gp_weight_image& w : s->wimgs)
@@ -1127,17 +1131,25 @@ gp_status gp_launch_sequences_tc(const gp_structures_s* s, const gp_hp_params& h
             w.lin = hp.lin; w.quad = hp.quad;
             const bool cache = s->wimgs.size() < 8;
             if (cache) GP_CUDA(cudaMalloc(&w.d_img, (size_t)n_tiles * SQ_TILE));  // first use of these energies only
-            else { GP_CUDA(cudaMallocAsync(&d_private, (size_t)n_tiles * SQ_TILE, st)); w.d_img = d_private; }
+            else { GP_CUDA(private_img.alloc((size_t)n_tiles * SQ_TILE, st)); w.d_img = private_img.as<int8_t>(); }
             SqImgArgs ia;
             ia.contacts = s->d_contacts; ia.pairidx = s->d_pairidx; ia.img = w.d_img; ia.D = s->D;
             ia.N = s->N; ia.NBP = s->NBP; ia.lin = hp.lin; ia.quad = hp.quad;
             build_full_image_kernel<<<n_tiles, TN, 0, st>>>(ia);
-            GP_CUDA(cudaGetLastError());
+            cudaError_t e = cudaGetLastError();
+            cudaEvent_t ev = nullptr;
+            if (e == cudaSuccess && cache) {
+                e = cudaEventCreateWithFlags(&ev, cudaEventDisableTiming);
+                if (e == cudaSuccess) e = cudaEventRecord(ev, st);
+            }
+            if (e != cudaSuccess) {   // an image that never reached the cache is not kept
+                gp_set_cuda_error(e, "gp_enumerate_seqs: weight image build");
+                if (ev) cudaEventDestroy(ev);
+                if (cache) { cudaStreamSynchronize(st); cudaFree(w.d_img); }
+                return GP_CUDA_ERROR;
+            }
             gp_count_launches(1);
             if (cache) {
-                cudaEvent_t ev;
-                GP_CUDA(cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
-                GP_CUDA(cudaEventRecord(ev, st));
                 w.ready = ev;
                 s->wimgs.push_back(w);
             }
@@ -1163,12 +1175,12 @@ gp_status gp_launch_sequences_tc(const gp_structures_s* s, const gp_hp_params& h
     a.n_items = (uint32_t)((count + SQ_ROWS - 1) / SQ_ROWS); a.n_tiles = n_tiles;
     a.N = s->N; a.ksteps = (ncol + 31) / 32; a.threshold = hp.threshold;
     const unsigned grid = a.n_items < (uint32_t)sms ? a.n_items : (uint32_t)sms;
-    gp_time_begin(GP_KERNEL_SCORING, st);
+    const uint64_t tk5 = gp_time_begin(GP_KERNEL_SCORING, st);
     sequence_kernel<<<grid, SQ_THREADS, smem, st>>>(a, cols);
-    gp_time_end(GP_KERNEL_SCORING, st);
+    gp_time_end(GP_KERNEL_SCORING, tk5, st);
     GP_CUDA(cudaGetLastError());
     gp_count_launches(1);
-    if (d_private) GP_CUDA(cudaFreeAsync(d_private, st));
+    GP_CUDA(private_img.release());
     return GP_OK;
 }
 
@@ -1201,9 +1213,17 @@ extern "C" gp_status gp_probe_i8_peak(int k_steps, double seconds, double* ops_p
     GP_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     unsigned long long* d_cycles = nullptr;
     GP_CUDA(cudaMalloc(&d_cycles, sms * sizeof(unsigned long long)));
-    cudaEvent_t e0, e1;
-    GP_CUDA(cudaEventCreate(&e0));
-    GP_CUDA(cudaEventCreate(&e1));
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    {
+        cudaError_t e = cudaEventCreate(&e0);
+        if (e == cudaSuccess) e = cudaEventCreate(&e1);
+        if (e != cudaSuccess) {
+            gp_set_cuda_error(e, "gp_probe_i8_peak: cudaEventCreate");
+            if (e0) cudaEventDestroy(e0);
+            cudaFree(d_cycles);
+            return GP_CUDA_ERROR;
+        }
+    }
     const uint32_t mma_per_group = (64 / k_steps) * k_steps;
     uint32_t groups = 2000;  // ~4 ms; then scaled to the requested duration
     float ms = 0;

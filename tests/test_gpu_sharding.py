@@ -63,6 +63,41 @@ def test_cross_shard_flip_on_synthetic_stores():
     assert int(gpmap.pair_bitmap_count(bm, C)) == pco
 
 
+@pytest.mark.parametrize("C,hot", [(300, 0.7), (28728, 0.5), (51704, 0.2)])
+def test_cross_shard_flip_with_the_shared_memory_class_table(C, hot):
+    """gp_robustness_cross on shards long enough for its per-block class table (packed 11 | 11 | 10-bit fields emptied
+    through their half marks): a store with a few very hot classes, so that every field passes its half mark many times
+    in every block, against the oracle's neighbour pass of the whole store (Eq. 2) — and, on slices
+    that start one entry late (scalar loads, ragged count), against the definition written out in numpy."""
+    from oracle import gp_oracle as orc
+    rng = np.random.default_rng(C)
+    n_bits = 21
+    n = 1 << n_bits
+    store = rng.integers(0, C, size=n).astype(np.uint16)
+    pick = rng.random(n) < hot
+    store[pick] = rng.integers(0, 3, size=int(pick.sum())).astype(np.uint16)      # classes 0..2 take most entries
+    store[rng.random(n) < 0.4] = 0xFFFF
+    half = n >> 1
+    store[half:][rng.random(half) < 0.5] = 0                                     # many neutral and to-class-0 pairs across the top bit
+    ph = torch.from_numpy(store.view(np.int16)).cuda().view(torch.uint16)
+    rdo = torch.zeros((3, C), dtype=torch.int64, device="cuda")
+    bm = gpmap.pair_bitmap(C)
+    for a, b in ((ph[:half], ph[half:]), (ph[half:], ph[:half])):
+        gpmap.robustness_partial(a, n_bits - 1, C, rdo, bm)
+        gpmap.robustness_cross(a, b, C, rdo, bm)
+    Ro, Do, Oo, pco = orc.robustness(store, n_bits, C)
+    got = rdo.cpu().numpy().astype(np.uint64)
+    assert np.array_equal(got[0], Ro) and np.array_equal(got[1], Do) and np.array_equal(got[2], Oo)
+    assert int(gpmap.pair_bitmap_count(bm, C)) == pco
+    # misaligned, ragged slices: entry i of `mine` against entry i of `theirs`
+    mine, theirs = store[1:half - 2], store[half + 1:n - 2]
+    rdo2 = torch.zeros((3, C), dtype=torch.int64, device="cuda")
+    gpmap.robustness_cross(ph[1:half - 2], ph[half + 1:n - 2], C, rdo2, None)
+    ok = mine != 0xFFFF
+    want = [np.bincount(mine[ok & sel], minlength=C) for sel in (theirs == mine, theirs == 0xFFFF, (theirs != mine) & (theirs != 0xFFFF))]
+    assert np.array_equal(rdo2.cpu().numpy(), np.stack(want))
+
+
 def _rank_main(rank, world, port, out):
     """One rank of a two-process run on the same device: libgpmap for every kernel, torch.distributed (gloo, device
     shards staged through the host) for every exchange.  The two processes never wait for each other inside a kernel."""
