@@ -71,7 +71,7 @@ def test_cross_shard_flip_with_the_shared_memory_class_table(C, hot):
     that start one entry late (scalar loads, ragged count), against the definition written out in numpy."""
     from oracle import gp_oracle as orc
     rng = np.random.default_rng(C)
-    n_bits = 21
+    n_bits = 22   # 2^21 entries per shard over 148 blocks: the hot classes pass every field's half mark in every block
     n = 1 << n_bits
     store = rng.integers(0, C, size=n).astype(np.uint16)
     pick = rng.random(n) < hot
