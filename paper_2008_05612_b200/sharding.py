@@ -41,12 +41,6 @@ def shard_range(n_bits, world, rank, align=1):
     return min(lo, total), max(0, min(hi, total) - min(lo, total))
 
 
-def prefix_tiles(n_bits, tile_bits, world, rank):
-    """Round-robin assignment of the 2^(n_bits-tile_bits) prefix tiles to ranks: tile t goes to rank t % world."""
-    n = 1 << max(0, n_bits - tile_bits)
-    return [t << tile_bits for t in range(rank, n, world)]
-
-
 class LibOps:
     """libgpmap's reductions on CUDA tensors (argument marshalling only)."""
 
@@ -193,20 +187,3 @@ def exchange_bytes_per_rank(n_bits, world, n_classes):
     one pair bitmap."""
     q = log2_exact(world)
     return q * (2 << (n_bits - q)) + 8 * (4 * n_classes + 1) + 4 * ((n_classes * n_classes + 31) // 32)
-
-
-# kept for callers that only need the count reduction (bench.py weak-scaling tiles)
-def reduce_counts(*tensors, group=None):
-    """Sum per-class count tensors (hist, R, D, O ...) over all ranks, in place; returns them."""
-    if dist.is_available() and dist.is_initialized() and dist.get_world_size(group) > 1:
-        for t in tensors:
-            dist.all_reduce(t, op=dist.ReduceOp.SUM, group=group)
-    return tensors
-
-
-def max_over_ranks(value, device="cpu", group=None):
-    """Max of a python float over ranks (device timings are reported as the max over ranks)."""
-    t = torch.tensor([float(value)], dtype=torch.float64, device=device)
-    if dist.is_available() and dist.is_initialized() and dist.get_world_size(group) > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX, group=group)
-    return float(t.item())

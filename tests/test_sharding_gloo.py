@@ -53,8 +53,6 @@ def test_shard_ranges_cover_the_map_and_are_aligned():
             assert b == pos and b % align == 0
             pos = b + c
         assert pos == 1 << n_bits
-    tiles = [t for r in range(3) for t in sharding.prefix_tiles(10, 6, 3, r)]
-    assert sorted(tiles) == [t << 6 for t in range(16)]
     with pytest.raises(ValueError):
         sharding.log2_exact(3)
     assert sharding.exchange_bytes_per_rank(36, 8, 28728) == 3 * (2 << 33) + 8 * (4 * 28728 + 1) + 4 * ((28728 ** 2 + 31) // 32)
