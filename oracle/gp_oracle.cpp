@@ -298,6 +298,16 @@ void oracle_seeded_sequences(uint64_t seed, uint64_t first, uint64_t count, int 
             seqs[n * N + k] = (uint8_t)(((u >> 32) * 20) >> 32);
         }
 }
+// the same stream cut into `alphabet` letters (letter = floor(alphabet * hi32(draw) / 2^32); alphabet
+// 20 is oracle_seeded_sequences, alphabet 2 — the paper's random H/P sampling runs, PAPER.md:195-204, :762-775 — takes
+// the top bit of the draw, 1 = H)
+void oracle_seeded_letters(uint64_t seed, uint64_t first, uint64_t count, int N, int alphabet, uint8_t* seqs) {
+    for (uint64_t n = 0; n < count; n++)
+        for (int k = 0; k < N; k++) {
+            uint64_t u = draw(seed, (first + n) * 64 + (uint64_t)k);
+            seqs[n * N + k] = (uint8_t)(((u >> 32) * (uint64_t)alphabet) >> 32);
+        }
+}
 // symmetric 20x20 matrix, entries -750..-50 (units of 0.01)
 void oracle_seeded_matrix(uint64_t seed, int32_t* M /*400*/) {
     for (int a = 0; a < 20; a++)

@@ -54,6 +54,7 @@ def lib():
         L.oracle_draw.restype = ctypes.c_uint64
         L.oracle_draw.argtypes = [ctypes.c_uint64, ctypes.c_uint64]
         L.oracle_seeded_sequences.argtypes = [ctypes.c_uint64, ctypes.c_uint64, ctypes.c_uint64, ctypes.c_int, u8p]
+        L.oracle_seeded_letters.argtypes = [ctypes.c_uint64, ctypes.c_uint64, ctypes.c_uint64, ctypes.c_int, ctypes.c_int, u8p]
         L.oracle_seeded_matrix.argtypes = [ctypes.c_uint64, i32p]
         L.oracle_designability.argtypes = [u16p, ctypes.c_uint64, ctypes.c_uint32, u64p]
         L.oracle_robustness.argtypes = [u16p, ctypes.c_int, ctypes.c_uint32, u64p, u64p, u64p, u64p]
@@ -139,6 +140,13 @@ def draw(seed, ctr):
 def seeded_sequences(seed, first, count, N):
     seqs = np.zeros((count, N), np.uint8)
     lib().oracle_seeded_sequences(seed, first, count, N, _p(seqs, ctypes.c_uint8))
+    return seqs
+
+
+def seeded_letters(seed, first, count, N, alphabet):
+    """Sequences first..first+count-1 of the DESIGN.md section 4 stream over `alphabet` letters (2 = random H/P)."""
+    seqs = np.zeros((count, N), np.uint8)
+    lib().oracle_seeded_letters(seed, first, count, N, alphabet, _p(seqs, ctypes.c_uint8))
     return seqs
 
 

@@ -177,3 +177,23 @@ def test_generator():
     assert (M == M.T).all() and M.min() >= -750 and M.max() <= -50 and len(np.unique(M)) > 100
     u = orc.draw(200805612, (1 << 62) + 3 * 20 + 7)
     assert M[3, 7] == -750 + (((u >> 32) * 701) >> 32)
+
+
+def test_generator_two_letters():
+    """The random H/P sampling sequences: the same splitmix stream cut
+    into two letters = the top bit of each draw.  Pinned by the published stream itself (draws 0..2 of seed 0 start
+    0xE2.., 0x6E.., 0x06..: letters 1, 0, 0), by the alphabet-20 routine (same counters: letter20 >= 10 <=> letter2 = 1), a
+    chi-square on the H fraction and on pairs of neighbouring letters, and range slicing."""
+    assert orc.seeded_letters(0, 0, 1, 3, 2).tolist() == [[1, 0, 0]]
+    s2 = orc.seeded_letters(200805612, 0, 40000, 36, 2)
+    s20 = orc.seeded_sequences(200805612, 0, 40000, 36)
+    assert s2.max() == 1 and ((s20 >= 10) == (s2 == 1)).all()
+    assert (orc.seeded_letters(200805612, 0, 300, 16, 20) == s20[:300, :16]).all()       # alphabet 20 is the old routine
+    n = s2.size
+    h = int(s2.sum())
+    assert abs(h - n / 2) < 4.0 * np.sqrt(n / 4)                                         # 4 sigma of a fair coin
+    pairs = np.bincount((s2[:, :-1] * 2 + s2[:, 1:]).reshape(-1), minlength=4)
+    assert float(((pairs - pairs.mean()) ** 2 / pairs.mean()).sum()) < 25.0              # 3 dof
+    assert (orc.seeded_letters(200805612, 777, 50, 36, 2) == s2[777:827]).all()
+    u = orc.draw(200805612, 9 * 64 + 35)
+    assert s2[9, 35] == u >> 63
