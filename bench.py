@@ -136,6 +136,9 @@ def peaks():
 PROFILE_CSV = os.path.join(ROOT, "profiles", "r3_scoring_ncu_raw.csv")
 
 
+ROB_WARP_INSTR_PER_FLIP = 0.285   # profiles/r2_robustness_ncu.md: (2.69e8 + 2.29e8) warp instructions / (2^26 x 26 genotype-flips)
+
+
 def folded_columns(mon):
     """Contraction columns the scoring kernel executes when the monomers `mon` stay free inside one weight image
     (DESIGN.md 6.1): 2 bias columns + the monomers + the monomer pairs that can touch (odd distance >= 3)."""
@@ -516,6 +519,10 @@ def run_rows(args):
             t = dev_time(lambda: S.enumerate_seqs(seqs[:c], ph[:c], None, e=e, alphabet=2), reps=1)
             rows.append(dict(row="f3 sampling, random HP sequences (%s)" % label, config="%s, %d sequences" % (name, c), seconds=t,
                              evals_per_s=c * S.D / t, seconds_per_sequence=t / c, paper_gpu_seconds_per_sequence=paper_hp))
+        S.tune(seq_tensor=1)
+        t = dev_time(lambda: S.enumerate_seeded(SEED, 0, cnt, ph, e=e, alphabet=2), reps=1)
+        rows.append(dict(row="f3 sampling, seeded HP sequences drawn on chip (tensor cores)", config="%s, %d sequences" % (name, cnt),
+                         seconds=t, evals_per_s=cnt * S.D / t, seconds_per_sequence=t / cnt, paper_gpu_seconds_per_sequence=paper_hp))
         M = gpmap.seeded_matrix(SEED)
         for label, on, c in (("tensor cores, two int8 limbs", 2, 1 << 20), ("CUDA cores", 0, 1 << 17)):
             S.tune(seq_tensor=on)
@@ -717,7 +724,7 @@ def run_ours(args):
     hs_ms, hs_n = ktime[gpmap.KERNEL_HIST]
     im_ms, im_n = ktime[gpmap.KERNEL_IMAGE]
     other = {
-        "robustness_kernel": {"bound": "alu (instruction-bound, DESIGN.md 6.4; the HBM figure is what one read of the store would need)", "algorithmic_GBps": 2.0 * n / (rb_ms / max(1, rb_n) * 1e-3) / 1e9 if rb_ms else None,
+        "robustness_kernel": {"bound": "hbm", "algorithmic_GBps": 2.0 * n / (rb_ms / max(1, rb_n) * 1e-3) / 1e9 if rb_ms else None,
                               "peak": hbm, "avg_launch_ms": rb_ms / max(1, rb_n), "share_of_step": rb_ms / ms},
         "hist_kernel": {"bound": "hbm", "algorithmic_GBps": 2.0 * n / (hs_ms / max(1, hs_n) * 1e-3) / 1e9 if hs_ms else None,
                         "peak": hbm, "avg_launch_ms": hs_ms / max(1, hs_n), "share_of_step": hs_ms / ms, "launches": int(hs_n),
@@ -728,7 +735,18 @@ def run_ours(args):
     }
     for kname in ("robustness_kernel", "hist_kernel"):
         if other[kname]["algorithmic_GBps"]:
-            other[kname]["frac"] = other[kname]["algorithmic_GBps"] / hbm
+            other[kname]["frac_of_hbm"] = other[kname]["algorithmic_GBps"] / hbm
+    if rb_ms:
+        # the neighbour pass is bound by instruction issue, not HBM.  Peak = 4 schedulers x 148 SMs x one
+        # warp instruction per clock at the clock sampled in this run; the kernel's cost is 0.285 warp instructions per
+        # genotype-flip (profiles/r2_robustness_ncu.md: 4.98e8 warp instructions for the 2^26 x 26 flips of this tile)
+        sm_clk = (clocks or {}).get("sm_mhz") or 1965.0
+        issue_peak = 4.0 * 148 * sm_clk * 1e6
+        flips_per_s = float(n) * G * args.steps / (rb_ms * 1e-3)
+        other["robustness_kernel"].update({"bound": "alu", "unit": "warp instructions/s", "peak": issue_peak,
+                                           "achieved": flips_per_s * ROB_WARP_INSTR_PER_FLIP, "frac": flips_per_s * ROB_WARP_INSTR_PER_FLIP / issue_peak,
+                                           "genotype_flips_per_s": flips_per_s, "warp_instr_per_flip": ROB_WARP_INSTR_PER_FLIP,
+                                           "hbm_peak": hbm})
 
     whole = None
     if world == 1 and not args.full and not args.no_whole_map:

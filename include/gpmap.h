@@ -151,13 +151,16 @@ gp_status gp_enumerate_simple(const gp_structures_t* s, const gp_energies* en, u
  * The first call on a handle that needs an image allocates it (cudaMalloc). */
 gp_status gp_enumerate_seqs(const gp_structures_t* s, const gp_energies* en, const uint8_t* d_seqs, uint64_t count,
                             uint16_t* d_pheno, int16_t* d_gap, void* stream);
-/* a8. Sequences first..first+count-1 of the counter-based 20-letter generator of DESIGN.md section 4, drawn on chip; same
- * kernel choice as gp_enumerate_seqs. */
+/* a8 / f3. Sequences first..first+count-1 of the counter-based generator of DESIGN.md section 4 over en->alphabet letters
+ * (2..20), drawn on chip ("generation of random numbers on the GPU"): alphabet 20 with the seeded matrix is
+ * BASELINE config 5, alphabet 2 the random H/P sampling runs (:195-204 Table 3 HP rows) with no sequence upload.  Same
+ * kernel choice and same results as gp_enumerate_seqs on gp_seeded_letters(seed, first, count, N, alphabet). */
 gp_status gp_enumerate_seeded(const gp_structures_t* s, const gp_energies* en, uint64_t seed, uint64_t first,
                               uint64_t count, uint16_t* d_pheno, int16_t* d_gap, void* stream);
 /* Host helpers for the same generator: the seeded 20x20 matrix and sequences. */
 gp_status gp_seeded_matrix(uint64_t seed, int32_t* m400);
-gp_status gp_seeded_sequences(uint64_t seed, uint64_t first, uint64_t count, int n, uint8_t* seqs);
+gp_status gp_seeded_sequences(uint64_t seed, uint64_t first, uint64_t count, int n, uint8_t* seqs);                /* 20 letters */
+gp_status gp_seeded_letters(uint64_t seed, uint64_t first, uint64_t count, int n, int alphabet, uint8_t* seqs);   /* 2..20 */
 
 /* a5. Designability (:138): d_hist[c] = #{g : d_pheno[g] = c} for c < n_classes, d_hist[n_classes] = #null. */
 gp_status gp_designability(const uint16_t* d_pheno, uint64_t count, uint32_t n_classes, uint64_t* d_hist, void* stream);

@@ -260,6 +260,13 @@ extern "C" gp_status gp_seeded_sequences(uint64_t seed, uint64_t first, uint64_t
     return GP_OK;
 }
 
+extern "C" gp_status gp_seeded_letters(uint64_t seed, uint64_t first, uint64_t count, int n, int alphabet, uint8_t* seqs) {
+    if (!seqs || n < 1 || n > 64 || alphabet < 2 || alphabet > 20) return GP_INVALID_ARG;
+    for (uint64_t q = 0; q < count; q++)
+        for (int k = 0; k < n; k++) seqs[q * n + k] = (uint8_t)gp_letter(seed, first + q, k, (uint32_t)alphabet);
+    return GP_OK;
+}
+
 // End-to-end call from host buffers: device store allocated here, results copied back.
 extern "C" gp_status gp_enumerate_host(const gp_structures_t* s, const gp_energies* en, uint64_t g_begin,
                                        uint64_t g_count, uint16_t* pheno, uint64_t* hist, uint64_t* rdo,

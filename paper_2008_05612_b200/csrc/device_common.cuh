@@ -63,16 +63,19 @@ __host__ __device__ inline uint64_t gp_mix64(uint64_t z) {
 __host__ __device__ inline uint64_t gp_draw(uint64_t seed, uint64_t ctr) {
     return gp_mix64(seed + (ctr + 1) * 0x9E3779B97F4A7C15ULL);
 }
-__host__ __device__ inline uint32_t gp_letter20(uint64_t seed, uint64_t seq, int k) {
+// letter k of sequence seq over `alphabet` letters: floor(alphabet * hi32(draw) / 2^32); alphabet 2 = the top bit, 1 = H
+__host__ __device__ inline uint32_t gp_letter(uint64_t seed, uint64_t seq, int k, uint32_t alphabet) {
     uint64_t u = gp_draw(seed, seq * 64 + (uint64_t)k);
-    return (uint32_t)(((u >> 32) * 20) >> 32);
+    return (uint32_t)(((u >> 32) * alphabet) >> 32);
 }
+__host__ __device__ inline uint32_t gp_letter20(uint64_t seed, uint64_t seq, int k) { return gp_letter(seed, seq, k, 20u); }
 
 // scoring_tc.cu
 gp_status gp_launch_scoring_tc(const gp_structures_s* s, const gp_hp_params& hp, uint64_t g_begin, uint64_t g_count,
                                uint16_t* d_pheno, int16_t* d_gap, cudaStream_t st);
-gp_status gp_launch_sequences_tc(const gp_structures_s* s, const gp_hp_params& hp, const uint8_t* d_seqs, uint64_t count,
-                                 uint16_t* d_pheno, int16_t* d_gap, cudaStream_t st);
+// d_seqs = NULL: the two-letter sequences first .. first+count-1 of the seeded stream, drawn on chip
+gp_status gp_launch_sequences_tc(const gp_structures_s* s, const gp_hp_params& hp, const uint8_t* d_seqs, uint64_t seed,
+                                 uint64_t first, uint64_t count, uint16_t* d_pheno, int16_t* d_gap, cudaStream_t st);
 // scoring_seq20.cu
 gp_status gp_launch_seq20_tc(const gp_structures_s* s, const gp_energies* en, int seeded, const uint8_t* d_seqs, uint64_t seed,
                              uint64_t first, uint64_t count, uint16_t* d_pheno, int16_t* d_gap, cudaStream_t st);

@@ -215,7 +215,7 @@ __global__ void __launch_bounds__(Q_THREADS, 1) seq20_kernel(const QArgs a) {
             const uint64_t q = (uint64_t)item * Q_ROWS + r;
             for (int i = 0; i < a.N; i++) {   // the row's four threads each need all letters: every one writes the same bytes
                 uint32_t l = 0;
-                if (q < a.count) l = SRC == QSRC_SEQS ? a.seqs[q * a.N + i] : gp_letter20(a.seed, a.first + q, i);
+                if (q < a.count) l = SRC == QSRC_SEQS ? a.seqs[q * a.N + i] : gp_letter(a.seed, a.first + q, i, (uint32_t)a.alphabet);
                 my_let[i * Q_ROWS] = (uint8_t)min(l, (uint32_t)a.alphabet - 1u);  // a letter outside the alphabet counts as the last one
             }
             mbar_wait(&bar->a_empty, (item_no & 1) ^ 1);

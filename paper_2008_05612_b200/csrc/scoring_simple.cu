@@ -54,7 +54,7 @@ __global__ void __launch_bounds__(128) score_simple_kernel(SimpleArgs a, const i
                 if (live[h]) {
                     if (SRC == SRC_BITS) l = (uint32_t)(((a.first + q[h]) >> k) & 1ULL);
                     else if (SRC == SRC_SEQS) l = min((uint32_t)a.seqs[q[h] * a.N + k], (uint32_t)a.alphabet - 1u);  // outside the alphabet = the last letter
-                    else l = gp_letter20(a.seed, a.first + q[h], k);
+                    else l = gp_letter(a.seed, a.first + q[h], k, (uint32_t)a.alphabet);
                 }
                 let[(k * 2 + h) * BD + tid] = (uint8_t)l;
             }
@@ -98,7 +98,6 @@ gp_status launch_simple(const gp_structures_s* s, const gp_energies* en, int src
                         uint64_t first, uint64_t count, uint16_t* d_pheno, int16_t* d_gap, cudaStream_t st) {
     if (!s || !en || !en->e || !d_pheno) return GP_INVALID_ARG;
     if (en->alphabet < 2 || en->alphabet > 20 || en->threshold < 1) return GP_INVALID_ARG;
-    if (src == SRC_SEEDED && en->alphabet != 20) return GP_INVALID_ARG;
     if (src == SRC_SEQS && !d_seqs) return GP_INVALID_ARG;
     if (s->device < 0) { gp_set_cuda_error(cudaErrorNoDevice, "handle has no device tables"); return GP_CUDA_ERROR; }
     const int A = en->alphabet;
@@ -164,7 +163,7 @@ static gp_status seqs_any_alphabet(const gp_structures_t* s, const gp_energies* 
     // CUDA-core kernel is 3x faster; 6x6 / 3x3x3: the tensor cores are 20x faster)
     const bool want_tc = s && (s->tuning.seq_tensor == 2 || (s->tuning.seq_tensor == 1 && s->D >= 4096));
     if (want_tc && en && en->e && d_pheno && count >= 128 && s->device >= 0 && en->alphabet >= 2 &&
-        en->alphabet <= 20 && en->threshold >= 1 && (seeded ? en->alphabet == 20 : d_seqs != nullptr)) {
+        en->alphabet <= 20 && en->threshold >= 1 && (seeded || d_seqs != nullptr)) {
         bool symmetric = true;
         for (int i = 0; i < en->alphabet && symmetric; i++)
             for (int j = 0; j < i; j++)
@@ -183,7 +182,7 @@ extern "C" gp_status gp_enumerate_seqs(const gp_structures_t* s, const gp_energi
     gp_hp_params hp;
     if (s && s->tuning.seq_tensor && en && en->alphabet == 2 && d_seqs && d_pheno && count >= 256 && s->device >= 0 &&
         gp_check_hp(s, en, &hp) == GP_OK) {
-        gp_status st = gp_launch_sequences_tc(s, hp, d_seqs, count, d_pheno, d_gap, (cudaStream_t)stream);
+        gp_status st = gp_launch_sequences_tc(s, hp, d_seqs, 0, 0, count, d_pheno, d_gap, (cudaStream_t)stream);
         if (st != GP_UNSUPPORTED_LATTICE) return st;
     }
     return seqs_any_alphabet(s, en, 0, d_seqs, 0, 0, count, d_pheno, d_gap, (cudaStream_t)stream);
@@ -191,5 +190,12 @@ extern "C" gp_status gp_enumerate_seqs(const gp_structures_t* s, const gp_energi
 
 extern "C" gp_status gp_enumerate_seeded(const gp_structures_t* s, const gp_energies* en, uint64_t seed, uint64_t first,
                                          uint64_t count, uint16_t* d_pheno, int16_t* d_gap, void* stream) {
+    // seeded H/P sequences whose energies fit the int8 weights: sequence_kernel draws its feature rows from the counter
+    gp_hp_params hp;
+    if (s && s->tuning.seq_tensor && en && en->alphabet == 2 && d_pheno && count >= 256 && s->device >= 0 &&
+        gp_check_hp(s, en, &hp) == GP_OK) {
+        gp_status st = gp_launch_sequences_tc(s, hp, nullptr, seed, first, count, d_pheno, d_gap, (cudaStream_t)stream);
+        if (st != GP_UNSUPPORTED_LATTICE) return st;
+    }
     return seqs_any_alphabet(s, en, 1, nullptr, seed, first, count, d_pheno, d_gap, (cudaStream_t)stream);
 }

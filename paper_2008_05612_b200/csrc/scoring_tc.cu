@@ -528,7 +528,8 @@ __global__ void __launch_bounds__(TN) build_full_image_kernel(const SqImgArgs a)
 struct SqArgs {
     const int8_t* img;        // [n_tiles][SQ_KB][TILE_BYTES]
     const uint16_t* class_of;
-    const uint8_t* seqs;      // count x N letters (0 / 1)
+    const uint8_t* seqs;      // count x N letters (0 / 1); NULL: letters drawn from the seeded stream (seed, first)
+    uint64_t seed, first;
     uint16_t* pheno;
     int16_t* gap;             // nullable
     uint64_t count;
@@ -631,8 +632,12 @@ __global__ void __launch_bounds__(SQ_THREADS, 1) sequence_kernel(const SqArgs a,
         for (uint32_t item = blockIdx.x; item < a.n_items; item += gridDim.x, item_no++) {
             const uint64_t q = (uint64_t)item * SQ_ROWS + m * TM + r;
             unsigned long long h = 1ULL << 63;  // bit 63: the constant-1 feature; bit 62 stays 0 for unused columns
-            if (q < a.count)
-                for (int i = 0; i < a.N; i++) h |= (unsigned long long)(a.seqs[q * a.N + i] != 0) << i;  // a letter outside {0, 1} is the last letter, H (R19)
+            if (q < a.count) {
+                if (a.seqs)
+                    for (int i = 0; i < a.N; i++) h |= (unsigned long long)(a.seqs[q * a.N + i] != 0) << i;  // a letter outside {0, 1} is the last letter, H (R19)
+                else
+                    for (int i = 0; i < a.N; i++) h |= (unsigned long long)gp_letter(a.seed, a.first + q, i, 2u) << i;
+            }
             mbar_wait(&bar->a_empty, (item_no & 1) ^ 1);
 #pragma unroll 1
             for (uint32_t c16 = 0; c16 < SQ_MAXCOL / 16; c16++) {
@@ -1110,8 +1115,8 @@ extern "C" gp_status gp_enumerate_map(const gp_structures_t* s, const gp_energie
 
 // Explicit HP sequences on the tensor cores (sequence_kernel).  GP_UNSUPPORTED_LATTICE = this lattice needs more than
 // 384 columns: the caller falls back to the CUDA-core kernel.
-gp_status gp_launch_sequences_tc(const gp_structures_s* s, const gp_hp_params& hp, const uint8_t* d_seqs, uint64_t count,
-                                 uint16_t* d_pheno, int16_t* d_gap, cudaStream_t st) {
+gp_status gp_launch_sequences_tc(const gp_structures_s* s, const gp_hp_params& hp, const uint8_t* d_seqs, uint64_t seed,
+                                 uint64_t first, uint64_t count, uint16_t* d_pheno, int16_t* d_gap, cudaStream_t st) {
     using namespace tc;
     const int ncol = 2 + s->N + s->P;
     if (ncol > SQ_MAXCOL || s->N > 62 || s->D >= (1u << KEY_SHIFT)) return GP_UNSUPPORTED_LATTICE;
@@ -1171,7 +1176,7 @@ gp_status gp_launch_sequences_tc(const gp_structures_s* s, const gp_hp_params& h
     const size_t smem = (size_t)(SQ_MT + SQ_STAGES) * SQ_TILE + sizeof(SqBarriers) + sizeof(SqCols) + 1024 + 64;
     GP_CUDA(cudaFuncSetAttribute(sequence_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     SqArgs a;
-    a.img = d_img; a.class_of = s->d_class_of; a.seqs = d_seqs; a.pheno = d_pheno; a.gap = d_gap; a.count = count;
+    a.img = d_img; a.class_of = s->d_class_of; a.seqs = d_seqs; a.seed = seed; a.first = first; a.pheno = d_pheno; a.gap = d_gap; a.count = count;
     a.n_items = (uint32_t)((count + SQ_ROWS - 1) / SQ_ROWS); a.n_tiles = n_tiles;
     a.N = s->N; a.ksteps = (ncol + 31) / 32; a.threshold = hp.threshold;
     const unsigned grid = a.n_items < (uint32_t)sms ? a.n_items : (uint32_t)sms;

@@ -55,6 +55,7 @@ SIGNATURES = {
                                            ctypes.c_uint64, _vp, _vp, _vp]),
     "gp_seeded_matrix": (ctypes.c_int, [ctypes.c_uint64, _i32p]),
     "gp_seeded_sequences": (ctypes.c_int, [ctypes.c_uint64, ctypes.c_uint64, ctypes.c_uint64, ctypes.c_int, _u8p]),
+    "gp_seeded_letters": (ctypes.c_int, [ctypes.c_uint64, ctypes.c_uint64, ctypes.c_uint64, ctypes.c_int, ctypes.c_int, _u8p]),
     "gp_designability": (ctypes.c_int, [_vp, ctypes.c_uint64, ctypes.c_uint32, _vp, _vp]),
     "gp_robustness": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_uint32, _vp, _vp, _vp, _vp, _vp]),
     "gp_reduce_store": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_uint32, _vp, _vp, _vp, _vp, _vp, _vp]),
@@ -294,9 +295,11 @@ class Structures:
                                        _dptr(pheno, torch.uint16), _dptr(gap, torch.int16), _stream(stream)),
                "gp_enumerate_seqs")
 
-    def enumerate_seeded(self, seed, first, count, pheno, gap=None, e=None, threshold=1, stream=None):
+    def enumerate_seeded(self, seed, first, count, pheno, gap=None, e=None, threshold=1, stream=None, alphabet=20):
+        """gp_enumerate_seeded: sequences first..first+count-1 of the seeded stream over `alphabet` letters, drawn on chip
+        (alphabet 2: random H/P sequences, e = the 2x2 energies)."""
         import torch
-        en = _energies(e, 20, threshold)
+        en = _energies(e, alphabet, threshold)
         _check(lib().gp_enumerate_seeded(self._h, ctypes.byref(en), seed, first, count, _dptr(pheno, torch.uint16),
                                          _dptr(gap, torch.int16), _stream(stream)), "gp_enumerate_seeded")
 
@@ -330,6 +333,13 @@ def seeded_matrix(seed):
 def seeded_sequences(seed, first, count, n):
     s = np.zeros((count, n), np.uint8)
     _check(lib().gp_seeded_sequences(seed, first, count, n, s.ctypes.data_as(_u8p)), "gp_seeded_sequences")
+    return s
+
+
+def seeded_letters(seed, first, count, n, alphabet):
+    """Host copy of the stream gp_enumerate_seeded draws on chip, over `alphabet` letters (gp_seeded_letters)."""
+    s = np.zeros((count, n), np.uint8)
+    _check(lib().gp_seeded_letters(seed, first, count, n, alphabet, s.ctypes.data_as(_u8p)), "gp_seeded_letters")
     return s
 
 

@@ -143,6 +143,9 @@ def test_seeded_generator_matches_recipe():
         assert np.array_equal(gpmap.seeded_matrix(seed), orc.seeded_matrix(seed))
         assert np.array_equal(gpmap.seeded_sequences(seed, 12345, 300, 16), orc.seeded_sequences(seed, 12345, 300, 16))
         assert np.array_equal(gpmap.seeded_sequences(seed, 1 << 40, 50, 36), orc.seeded_sequences(seed, 1 << 40, 50, 36))
+        for alphabet in (2, 3, 20):
+            assert np.array_equal(gpmap.seeded_letters(seed, 999, 200, 36, alphabet), orc.seeded_letters(seed, 999, 200, 36, alphabet))
+    assert gpmap.lib().gp_seeded_letters(1, 0, 1, 16, 21, np.zeros(16, np.uint8).ctypes.data_as(gpmap._u8p)) == 1
     M = gpmap.seeded_matrix(200805612)
     assert M.min() >= -750 and M.max() <= -50 and np.array_equal(M, M.T)
 

@@ -441,3 +441,32 @@ def test_letters_outside_the_alphabet_on_every_sequence_kernel(oracle_structures
                     assert np.array_equal(gap.cpu().numpy().astype(np.int32), gap_o[:count]), (dims, alphabet, tensor, count)
         finally:
             S.tune(seq_tensor=1)
+
+
+@pytest.mark.parametrize("dims,count", [((6, 6, 1), 2500), ((3, 3, 3), 1200), ((4, 4, 1), 700)])
+def test_seeded_hp_sequences_drawn_on_chip(oracle_structures, dims, count):
+    """The paper's HP sampling runs with the sequences drawn on the GPU (Table 3 HP rows,
+    :762-775; the top bit of each draw): gp_enumerate_seeded with alphabet 2 against the oracle on the
+    oracle's own copy of the stream — ids and gaps, a first sequence that is not 0, every kernel the call can pick
+    (sequence_kernel from 256 sequences on, seq20_kernel from 128, the CUDA-core kernel), a threshold, and other energies."""
+    S, O = lib_structures(dims), oracle_structures(*dims)
+    seed, first = 200805612, (1 << 33) + 12345
+    seqs = orc.seeded_letters(seed, first, count, S.N, 2)
+    for e, thr in ((np.array(gpmap.HP_ENERGIES, np.int32), 1), (np.array([1, -7, -7, -19], np.int32), 3)):
+        ph_o, gap_o = O.enumerate_seqs(seqs, e, 2, threshold=thr)
+        try:
+            for tensor in (1, 2, 0):
+                S.tune(seq_tensor=tensor)
+                for c in (count, 200, 100):
+                    ph = torch.empty(c, dtype=torch.uint16, device="cuda")
+                    gap = torch.empty(c, dtype=torch.int16, device="cuda")
+                    S.enumerate_seeded(seed, first, c, ph, gap, e=e, threshold=thr, alphabet=2)
+                    assert np.array_equal(ph.cpu().numpy(), ph_o[:c]), (dims, tensor, c)
+                    assert np.array_equal(gap.cpu().numpy().astype(np.int32), gap_o[:c]), (dims, tensor, c)
+        finally:
+            S.tune(seq_tensor=1)
+    # the explicit-sequence call on the library's host copy of the stream gives the same phenotypes
+    d_seqs = torch.from_numpy(gpmap.seeded_letters(seed, first, count, S.N, 2)).cuda()
+    a = torch.empty(count, dtype=torch.uint16, device="cuda")
+    S.enumerate_seqs(d_seqs, a, None, e=np.array(gpmap.HP_ENERGIES, np.int32), alphabet=2)
+    assert np.array_equal(a.cpu().numpy(), O.enumerate_seqs(seqs, np.array(gpmap.HP_ENERGIES, np.int32), 2, want_gap=False))
